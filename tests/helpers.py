@@ -1,0 +1,121 @@
+"""Test-side glue: feeds the seeded workloads to the fp64 oracle, carves top-k margins, compares.
+
+Lives in tests/ because it calls oracle/ (only tests, smoke() and bench.py's CPU legs may).
+"""
+from __future__ import annotations
+
+import copy
+
+import numpy as np
+
+from oracle import sx_oracle as orc
+from paper_2606_01751_b200 import workloads as wl
+
+# tolerances fixed by BASELINE.json north_star (bf16 in / fp32 accumulate vs fp64)
+MAX_ABS = 2e-2
+MEAN_ABS = 2e-3
+# reading A12: on rows whose |value| exceeds 2.56 one bf16 ulp is already > 2e-2; per-element bound
+# max(2e-2, 2^-7 |ref|) (2^-7 |ref| >= one bf16 ulp of ref).
+BF16_ULP_REL = 2.0 ** -7
+
+
+def oracle_layer(lay: wl.Layout, lt: wl.LayerTensors, mode="sparse", rows_given=None, tables=None,
+                 k_per_req=None):
+    """Run the oracle layer driver on COPIES of the pool/tables. Returns (result, pool_k, pool_v, kt, vt)."""
+    pk, pv = lt.pool_k.copy(), lt.pool_v.copy()
+    if tables is None:
+        kt, vt = lay.k_block_table.copy(), lay.v_block_table.copy()
+    else:
+        kt, vt = tables[0].copy(), tables[1].copy()
+    res = orc.layer_step(pk, pv, kt, vt, lay.cow_private if lay.cow else None, lay.segments,
+                         lay.src_blocks, lay.rope_theta, lay.rope_style, lay.seq_len, lay.tok_off,
+                         lay.new_off, lay.new_idx, lay.k_per_req if k_per_req is None else k_per_req,
+                         lay.num_q_heads, lt.q_full, lt.k_fresh, lt.v_fresh, mode=mode,
+                         rows_given=rows_given)
+    return res, pk, pv, kt, vt
+
+
+def oracle_scores_after_realign(lay: wl.LayerTensors, lt: wl.LayerTensors):
+    """fp64 scores of every request on the pool state stage (b) sees: realign + scatter(I_nr)."""
+    pk, pv = lt.pool_k.copy(), lt.pool_v.copy()
+    kt, vt = lay.k_block_table.copy(), lay.v_block_table.copy()
+    orc.realign(pk, pv, kt, vt, lay.segments, lay.src_blocks, lay.rope_theta, lay.rope_style)
+    out = []
+    for r in range(lay.num_reqs):
+        t, o = int(lay.seq_len[r]), int(lay.tok_off[r])
+        nidx = lay.new_idx[lay.new_off[r]:lay.new_off[r + 1]]
+        orc.scatter_kv(pk, pv, kt, vt, None, r, nidx, lt.k_fresh[o + nidx], lt.v_fresh[o + nidx])
+        out.append(orc.scores(pk, kt[r], t, lt.q_full[o + nidx], nidx, lay.num_q_heads))
+    return out
+
+
+def carve_margins(lay: wl.Layout, lt: wl.LayerTensors, tau: float = 1e-3, max_iter: int = 12):
+    """Reading A9/A10: the x4 salient tokens alone do not make the rank-k cut unambiguous
+    (ratio > salient fraction, the cut falls among ordinary tokens). Enforce a relative margin at the
+    cut: every cached token whose fp64 score lies within tau of the midpoint c between ranks k and k+1
+    has its SOURCE key row rescaled (x1.25 above the cut, x0.8 below), re-rounded to bf16; repeat until
+    the band is empty and the gap is >= 2 tau. Modifies lt.pool_k in place; returns per-iteration band
+    sizes. Uses the oracle, hence lives in tests/.
+    """
+    hist = []
+    bs = wl.PAGE
+    for _ in range(max_iter):
+        sc = oracle_scores_after_realign(lay, lt)
+        band_total = 0
+        for r in range(lay.num_reqs):
+            k = int(lay.k_per_req[r])
+            is_new = lay.is_new_mask(r)
+            cand = np.nonzero(~is_new)[0]
+            if k <= 0 or k >= len(cand):
+                continue
+            s = sc[r][cand]
+            order = np.lexsort((cand, -s))
+            c = 0.5 * (s[order[k - 1]] + s[order[k]])
+            gap_ok = (s[order[k - 1]] - s[order[k]]) >= 2 * tau * c
+            band = np.nonzero(np.abs(s - c) <= tau * c)[0]
+            if gap_ok and len(band) == 0:
+                continue
+            if len(band) == 0:          # gap too small but nobody inside the band: push the two neighbours
+                band = np.asarray([order[k - 1], order[k]])
+            band_total += len(band)
+            # map position -> (segment, offset) -> source page row
+            for bi in band.tolist():
+                pos = int(cand[bi])
+                scale = 1.25 if s[bi] > c else 0.8
+                for sidx in range(lay.num_segments):
+                    rq, ln, _, new_pos, src_off = (int(v) for v in lay.segments[sidx])
+                    if rq == r and new_pos <= pos < new_pos + ln:
+                        j = pos - new_pos
+                        blk = int(lay.src_blocks[src_off + j // bs])
+                        row = orc.bf16_to_f64(lt.pool_k[blk, :, j % bs, :]) * scale
+                        lt.pool_k[blk, :, j % bs, :] = orc.f64_to_bf16(row)
+                        break
+        hist.append(band_total)
+        if band_total == 0:
+            return hist
+    raise RuntimeError("margin carving did not converge: %r" % hist)
+
+
+def check_close(name, got, ref64, max_abs=MAX_ABS, mean_abs=MEAN_ABS, ulp_floor=False):
+    """Tolerance of BASELINE.json north_star. With ulp_floor the per-element bound is
+    max(max_abs, 2^-7 |ref|) (reading A12: one bf16 ulp on the x4 salient key rows)."""
+    got = np.asarray(got, dtype=np.float64)
+    ref64 = np.asarray(ref64, dtype=np.float64)
+    assert got.shape == ref64.shape, (name, got.shape, ref64.shape)
+    if got.size == 0:
+        return 0.0, 0.0
+    err = np.abs(got - ref64)
+    bound = np.full_like(err, max_abs)
+    if ulp_floor:
+        bound = np.maximum(bound, BF16_ULP_REL * np.abs(ref64))
+    worst = float(err.max())
+    mean = float(err.mean())
+    assert np.all(np.isfinite(got)), name + ": non-finite output"
+    assert np.all(err <= bound), "%s: max-abs %.4g exceeds bound (n_bad=%d)" % (
+        name, worst, int((err > bound).sum()))
+    assert mean <= mean_abs, "%s: mean-abs %.4g > %.4g" % (name, mean, mean_abs)
+    return worst, mean
+
+
+def clone_layer(lt: wl.LayerTensors) -> wl.LayerTensors:
+    return copy.deepcopy(lt)
