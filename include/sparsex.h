@@ -1,0 +1,166 @@
+/*
+ * sparsex.h -- C ABI of the B200 (sm_100a) Sparse-KV recomputation step of SparseX
+ * (arxiv/paper_2606_01751). Citations are PAPER.md line numbers (+ section / equation / Algorithm 1).
+ *
+ * One layer of the method is four stages over a paged bf16 KV pool (BASELINE.json north_star):
+ *   (a) sx_rope_realign  k^_{p'+j} <- R_{p'-p} k^_{p+j}, v^ copied      PAPER.md:151-165 (S3.1), Alg. 1 l.502-504
+ *   (b) sx_score_select  A_sq = softmax(Q_sq K^T/sqrt(d) + M_causal)      Eq. (1)
+ *                        s_j = sum_heads sum_{i in I_nr} A_sq[i,j]         Eq. (2)
+ *                        S_key = TopK(s, k) over cached positions          Eq. (3)
+ *                        R = I_nr U S_key                                  Alg. 1 l.537-539
+ *   (c) sx_sparse_attn   O[R] = SparseAttn(Q[R], K_cur[1:T], V_cur[1:T])   Alg. 1 l.546-548 (full mode: l.507-511)
+ *   (d) sx_scatter_kv    write fresh K,V of the computed rows into pages   Alg. 1 l.509-510, 544-545
+ *
+ * Conventions
+ *   - "device" pointers are CUDA device memory owned by the caller; "host" values are plain integers
+ *     in the structs below. The library allocates nothing, frees nothing and keeps no state.
+ *   - Every call is asynchronous on `stream` and never synchronises the device. A non-zero status
+ *     means nothing was launched (argument errors) or a launch failed (SX_ERR_CUDA);
+ *     sx_last_error() then returns a thread-local description.
+ *   - bf16 tensors are raw 16-bit patterns. All device pointers must be 16-byte aligned.
+ *   - head_dim must be 128 and block_size 16 (SX_ERR_UNSUPPORTED otherwise);
+ *     num_q_heads % num_kv_heads == 0, group size g = Hq/Hkv <= 128.
+ *   - Positions are 0-based; the query at absolute position i sees keys j <= i (Eq. 1 M_causal).
+ *   - Same inputs => bit-identical outputs (no floating-point atomics anywhere).
+ *   - There is no CPU fallback: without a CUDA device every stage call returns SX_ERR_CUDA.
+ */
+#ifndef SPARSEX_H_
+#define SPARSEX_H_
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef enum {
+  SX_OK = 0,
+  SX_ERR_INVALID_ARG = -1, /* null pointer, negative size, inconsistent counts                 */
+  SX_ERR_UNSUPPORTED = -2, /* head_dim != 128, block_size != 16, bad head grouping, bad style  */
+  SX_ERR_WORKSPACE = -3,   /* ws_bytes smaller than sx_workspace_size()                        */
+  SX_ERR_CUDA = -4,        /* a CUDA runtime / driver call or a launch failed                  */
+  SX_ERR_MISALIGNED = -5   /* a device pointer is not 16-byte aligned                          */
+} sx_status;
+
+typedef struct CUstream_st *sx_stream; /* a cudaStream_t / CUstream; NULL = legacy default stream */
+
+/* Paged KV pool of ONE layer (a block holds the K/V of block_size tokens).
+ * Layout chosen here (the paper fixes none): separate K and V arrays, each
+ *   bf16 [num_blocks][num_kv_heads][block_size=16][head_dim=128]
+ * so that one (page, kv head) tile is 4 KB contiguous = 16 rows of 256 B. */
+typedef struct {
+  void *k;            /* device */
+  void *v;            /* device */
+  int32_t num_blocks; /* host */
+  int32_t block_size; /* host, must be 16 */
+  int32_t num_kv_heads;
+  int32_t num_q_heads;
+  int32_t head_dim;   /* host, must be 128 */
+} sx_pool;
+
+/* One reused segment S_m of one request (Alg. 1 inputs l.497, l.502).
+ * len, old_pos (p_m) and new_pos (p'_m) are multiples of block_size (segment
+ * boundaries are padded to the block size). delta = new_pos - old_pos may be negative or zero.
+ * src_off indexes src_blocks[]; segments must be stored so that src_off is the running sum of
+ * len/block_size of the segments before it (segment i's pages follow segment i-1's). */
+typedef struct {
+  int32_t req;
+  int32_t len;
+  int32_t old_pos;
+  int32_t new_pos;
+  int32_t src_off;
+} sx_segment;
+
+/* Block-table / segment-map descriptor of one scheduling batch (scheduler output of PAPER.md:333:
+ * request layout, block table, slot mapping, sparse mask). Host fields mirror sizes so that grids
+ * can be sized without reading device memory. */
+typedef struct {
+  /* host mirrors */
+  int32_t num_reqs;
+  int32_t num_segments;
+  int32_t max_pages_per_req; /* row pitch of the block tables                                   */
+  int32_t total_tokens;      /* sum_r T_r                                                        */
+  int32_t total_new;         /* sum_r |I_nr|                                                     */
+  int32_t total_seg_pages;   /* sum_m len_m / block_size                                         */
+  int32_t max_seq_len;       /* max_r T_r                                                        */
+  /* device arrays */
+  const int32_t *seq_len;    /* [num_reqs]     T_r (any value >= 1; last page may be partial)   */
+  const int32_t *tok_off;    /* [num_reqs+1]   prefix sum of seq_len                             */
+  int32_t *k_block_table;    /* [num_reqs][max_pages_per_req] logical page -> physical K page    */
+  int32_t *v_block_table;    /* same for V; may alias k_block_table; written only under COW      */
+  const int32_t *cow_private;/* [num_reqs][max_pages_per_req] reserved private page or -1; may be NULL */
+  const sx_segment *segments;/* [num_segments]                                                   */
+  const int32_t *src_blocks; /* [total_seg_pages] physical source pages (shared, never written)  */
+  const int32_t *new_off;    /* [num_reqs+1]   CSR offsets into new_idx                          */
+  const int32_t *new_idx;    /* [total_new]    sorted positions of I_nr per request (sparse mask m_i = 1) */
+  /* RoPE: theta_i = rope_theta^(-2i/head_dim); rotation by angle delta*theta_i */
+  double rope_theta;         /* host */
+  int32_t rope_style;        /* host: 0 = pairs (i, i+head_dim/2) ("half-split"), 1 = pairs (2i, 2i+1) */
+} sx_batch;
+
+/* Bytes of caller-provided workspace that any stage call on (pool, batch) may need. Host only. */
+sx_status sx_workspace_size(const sx_pool *pool, const sx_batch *batch, size_t *bytes);
+
+/* (a) PAPER.md:151-165, Alg. 1 l.502-504. For every segment m and token j < len:
+ *   K[k_block_table[req][(new_pos+j)/16]][h][(new_pos+j)%16][:] = RNE_bf16(R_{delta_m} K[src page][h][j%16][:])
+ *   V[v_block_table[...]] = V[src page] (bit copy; skipped when the V table entry IS the source
+ *   page, i.e. the page is still shared copy-on-write).
+ * Rotation in fp32 on angles computed in fp64 on the device; one rounding to bf16.
+ * One launch for the whole batch ("fused copy-Delta-RoPE"). Source pages are
+ * only read. Uses ws. */
+sx_status sx_rope_realign(const sx_pool *pool, const sx_batch *batch, void *ws, size_t ws_bytes,
+                          sx_stream stream);
+
+/* (d) Alg. 1 l.509-510 / 544-545; slot mapping PAPER.md:333. Rows of request r are
+ * rows[rows_off[r] .. rows_off[r+1]) (absolute positions, strictly ascending within a request);
+ * k_fresh / v_fresh are bf16 [n][Hkv][128] in the same order. For each row p:
+ *   K[k_block_table[r][p/16]][:][p%16][:] = k_fresh[n],  V likewise through v_block_table.
+ * Copy-on-write (batch->cow_private != NULL): before any row is written, a touched page whose
+ * table entry differs from its reserved private page (>= 0) is copied there and the entry is
+ * flipped (K and V tables independently). Rows not listed are untouched.
+ * max_rows (host) >= rows_off[num_reqs] sizes the grid. */
+sx_status sx_scatter_kv(const sx_pool *pool, const sx_batch *batch, const void *k_fresh,
+                        const void *v_fresh, const int32_t *rows, const int32_t *rows_off,
+                        int32_t max_rows, sx_stream stream);
+
+/* (b) Eq. (1)-(3); Alg. 1 l.515-531, 537-539.
+ *   q_new     device bf16 [total_new][Hq][128]: queries of I_nr in new_idx order, already rotated.
+ *   lse_new   device fp32 [total_new][Hq] natural-log softmax normaliser of those rows over the
+ *             CURRENT pool, or NULL (then a first QK^T sweep computes it).
+ *   sel_off   device [num_reqs+1]: request r selects k_r = sel_off[r+1]-sel_off[r] cached tokens
+ *             (k_r <= number of cached tokens of r); rows_off device [num_reqs+1] with
+ *             rows_off[r+1]-rows_off[r] = |I_nr(r)| + k_r.
+ *   scores    device fp32 [total_tokens] or NULL: s_j of every position (token (r,j) at tok_off[r]+j).
+ *   sel_idx   device int32 [sel_off[num_reqs]]: S_key per request, ascending positions.
+ *   rows_R    device int32 [rows_off[num_reqs]]: R = I_nr U S_key per request, ascending.
+ * Candidates are the cached positions only; order = (score descending, position ascending).
+ * Scores are fp32 sums in a fixed order (deterministic). Uses ws. */
+sx_status sx_score_select(const sx_pool *pool, const sx_batch *batch, const void *q_new,
+                          const float *lse_new, const int32_t *sel_off, const int32_t *rows_off,
+                          float *scores, int32_t *sel_idx, int32_t *rows_R, void *ws,
+                          size_t ws_bytes, sx_stream stream);
+
+/* (c) Alg. 1 l.546-548 (sparse) / l.507-511 (full). mode 0: query rows are rows_R (as produced by
+ * sx_score_select); mode 1: rows_R and rows_off are ignored, every position of every request is
+ * a query row (R = {0..T-1}, row n of the batch = token tok_off[r]+j).
+ *   q    device bf16 [total_rows][Hq][128], compact in rows order; out same shape (bf16);
+ *   lse  device fp32 [total_rows][Hq] natural-log normaliser, or NULL.
+ *   total_rows (host) = rows_off[num_reqs] (mode 0) or total_tokens (mode 1).
+ * O[n][h] = sum_{j <= pos(n)} softmax_j(<q, k_j>/sqrt(128)) v_j with kv head h / g, K and V read
+ * through the block tables. bf16 x bf16 -> fp32 tensor-core accumulate, fp32 softmax, P rounded to
+ * bf16 before PV. */
+sx_status sx_sparse_attn(const sx_pool *pool, const sx_batch *batch, int32_t mode, const void *q,
+                         const int32_t *rows_R, const int32_t *rows_off, int32_t total_rows,
+                         void *out, float *lse, void *ws, size_t ws_bytes, sx_stream stream);
+
+/* Thread-local text of the last error returned on this thread ("" if none). Static storage. */
+const char *sx_last_error(void);
+
+/* Library build tag, e.g. "sparsex-b200 sm_100a". Static storage. */
+const char *sx_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* SPARSEX_H_ */

@@ -1,0 +1,239 @@
+// sx_api.cu -- the C ABI of include/sparsex.h: argument validation, workspace carve-up, TMA
+// descriptor construction and stage sequencing. All arithmetic of the method is in the kernels.
+#include <stdarg.h>
+#include <stdio.h>
+#include <string.h>
+
+#include "sx_internal.h"
+
+namespace sx {
+
+static thread_local char g_err[512] = "";
+
+sx_status set_error(sx_status st, const char *fmt, ...) {
+  va_list ap;
+  va_start(ap, fmt);
+  vsnprintf(g_err, sizeof g_err, fmt, ap);
+  va_end(ap);
+  return st;
+}
+
+sx_status check_launch(const char *what) {
+  cudaError_t e = cudaGetLastError();
+  if (e != cudaSuccess) return set_error(SX_ERR_CUDA, "%s: %s", what, cudaGetErrorString(e));
+  return SX_OK;
+}
+
+static size_t align_up(size_t x, size_t a) { return (x + a - 1) / a * a; }
+
+WsLayout ws_layout(const sx_pool *pool, const sx_batch *b) {
+  WsLayout w;
+  size_t off = 0;
+  w.rope_table = off;
+  off = align_up(off + sizeof(float2) * 64 * (size_t)(b->num_segments > 0 ? b->num_segments : 1), 256);
+  w.lse_new = off;
+  off = align_up(off + sizeof(float) * (size_t)(b->total_new > 0 ? b->total_new : 1) * pool->num_q_heads, 256);
+  w.partial = off;
+  off = align_up(off + sizeof(float) * (size_t)pool->num_kv_heads * b->total_tokens, 256);
+  w.scores = off;
+  off = align_up(off + sizeof(float) * (size_t)b->total_tokens, 256);
+  w.total = off;
+  return w;
+}
+
+static bool misaligned(const void *p) { return (reinterpret_cast<uintptr_t>(p) & 15u) != 0; }
+
+static sx_status validate(const sx_pool *pool, const sx_batch *b) {
+  if (!pool || !b) return set_error(SX_ERR_INVALID_ARG, "pool or batch is NULL");
+  if (!pool->k || !pool->v) return set_error(SX_ERR_INVALID_ARG, "pool.k / pool.v is NULL");
+  if (pool->head_dim != kHeadDim) return set_error(SX_ERR_UNSUPPORTED, "head_dim must be 128 (got %d)", pool->head_dim);
+  if (pool->block_size != kPage) return set_error(SX_ERR_UNSUPPORTED, "block_size must be 16 (got %d)", pool->block_size);
+  if (pool->num_blocks <= 0 || pool->num_kv_heads <= 0 || pool->num_q_heads <= 0)
+    return set_error(SX_ERR_INVALID_ARG, "pool sizes must be positive");
+  if (pool->num_q_heads % pool->num_kv_heads != 0 || pool->num_q_heads / pool->num_kv_heads > 128)
+    return set_error(SX_ERR_UNSUPPORTED, "num_q_heads must be a multiple of num_kv_heads with group <= 128");
+  if ((int64_t)pool->num_blocks * pool->num_kv_heads * kPage >= (int64_t)1 << 31)
+    return set_error(SX_ERR_UNSUPPORTED, "pool too large for 32-bit TMA row coordinates");
+  if (b->num_reqs <= 0 || b->num_segments < 0 || b->max_pages_per_req <= 0 || b->total_tokens <= 0 ||
+      b->total_new < 0 || b->total_seg_pages < 0 || b->max_seq_len <= 0)
+    return set_error(SX_ERR_INVALID_ARG, "batch sizes out of range");
+  if (b->max_seq_len > b->max_pages_per_req * kPage)
+    return set_error(SX_ERR_INVALID_ARG, "max_seq_len exceeds max_pages_per_req * 16");
+  if (!b->seq_len || !b->tok_off || !b->k_block_table || !b->v_block_table || !b->new_off)
+    return set_error(SX_ERR_INVALID_ARG, "a required batch array is NULL");
+  if (b->num_segments > 0 && (!b->segments || !b->src_blocks))
+    return set_error(SX_ERR_INVALID_ARG, "segments / src_blocks is NULL");
+  if (b->total_new > 0 && !b->new_idx) return set_error(SX_ERR_INVALID_ARG, "new_idx is NULL");
+  if (b->rope_style != 0 && b->rope_style != 1)
+    return set_error(SX_ERR_UNSUPPORTED, "rope_style must be 0 (half-split) or 1 (interleaved)");
+  if (!(b->rope_theta > 1.0)) return set_error(SX_ERR_INVALID_ARG, "rope_theta must be > 1");
+  if (misaligned(pool->k) || misaligned(pool->v)) return set_error(SX_ERR_MISALIGNED, "pool.k / pool.v not 16-B aligned");
+  return SX_OK;
+}
+
+static sx_status validate_ws(const sx_pool *pool, const sx_batch *b, const void *ws, size_t ws_bytes) {
+  WsLayout w = ws_layout(pool, b);
+  if (!ws) return set_error(SX_ERR_INVALID_ARG, "workspace is NULL");
+  if ((reinterpret_cast<uintptr_t>(ws) & 255u) != 0) return set_error(SX_ERR_MISALIGNED, "workspace not 256-B aligned");
+  if (ws_bytes < w.total) return set_error(SX_ERR_WORKSPACE, "workspace too small: %zu < %zu", ws_bytes, w.total);
+  return SX_OK;
+}
+
+// ------------------------------------------------------------------------------------ tensor maps
+typedef CUresult (*EncodeTiledFn)(CUtensorMap *, CUtensorMapDataType, cuuint32_t, void *, const cuuint64_t *,
+                                  const cuuint64_t *, const cuuint32_t *, const cuuint32_t *,
+                                  CUtensorMapInterleave, CUtensorMapSwizzle, CUtensorMapL2promotion,
+                                  CUtensorMapFloatOOBfill);
+
+static sx_status get_encode(EncodeTiledFn *fn) {
+  static EncodeTiledFn cached = nullptr;
+  if (!cached) {
+    void *p = nullptr;
+    cudaDriverEntryPointQueryResult q;
+    cudaError_t e = cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &p, cudaEnableDefault, &q);
+    if (e != cudaSuccess || q != cudaDriverEntryPointSuccess || !p) {
+      cudaGetLastError();
+      return set_error(SX_ERR_CUDA, "cuTensorMapEncodeTiled unavailable: %s", cudaGetErrorString(e));
+    }
+    cached = reinterpret_cast<EncodeTiledFn>(p);
+  }
+  *fn = cached;
+  return SX_OK;
+}
+
+// Pool viewed as a 2-D bf16 matrix [num_blocks*Hkv*16 rows][128]; box = 64 columns x 16 rows (one
+// half of one (page, head) tile), 128-B swizzle: lands as two 8-row x 128-B swizzle atoms.
+sx_status make_tmap_pool(CUtensorMap *out, const void *base, int num_blocks, int num_kv_heads) {
+  EncodeTiledFn enc;
+  sx_status st = get_encode(&enc);
+  if (st != SX_OK) return st;
+  cuuint64_t dims[2] = {(cuuint64_t)kHeadDim, (cuuint64_t)num_blocks * num_kv_heads * kPage};
+  cuuint64_t strides[1] = {(cuuint64_t)kHeadDim * 2};
+  cuuint32_t box[2] = {64, (cuuint32_t)kPage};
+  cuuint32_t estr[2] = {1, 1};
+  CUresult r = enc(out, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 2, const_cast<void *>(base), dims, strides, box, estr,
+                   CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
+                   CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+  if (r != CUDA_SUCCESS) return set_error(SX_ERR_CUDA, "cuTensorMapEncodeTiled(pool) failed: %d", (int)r);
+  return SX_OK;
+}
+
+// Query rows [total_rows][Hq][128] viewed as 3-D (d, head, row); box = 64 d x g heads x rows_per_tile
+// rows: the g query heads of one KV group for rows_per_tile consecutive rows land as (row, head)-
+// ordered 128-B lines = the GQA-packed M (or N) dimension of a tile. Rows beyond total_rows are
+// zero-filled by the TMA unit.
+sx_status make_tmap_q(CUtensorMap *out, const void *base, int total_rows, int num_q_heads, int group,
+                      int rows_per_tile) {
+  EncodeTiledFn enc;
+  sx_status st = get_encode(&enc);
+  if (st != SX_OK) return st;
+  cuuint64_t dims[3] = {(cuuint64_t)kHeadDim, (cuuint64_t)num_q_heads, (cuuint64_t)total_rows};
+  cuuint64_t strides[2] = {(cuuint64_t)kHeadDim * 2, (cuuint64_t)kHeadDim * 2 * num_q_heads};
+  cuuint32_t box[3] = {64, (cuuint32_t)group, (cuuint32_t)rows_per_tile};
+  cuuint32_t estr[3] = {1, 1, 1};
+  CUresult r = enc(out, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 3, const_cast<void *>(base), dims, strides, box, estr,
+                   CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
+                   CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+  if (r != CUDA_SUCCESS) return set_error(SX_ERR_CUDA, "cuTensorMapEncodeTiled(q) failed: %d", (int)r);
+  return SX_OK;
+}
+
+}  // namespace sx
+
+using namespace sx;
+
+extern "C" {
+
+const char *sx_last_error(void) { return g_err; }
+
+const char *sx_version(void) { return "sparsex-b200 0.1 (sm_100a; tcgen05/TMEM/TMA)"; }
+
+sx_status sx_workspace_size(const sx_pool *pool, const sx_batch *batch, size_t *bytes) {
+  if (!bytes) return set_error(SX_ERR_INVALID_ARG, "bytes is NULL");
+  if (!pool || !batch) return set_error(SX_ERR_INVALID_ARG, "pool or batch is NULL");
+  if (pool->num_kv_heads <= 0 || pool->num_q_heads <= 0 || batch->total_tokens <= 0 || batch->num_segments < 0 ||
+      batch->total_new < 0)
+    return set_error(SX_ERR_INVALID_ARG, "sizes out of range");
+  *bytes = ws_layout(pool, batch).total;
+  return SX_OK;
+}
+
+sx_status sx_rope_realign(const sx_pool *pool, const sx_batch *batch, void *ws, size_t ws_bytes, sx_stream stream) {
+  sx_status st = validate(pool, batch);
+  if (st != SX_OK) return st;
+  st = validate_ws(pool, batch, ws, ws_bytes);
+  if (st != SX_OK) return st;
+  if (batch->num_segments == 0 || batch->total_seg_pages == 0) return SX_OK;
+  WsLayout w = ws_layout(pool, batch);
+  return launch_realign(pool, batch, reinterpret_cast<float2 *>(static_cast<char *>(ws) + w.rope_table),
+                        reinterpret_cast<cudaStream_t>(stream));
+}
+
+sx_status sx_scatter_kv(const sx_pool *pool, const sx_batch *batch, const void *k_fresh, const void *v_fresh,
+                        const int32_t *rows, const int32_t *rows_off, int32_t max_rows, sx_stream stream) {
+  sx_status st = validate(pool, batch);
+  if (st != SX_OK) return st;
+  if (max_rows < 0) return set_error(SX_ERR_INVALID_ARG, "max_rows < 0");
+  if (max_rows == 0) return SX_OK;
+  if (!k_fresh || !v_fresh || !rows || !rows_off) return set_error(SX_ERR_INVALID_ARG, "scatter: NULL array");
+  if (misaligned(k_fresh) || misaligned(v_fresh)) return set_error(SX_ERR_MISALIGNED, "k_fresh / v_fresh not 16-B aligned");
+  return launch_scatter(pool, batch, k_fresh, v_fresh, rows, rows_off, max_rows, reinterpret_cast<cudaStream_t>(stream));
+}
+
+sx_status sx_score_select(const sx_pool *pool, const sx_batch *batch, const void *q_new, const float *lse_new,
+                          const int32_t *sel_off, const int32_t *rows_off, float *scores, int32_t *sel_idx,
+                          int32_t *rows_R, void *ws, size_t ws_bytes, sx_stream stream) {
+  sx_status st = validate(pool, batch);
+  if (st != SX_OK) return st;
+  st = validate_ws(pool, batch, ws, ws_bytes);
+  if (st != SX_OK) return st;
+  if (!sel_off || !rows_off || !sel_idx || !rows_R) return set_error(SX_ERR_INVALID_ARG, "score_select: NULL array");
+  if (batch->total_new > 0 && !q_new) return set_error(SX_ERR_INVALID_ARG, "q_new is NULL");
+  if (q_new && misaligned(q_new)) return set_error(SX_ERR_MISALIGNED, "q_new not 16-B aligned");
+  cudaStream_t s = reinterpret_cast<cudaStream_t>(stream);
+  WsLayout w = ws_layout(pool, batch);
+  char *base = static_cast<char *>(ws);
+  float *partial = reinterpret_cast<float *>(base + w.partial);
+  const float *lse = lse_new;
+  if (batch->total_new > 0) {
+    if (!lse) {  // sweep 1: row normaliser of Eq. (1) for the Sparse-Q rows
+      float *lse_ws = reinterpret_cast<float *>(base + w.lse_new);
+      st = launch_attn(pool, batch, /*with_pv=*/false, q_new, batch->new_idx, batch->new_off, batch->total_new,
+                       nullptr, lse_ws, s);
+      if (st != SX_OK) return st;
+      lse = lse_ws;
+    }
+    // sweep 2: column sums of A_sq (Eq. 2), one partial vector per KV head
+    st = launch_colsum(pool, batch, q_new, lse, partial, s);
+    if (st != SX_OK) return st;
+  } else {
+    cudaError_t e = cudaMemsetAsync(partial, 0, sizeof(float) * (size_t)pool->num_kv_heads * batch->total_tokens, s);
+    if (e != cudaSuccess) return set_error(SX_ERR_CUDA, "memset: %s", cudaGetErrorString(e));
+  }
+  float *sc = scores ? scores : reinterpret_cast<float *>(base + w.scores);
+  return launch_select(pool, batch, partial, sel_off, rows_off, sc, sel_idx, rows_R, s);
+}
+
+sx_status sx_sparse_attn(const sx_pool *pool, const sx_batch *batch, int32_t mode, const void *q,
+                         const int32_t *rows_R, const int32_t *rows_off, int32_t total_rows, void *out, float *lse,
+                         void *ws, size_t ws_bytes, sx_stream stream) {
+  sx_status st = validate(pool, batch);
+  if (st != SX_OK) return st;
+  (void)ws;
+  (void)ws_bytes;
+  if (mode != 0 && mode != 1) return set_error(SX_ERR_INVALID_ARG, "mode must be 0 (sparse rows) or 1 (full)");
+  if (total_rows < 0) return set_error(SX_ERR_INVALID_ARG, "total_rows < 0");
+  if (total_rows == 0) return SX_OK;
+  if (!q || !out) return set_error(SX_ERR_INVALID_ARG, "q / out is NULL");
+  if (misaligned(q) || misaligned(out)) return set_error(SX_ERR_MISALIGNED, "q / out not 16-B aligned");
+  cudaStream_t s = reinterpret_cast<cudaStream_t>(stream);
+  if (mode == 1) {
+    if (total_rows != batch->total_tokens)
+      return set_error(SX_ERR_INVALID_ARG, "full mode: total_rows must equal total_tokens");
+    return launch_attn(pool, batch, true, q, nullptr, batch->tok_off, total_rows, out, lse, s);
+  }
+  if (!rows_R || !rows_off) return set_error(SX_ERR_INVALID_ARG, "rows_R / rows_off is NULL");
+  return launch_attn(pool, batch, true, q, rows_R, rows_off, total_rows, out, lse, s);
+}
+
+}  // extern "C"

@@ -1,0 +1,48 @@
+// sx_internal.h -- declarations shared by the translation units of libsparsex.so (not installed).
+#pragma once
+#include <cuda.h>
+#include <cuda_runtime.h>
+#include <stddef.h>
+#include <stdint.h>
+
+#include "../../include/sparsex.h"
+
+namespace sx {
+
+constexpr int kHeadDim = 128;   // D
+constexpr int kPage = 16;       // block_size b
+constexpr int kTile = 128;      // keys per K/V tile = 8 pages; rows per Q tile
+constexpr double kLog2e = 1.4426950408889634;
+
+// Workspace carve-up (all offsets 256-B aligned). Computed from host mirrors only.
+struct WsLayout {
+  size_t rope_table;   // float2 [num_segments][64]       (cos, sin)(delta_m * theta_i)
+  size_t lse_new;      // float  [total_new][Hq]          sweep-1 normaliser (natural log)
+  size_t partial;      // float  [Hkv][total_tokens]      per-kv-head column sums of A_sq
+  size_t scores;       // float  [total_tokens]           head-summed scores when the caller passes none
+  size_t total;
+};
+WsLayout ws_layout(const sx_pool *pool, const sx_batch *batch);
+
+sx_status set_error(sx_status st, const char *fmt, ...);
+sx_status check_launch(const char *what);
+
+// kernels (one launcher per translation unit)
+sx_status launch_realign(const sx_pool *pool, const sx_batch *b, float2 *table, cudaStream_t st);
+sx_status launch_scatter(const sx_pool *pool, const sx_batch *b, const void *k_fresh, const void *v_fresh,
+                         const int32_t *rows, const int32_t *rows_off, int32_t max_rows, cudaStream_t st);
+sx_status launch_select(const sx_pool *pool, const sx_batch *b, const float *partial, const int32_t *sel_off,
+                        const int32_t *rows_off, float *scores, int32_t *sel_idx, int32_t *rows_R,
+                        cudaStream_t st);
+// tcgen05 kernels. q_rows: bf16 [total_rows][Hq][128]; rows == nullptr => row n is position n - off[req].
+sx_status launch_attn(const sx_pool *pool, const sx_batch *b, bool with_pv, const void *q, const int32_t *rows,
+                      const int32_t *rows_off, int32_t total_rows, void *out, float *lse, cudaStream_t st);
+sx_status launch_colsum(const sx_pool *pool, const sx_batch *b, const void *q_new, const float *lse_new,
+                        float *partial, cudaStream_t st);
+
+// TMA descriptor construction (driver entry point fetched through the runtime; no libcuda link)
+sx_status make_tmap_pool(CUtensorMap *out, const void *base, int num_blocks, int num_kv_heads);
+sx_status make_tmap_q(CUtensorMap *out, const void *base, int total_rows, int num_q_heads, int group,
+                      int rows_per_tile);
+
+}  // namespace sx

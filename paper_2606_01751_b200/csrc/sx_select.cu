@@ -1,0 +1,187 @@
+// sx_select.cu -- stage (b), second half: head aggregation of the column sums,
+// S_key = TopK({s_j}, k) over the cached positions (Eq. 3; DESIGN.md readings
+// A7/A8: candidates = I_reuse, order = score descending then position ascending) and the
+// recompute set R = I_nr U S_key (Alg. 1 l.537-539), both emitted in ascending position order.
+//
+// One CTA per request. Scores are non-negative fp32, so their bit patterns order like unsigned
+// integers: 4-pass 8-bit radix select finds the k-th largest pattern, one ordered pass with block
+// scans then emits S_key and R. Integer atomics only (deterministic).
+#include "sx_internal.h"
+#include "sx_ptx.cuh"
+
+namespace sx {
+
+constexpr int kSelThreads = 1024;
+constexpr int kSelWarps = kSelThreads / 32;
+
+// exclusive block scan of three small counters at once; returns exclusive prefixes, adds totals to base
+struct Scan3 {
+  int a, b, c;
+};
+
+__device__ __forceinline__ Scan3 block_scan3(bool fa, bool fb, bool fc, int (*warp_tot)[kSelWarps], int *tot) {
+  const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
+  const unsigned ba = __ballot_sync(0xffffffffu, fa), bb = __ballot_sync(0xffffffffu, fb),
+                 bc = __ballot_sync(0xffffffffu, fc);
+  const unsigned lt = (1u << lane) - 1u;
+  if (lane == 0) {
+    warp_tot[0][w] = __popc(ba);
+    warp_tot[1][w] = __popc(bb);
+    warp_tot[2][w] = __popc(bc);
+  }
+  __syncthreads();
+  if (w < 3) {  // warp w scans counter w over the 32 warp totals
+    int v = warp_tot[w][lane];
+    int x = v;
+#pragma unroll
+    for (int d = 1; d < 32; d <<= 1) {
+      int y = __shfl_up_sync(0xffffffffu, x, d);
+      if (lane >= d) x += y;
+    }
+    warp_tot[w][lane] = x - v;  // exclusive
+    if (lane == 31) tot[w] = x;
+  }
+  __syncthreads();
+  Scan3 r;
+  r.a = warp_tot[0][w] + __popc(ba & lt);
+  r.b = warp_tot[1][w] + __popc(bb & lt);
+  r.c = warp_tot[2][w] + __popc(bc & lt);
+  return r;
+}
+
+__global__ void __launch_bounds__(kSelThreads)
+select_kernel(int num_kv_heads, int total_tokens, const int32_t *__restrict__ seq_len,
+              const int32_t *__restrict__ tok_off, const int32_t *__restrict__ new_off,
+              const int32_t *__restrict__ new_idx, const float *__restrict__ partial,
+              const int32_t *__restrict__ sel_off, const int32_t *__restrict__ rows_off, float *__restrict__ scores,
+              int32_t *__restrict__ sel_idx, int32_t *__restrict__ rows_R) {
+  extern __shared__ uint32_t is_new[];  // bitmap over positions
+  __shared__ int hist[256];
+  __shared__ int warp_tot[3][kSelWarps];
+  __shared__ int tot[3];
+  __shared__ uint32_t sh_prefix;
+  __shared__ int sh_remaining;
+
+  const int req = blockIdx.x;
+  const int T = seq_len[req];
+  const int off = tok_off[req];
+  const int n0 = new_off[req], nn = new_off[req + 1] - n0;
+  const int words = (T + 31) >> 5;
+  int k = sel_off[req + 1] - sel_off[req];
+  const int n_cached = T - nn;
+  if (k > n_cached) k = n_cached;
+  if (k < 0) k = 0;
+
+  for (int i = threadIdx.x; i < words; i += kSelThreads) is_new[i] = 0u;
+  __syncthreads();
+  for (int i = threadIdx.x; i < nn; i += kSelThreads) {
+    int p = new_idx[n0 + i];
+    atomicOr(&is_new[p >> 5], 1u << (p & 31));
+  }
+  // head aggregation in fixed order kvh = 0..Hkv-1 (global score across heads)
+  for (int j = threadIdx.x; j < T; j += kSelThreads) {
+    float s = 0.f;
+    for (int h = 0; h < num_kv_heads; ++h) s += partial[(size_t)h * total_tokens + off + j];
+    scores[off + j] = s;
+  }
+  __syncthreads();
+
+  // ---- radix select: bit pattern of the k-th largest candidate score
+  uint32_t prefix = 0, mask = 0;
+  int remaining = k;
+  if (k > 0) {
+    for (int pass = 3; pass >= 0; --pass) {
+      const int shift = pass * 8;
+      for (int i = threadIdx.x; i < 256; i += kSelThreads) hist[i] = 0;
+      __syncthreads();
+      for (int j = threadIdx.x; j < T; j += kSelThreads) {
+        if (!((is_new[j >> 5] >> (j & 31)) & 1u)) {
+          uint32_t u = __float_as_uint(scores[off + j]);
+          if ((u & mask) == prefix) atomicAdd(&hist[(u >> shift) & 255u], 1);
+        }
+      }
+      __syncthreads();
+      if (threadIdx.x < 32) {
+        // bins from high to low; lane l owns bins [255-8l-7, 255-8l]
+        const int lane = threadIdx.x;
+        int c[8], sum = 0;
+#pragma unroll
+        for (int i = 0; i < 8; ++i) {
+          c[i] = hist[255 - (lane * 8 + i)];
+          sum += c[i];
+        }
+        int incl = sum;
+#pragma unroll
+        for (int d = 1; d < 32; d <<= 1) {
+          int y = __shfl_up_sync(0xffffffffu, incl, d);
+          if (lane >= d) incl += y;
+        }
+        int before = incl - sum;  // candidates in bins above this lane's bins
+        if (before < remaining && remaining <= incl) {
+          int acc = before;
+#pragma unroll
+          for (int i = 0; i < 8; ++i) {
+            if (acc < remaining && remaining <= acc + c[i]) {
+              sh_prefix = prefix | ((uint32_t)(255 - (lane * 8 + i)) << shift);
+              sh_remaining = remaining - acc;
+            }
+            acc += c[i];
+          }
+        }
+      }
+      __syncthreads();
+      prefix = sh_prefix;
+      remaining = sh_remaining;
+      mask |= 255u << shift;
+      __syncthreads();
+    }
+  }
+  // prefix = threshold pattern; `remaining` = how many candidates equal to it are taken (lowest positions)
+  const uint32_t thr = prefix;
+  const int take_eq = (k > 0) ? remaining : 0;
+
+  // ---- ordered emission
+  int base_eq = 0, base_sel = 0, base_r = 0;
+  const int so = sel_off[req], ro = rows_off[req];
+  for (int j0 = 0; j0 < T; j0 += kSelThreads) {
+    const int j = j0 + threadIdx.x;
+    bool isn = false, gt = false, eq = false;
+    if (j < T) {
+      isn = (is_new[j >> 5] >> (j & 31)) & 1u;
+      if (!isn && k > 0) {
+        uint32_t u = __float_as_uint(scores[off + j]);
+        gt = u > thr;
+        eq = u == thr;
+      }
+    }
+    // rank among equals decides eq membership; it needs the eq scan first
+    Scan3 s1 = block_scan3(eq, false, false, warp_tot, tot);
+    const int tot_eq = tot[0];
+    const bool sel = gt || (eq && (base_eq + s1.a) < take_eq);
+    __syncthreads();
+    Scan3 s2 = block_scan3(sel, sel || isn, false, warp_tot, tot);
+    if (sel) sel_idx[so + base_sel + s2.a] = j;
+    if (sel || isn) rows_R[ro + base_r + s2.b] = j;
+    const int tsel = tot[0], tr = tot[1];
+    __syncthreads();
+    base_eq += tot_eq;
+    base_sel += tsel;
+    base_r += tr;
+  }
+}
+
+sx_status launch_select(const sx_pool *pool, const sx_batch *b, const float *partial, const int32_t *sel_off,
+                        const int32_t *rows_off, float *scores, int32_t *sel_idx, int32_t *rows_R, cudaStream_t st) {
+  size_t smem = sizeof(uint32_t) * (size_t)((b->max_seq_len + 31) / 32);
+  if (smem > 200 * 1024) return set_error(SX_ERR_UNSUPPORTED, "max_seq_len %d too large for the select bitmap", b->max_seq_len);
+  if (smem > 40 * 1024) {
+    cudaError_t e = cudaFuncSetAttribute(select_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    if (e != cudaSuccess) return set_error(SX_ERR_CUDA, "select smem attr: %s", cudaGetErrorString(e));
+  }
+  select_kernel<<<b->num_reqs, kSelThreads, smem, st>>>(pool->num_kv_heads, b->total_tokens, b->seq_len, b->tok_off,
+                                                       b->new_off, b->new_idx, partial, sel_off, rows_off, scores,
+                                                       sel_idx, rows_R);
+  return check_launch("select_kernel");
+}
+
+}  // namespace sx

@@ -1,0 +1,94 @@
+"""CPU-only checks of the C-ABI boundary: the library builds, loads, exports every symbol that
+include/sparsex.h declares, validates arguments on the host, and fails loudly without a GPU."""
+import ctypes
+import os
+import re
+
+import numpy as np
+import pytest
+import torch
+
+from paper_2606_01751_b200 import binding as sx
+from paper_2606_01751_b200 import build as sxbuild
+from paper_2606_01751_b200 import workloads as wl
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+
+
+@pytest.fixture(scope="module")
+def lib():
+    sxbuild.build()
+    return sx.load()
+
+
+def test_header_symbols_are_exported(lib):
+    hdr = open(os.path.join(ROOT, "include", "sparsex.h")).read()
+    hdr = re.sub(r"/\*.*?\*/", "", hdr, flags=re.S)
+    declared = set(re.findall(r"\b(sx_[a-z_]+)\s*\(", hdr))
+    assert declared == set(sx.EXPORTS), declared ^ set(sx.EXPORTS)
+    for name in declared:
+        assert getattr(lib, name) is not None
+    assert b"sm_100a" in lib.sx_version()
+
+
+def test_struct_sizes_match_header():
+    # int32 x5 after two pointers; the batch struct has 7 int32, 9 pointers, a double and an int32
+    assert ctypes.sizeof(sx.SxPool) == 2 * 8 + 5 * 4 + 4
+    assert ctypes.sizeof(sx.SxBatch) == 7 * 4 + 4 + 9 * 8 + 8 + 8
+
+
+def _host_structs(lay):
+    pool = sx.SxPool(0x1000, 0x2000, lay.num_blocks, 16, lay.num_kv_heads, lay.num_q_heads, 128)
+    b = sx.SxBatch(lay.num_reqs, lay.num_segments, lay.max_pages_per_req, lay.total_tokens, lay.total_new,
+                   lay.total_seg_pages, int(lay.seq_len.max()), 0x100, 0x100, 0x100, 0x100, None, 0x100, 0x100,
+                   0x100, 0x100, lay.rope_theta, lay.rope_style)
+    return pool, b
+
+
+def test_workspace_size_is_host_only(lib):
+    lay = wl.config_c1()
+    pool, b = _host_structs(lay)
+    n = ctypes.c_size_t(0)
+    assert lib.sx_workspace_size(ctypes.byref(pool), ctypes.byref(b), ctypes.byref(n)) == 0
+    # rope table + lse + per-head partial scores + scores, each 256-B aligned
+    lo = 8 * 64 * lay.num_segments + 4 * lay.total_new * 8 + 4 * 2 * lay.total_tokens + 4 * lay.total_tokens
+    assert lo <= n.value <= lo + 4 * 256
+    assert lib.sx_workspace_size(None, ctypes.byref(b), ctypes.byref(n)) == -1
+
+
+def test_argument_validation(lib):
+    lay = wl.config_c1()
+    pool, b = _host_structs(lay)
+    ws = ctypes.c_void_p(0x10000)
+    bad = sx.SxPool(0x1000, 0x2000, lay.num_blocks, 16, lay.num_kv_heads, lay.num_q_heads, 64)
+    assert lib.sx_rope_realign(ctypes.byref(bad), ctypes.byref(b), ws, 1 << 30, None) == -2     # head_dim
+    assert b"head_dim" in lib.sx_last_error()
+    bad = sx.SxPool(0x1000, 0x2000, lay.num_blocks, 32, lay.num_kv_heads, lay.num_q_heads, 128)
+    assert lib.sx_rope_realign(ctypes.byref(bad), ctypes.byref(b), ws, 1 << 30, None) == -2     # block_size
+    bad = sx.SxPool(0x1000, 0x2000, lay.num_blocks, 16, 3, 8, 128)
+    assert lib.sx_rope_realign(ctypes.byref(bad), ctypes.byref(b), ws, 1 << 30, None) == -2     # Hq % Hkv
+    bad = sx.SxPool(0x1008, 0x2000, lay.num_blocks, 16, lay.num_kv_heads, lay.num_q_heads, 128)
+    assert lib.sx_rope_realign(ctypes.byref(bad), ctypes.byref(b), ws, 1 << 30, None) == -5     # alignment
+    assert lib.sx_rope_realign(ctypes.byref(pool), ctypes.byref(b), ws, 16, None) == -3         # workspace
+    assert lib.sx_rope_realign(ctypes.byref(pool), ctypes.byref(b), None, 1 << 30, None) == -1  # NULL ws
+    assert lib.sx_sparse_attn(ctypes.byref(pool), ctypes.byref(b), 7, ws, ws, ws, 4, ws, None, ws, 1 << 30,
+                              None) == -1                                                         # mode
+    assert lib.sx_scatter_kv(ctypes.byref(pool), ctypes.byref(b), None, ws, ws, ws, 4, None) == -1
+
+
+@pytest.mark.skipif(torch.cuda.is_available(), reason="checks the no-GPU failure mode")
+def test_no_cpu_fallback(lib):
+    # valid arguments, no device: the stage must report SX_ERR_CUDA, never compute on the host
+    lay = wl.config_tiny()
+    pool, b = _host_structs(lay)
+    ws = ctypes.c_void_p(0x10000)
+    assert lib.sx_rope_realign(ctypes.byref(pool), ctypes.byref(b), ws, 1 << 30, None) == -4
+    assert len(lib.sx_last_error()) > 0
+
+
+def test_selection_offsets():
+    lay = wl.config_tiny()
+    sel_off, rows_off = sx.selection_offsets(lay)
+    n_new = np.diff(lay.new_off)
+    assert np.array_equal(np.diff(sel_off), lay.k_per_req)
+    assert np.array_equal(np.diff(rows_off), lay.k_per_req + n_new)
