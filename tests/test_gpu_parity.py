@@ -166,8 +166,9 @@ def test_sparse_layer_chained(name):
         fresh = np.zeros(t, dtype=bool)
         fresh[res.rows[r]] = True
         assert np.array_equal(a[fresh], b[fresh])                           # scattered rows bit-exact
-        # re-rotated rows: at most one bf16 ulp from the oracle's rounding
-        assert np.all(np.abs(a - b) <= 2.0 ** -7 * np.abs(b) + 1e-30)
+        # re-rotated rows: at most one bf16 ulp from the oracle's rounding (+ the fp32 rotation's absolute
+        # error ~2^-23 (|x|+|y|), which exceeds an ulp only for results that cancel to ~1e-5)
+        assert np.all(np.abs(a - b) <= 2.0 ** -7 * np.abs(b) + 1e-5)
 
 
 @pytest.mark.parametrize("name", ["tiny", "tiny-ragged", "tiny-g7", "C1", "C3-eighth"])
