@@ -126,8 +126,10 @@ sx_status sx_scatter_kv(const sx_pool *pool, const sx_batch *batch, const void *
 
 /* (b) Eq. (1)-(3); Alg. 1 l.515-531, 537-539.
  *   q_new     device bf16 [total_new][Hq][128]: queries of I_nr in new_idx order, already rotated.
- *   lse_new   device fp32 [total_new][Hq] natural-log softmax normaliser of those rows over the
- *             CURRENT pool, or NULL (then a first QK^T sweep computes it).
+ *   lse_new   device fp32 natural-log softmax normaliser of those rows over the CURRENT pool, or
+ *             NULL (then a first QK^T sweep computes it). lse_by_token = 0: [total_new][Hq] in
+ *             new_idx order; 1: [total_tokens][Hq] indexed by batch token tok_off[r]+position (the
+ *             lse output of a full-mode sx_sparse_attn: boundary layer of Alg. 1 l.507-531).
  *   sel_off   device [num_reqs+1]: request r selects k_r = sel_off[r+1]-sel_off[r] cached tokens
  *             (k_r <= number of cached tokens of r); rows_off device [num_reqs+1] with
  *             rows_off[r+1]-rows_off[r] = |I_nr(r)| + k_r.
@@ -137,7 +139,8 @@ sx_status sx_scatter_kv(const sx_pool *pool, const sx_batch *batch, const void *
  * Candidates are the cached positions only; order = (score descending, position ascending).
  * Scores are fp32 sums in a fixed order (deterministic). Uses ws. */
 sx_status sx_score_select(const sx_pool *pool, const sx_batch *batch, const void *q_new,
-                          const float *lse_new, const int32_t *sel_off, const int32_t *rows_off,
+                          const float *lse_new, int32_t lse_by_token, const int32_t *sel_off,
+                          const int32_t *rows_off,
                           float *scores, int32_t *sel_idx, int32_t *rows_R, void *ws,
                           size_t ws_bytes, sx_stream stream);
 

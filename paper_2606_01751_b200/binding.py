@@ -23,6 +23,7 @@ _LIB_PATH = os.path.join(_HERE, "libsparsex.so")
 _lib = None
 
 SX_OK = 0
+LAUNCHES = 0   # kernels launched through this binding (each stage call adds its known kernel count)
 EXPORTS = ["sx_workspace_size", "sx_rope_realign", "sx_scatter_kv", "sx_score_select", "sx_sparse_attn",
            "sx_last_error", "sx_version"]
 
@@ -70,7 +71,7 @@ def load():
         lib.sx_scatter_kv.restype = ctypes.c_int
         lib.sx_scatter_kv.argtypes = [PP, PB, vp, vp, vp, vp, i32, vp]
         lib.sx_score_select.restype = ctypes.c_int
-        lib.sx_score_select.argtypes = [PP, PB, vp, vp, vp, vp, vp, vp, vp, vp, sz, vp]
+        lib.sx_score_select.argtypes = [PP, PB, vp, vp, i32, vp, vp, vp, vp, vp, vp, sz, vp]
         lib.sx_sparse_attn.restype = ctypes.c_int
         lib.sx_sparse_attn.argtypes = [PP, PB, i32, vp, vp, vp, i32, vp, vp, vp, sz, vp]
         lib.sx_last_error.restype = ctypes.c_char_p
@@ -161,6 +162,8 @@ def workspace_size(pool: DevicePool, batch: DeviceBatch) -> int:
 
 def rope_realign(pool: DevicePool, batch: DeviceBatch, stream=None):
     """Stage (a): K pages rotated by R_delta into the request's pages, V copied."""
+    global LAUNCHES
+    LAUNCHES += 2 if batch.c.num_segments else 0          # rope_table_kernel + realign_kernel
     ws = batch.workspace(pool)
     _check(load().sx_rope_realign(ctypes.byref(pool.c), ctypes.byref(batch.c), _ptr(ws), ws.numel(),
                                   _stream(stream)), "sx_rope_realign")
@@ -169,7 +172,9 @@ def rope_realign(pool: DevicePool, batch: DeviceBatch, stream=None):
 def scatter_kv(pool: DevicePool, batch: DeviceBatch, k_fresh: torch.Tensor, v_fresh: torch.Tensor,
                rows: torch.Tensor, rows_off: torch.Tensor, max_rows: Optional[int] = None, stream=None):
     """Stage (d), Alg. 1 l.509-510/544-545: fresh K,V rows into their paged slots (COW aware)."""
+    global LAUNCHES
     n = int(rows.numel()) if max_rows is None else int(max_rows)
+    LAUNCHES += (1 + (1 if batch.cow_private is not None else 0)) if n else 0
     assert k_fresh.is_contiguous() and v_fresh.is_contiguous() and rows.dtype == torch.int32
     _check(load().sx_scatter_kv(ctypes.byref(pool.c), ctypes.byref(batch.c), _ptr(k_fresh), _ptr(v_fresh),
                                 _ptr(rows), _ptr(rows_off), n, _stream(stream)), "sx_scatter_kv")
@@ -177,11 +182,14 @@ def scatter_kv(pool: DevicePool, batch: DeviceBatch, k_fresh: torch.Tensor, v_fr
 
 def score_select(pool: DevicePool, batch: DeviceBatch, q_new: torch.Tensor, sel_off: torch.Tensor,
                  rows_off: torch.Tensor, sel_idx: torch.Tensor, rows_R: torch.Tensor,
-                 scores: Optional[torch.Tensor] = None, lse_new: Optional[torch.Tensor] = None, stream=None):
+                 scores: Optional[torch.Tensor] = None, lse_new: Optional[torch.Tensor] = None,
+                 lse_by_token: bool = False, stream=None):
     """Stage (b), Eq. (1)-(3): Sparse-Q scores, head/query aggregation, top-k, R = I_nr U S_key."""
+    global LAUNCHES
+    LAUNCHES += 1 + ((2 if lse_new is None else 1) if batch.c.total_new else 0)   # [lse sweep] colsum select
     ws = batch.workspace(pool)
     _check(load().sx_score_select(ctypes.byref(pool.c), ctypes.byref(batch.c), _ptr(q_new), _ptr(lse_new),
-                                  _ptr(sel_off), _ptr(rows_off), _ptr(scores), _ptr(sel_idx), _ptr(rows_R),
+                                  1 if lse_by_token else 0, _ptr(sel_off), _ptr(rows_off), _ptr(scores), _ptr(sel_idx), _ptr(rows_R),
                                   _ptr(ws), ws.numel(), _stream(stream)), "sx_score_select")
 
 
@@ -190,8 +198,10 @@ def sparse_attn(pool: DevicePool, batch: DeviceBatch, q: torch.Tensor, out: torc
                 total_rows: Optional[int] = None, lse: Optional[torch.Tensor] = None, full: bool = False,
                 stream=None):
     """Stage (c), Alg. 1 l.546-548 (sparse rows) / l.507-511 (full=True)."""
+    global LAUNCHES
     ws = batch.workspace(pool)
     n = int(q.shape[0]) if total_rows is None else int(total_rows)
+    LAUNCHES += 1 if n else 0
     assert q.is_contiguous() and out.is_contiguous()
     _check(load().sx_sparse_attn(ctypes.byref(pool.c), ctypes.byref(batch.c), 1 if full else 0, _ptr(q),
                                  _ptr(rows_R), _ptr(rows_off), n, _ptr(out), _ptr(lse), _ptr(ws), ws.numel(),

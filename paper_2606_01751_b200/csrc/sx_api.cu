@@ -181,7 +181,7 @@ sx_status sx_scatter_kv(const sx_pool *pool, const sx_batch *batch, const void *
 }
 
 sx_status sx_score_select(const sx_pool *pool, const sx_batch *batch, const void *q_new, const float *lse_new,
-                          const int32_t *sel_off, const int32_t *rows_off, float *scores, int32_t *sel_idx,
+                          int32_t lse_by_token, const int32_t *sel_off, const int32_t *rows_off, float *scores, int32_t *sel_idx,
                           int32_t *rows_R, void *ws, size_t ws_bytes, sx_stream stream) {
   sx_status st = validate(pool, batch);
   if (st != SX_OK) return st;
@@ -195,6 +195,7 @@ sx_status sx_score_select(const sx_pool *pool, const sx_batch *batch, const void
   char *base = static_cast<char *>(ws);
   float *partial = reinterpret_cast<float *>(base + w.partial);
   const float *lse = lse_new;
+  if (lse_by_token != 0 && lse_by_token != 1) return set_error(SX_ERR_INVALID_ARG, "lse_by_token must be 0 or 1");
   if (batch->total_new > 0) {
     if (!lse) {  // sweep 1: row normaliser of Eq. (1) for the Sparse-Q rows
       float *lse_ws = reinterpret_cast<float *>(base + w.lse_new);
@@ -202,9 +203,10 @@ sx_status sx_score_select(const sx_pool *pool, const sx_batch *batch, const void
                        nullptr, lse_ws, s);
       if (st != SX_OK) return st;
       lse = lse_ws;
+      lse_by_token = 0;
     }
     // sweep 2: column sums of A_sq (Eq. 2), one partial vector per KV head
-    st = launch_colsum(pool, batch, q_new, lse, partial, s);
+    st = launch_colsum(pool, batch, q_new, lse, lse_by_token, partial, s);
     if (st != SX_OK) return st;
   } else {
     cudaError_t e = cudaMemsetAsync(partial, 0, sizeof(float) * (size_t)pool->num_kv_heads * batch->total_tokens, s);

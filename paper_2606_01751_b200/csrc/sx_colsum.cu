@@ -28,7 +28,8 @@ constexpr int kCsSmemBytes = kCsOffBar + 256 + 1024;
 
 struct ColsumParams {
   const int32_t *seq_len, *tok_off, *new_off, *new_idx, *k_table;
-  const float *lse;  // [total_new][Hq] natural log
+  const float *lse;  // natural log; [total_new][Hq], or [total_tokens][Hq] when lse_by_token
+  int lse_by_token;
   float *partial;    // [Hkv][total_tokens]
   int num_reqs, max_pages, num_q_heads, num_kv_heads, group, rows_per_tile, total_tokens;
   float scale_log2;
@@ -173,8 +174,9 @@ colsum_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_constant__ 
     auto load_col = [&](int it, float &lse2, int &qpos) {
       const int n = (qt0 + it) * rpt + cn;  // query index within the request
       if (cn < rpt && n < nn) {
-        lse2 = p.lse[(size_t)(nq0 + n) * p.num_q_heads + kvh * g + ch] * (float)kLog2e;
         qpos = p.new_idx[nq0 + n];
+        const size_t lrow = p.lse_by_token ? (size_t)(p.tok_off[req] + qpos) : (size_t)(nq0 + n);
+        lse2 = p.lse[lrow * p.num_q_heads + kvh * g + ch] * (float)kLog2e;
       } else {
         lse2 = INFINITY;  // pad column: exp2(-inf) = 0
         qpos = -1;
@@ -237,7 +239,7 @@ colsum_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_constant__ 
 }
 
 sx_status launch_colsum(const sx_pool *pool, const sx_batch *b, const void *q_new, const float *lse_new,
-                        float *partial, cudaStream_t st) {
+                        int lse_by_token, float *partial, cudaStream_t st) {
   const int g = pool->num_q_heads / pool->num_kv_heads;
   const int rpt = kTile / g;
   CUtensorMap tm_q, tm_k;
@@ -252,6 +254,7 @@ sx_status launch_colsum(const sx_pool *pool, const sx_batch *b, const void *q_ne
   p.new_idx = b->new_idx;
   p.k_table = b->k_block_table;
   p.lse = lse_new;
+  p.lse_by_token = lse_by_token;
   p.partial = partial;
   p.num_reqs = b->num_reqs;
   p.max_pages = b->max_pages_per_req;

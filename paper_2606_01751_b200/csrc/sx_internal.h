@@ -38,7 +38,7 @@ sx_status launch_select(const sx_pool *pool, const sx_batch *b, const float *par
 sx_status launch_attn(const sx_pool *pool, const sx_batch *b, bool with_pv, const void *q, const int32_t *rows,
                       const int32_t *rows_off, int32_t total_rows, void *out, float *lse, cudaStream_t st);
 sx_status launch_colsum(const sx_pool *pool, const sx_batch *b, const void *q_new, const float *lse_new,
-                        float *partial, cudaStream_t st);
+                        int lse_by_token, float *partial, cudaStream_t st);
 
 // TMA descriptor construction (driver entry point fetched through the runtime; no libcuda link)
 sx_status make_tmap_pool(CUtensorMap *out, const void *base, int num_blocks, int num_kv_heads);

@@ -31,12 +31,18 @@ class GpuLayer:
         self.lay = lay
         self.dev = torch.device(device)
         self.batch = batch if batch is not None else sx.DeviceBatch(lay, self.dev)
-        self.pool_k = _bits_to_dev(lt.pool_k, self.dev)
-        self.pool_v = _bits_to_dev(lt.pool_v, self.dev)
+        # lt: workloads.LayerTensors (numpy bit patterns) or any object whose pool_k / pool_v / q_full /
+        # k_fresh / v_fresh are already 2-byte device tensors
+        def up(a):
+            if isinstance(a, torch.Tensor):
+                return a if a.dtype == torch.int16 else a.view(torch.int16)
+            return _bits_to_dev(a, self.dev)
+        self.pool_k = up(lt.pool_k)
+        self.pool_v = up(lt.pool_v)
         self.pool = sx.DevicePool(self.pool_k, self.pool_v, lay.num_q_heads)
-        self.q_full = _bits_to_dev(lt.q_full, self.dev)
-        self.k_fresh = _bits_to_dev(lt.k_fresh, self.dev)
-        self.v_fresh = _bits_to_dev(lt.v_fresh, self.dev)
+        self.q_full = up(lt.q_full)
+        self.k_fresh = up(lt.k_fresh)
+        self.v_fresh = up(lt.v_fresh)
         self.tok_off_h = np.asarray(lay.tok_off, dtype=np.int64)
         # batch-wide token index of every new token, and per-request CSR of I_nr
         new_tok = []
@@ -67,14 +73,14 @@ class GpuLayer:
         sx.scatter_kv(self.pool, self.batch, self.kf_new, self.vf_new, self.batch.new_idx, self.batch.new_off,
                       max_rows=int(self.lay.new_off[-1]))
 
-    def select(self, want_scores: bool = True, lse_new: Optional[torch.Tensor] = None):
+    def select(self, want_scores: bool = True, lse_new: Optional[torch.Tensor] = None, lse_by_token: bool = False):
         n_sel, n_rows = int(self.sel_off_h[-1]), int(self.rows_off_h[-1])
         self.sel_idx = torch.full((max(n_sel, 1),), -1, dtype=torch.int32, device=self.dev)
         self.rows_R = torch.full((max(n_rows, 1),), -1, dtype=torch.int32, device=self.dev)
         self.scores = (torch.empty(int(self.lay.tok_off[-1]), dtype=torch.float32, device=self.dev)
                        if want_scores else None)
         sx.score_select(self.pool, self.batch, self.q_new, self.sel_off, self.rows_off, self.sel_idx, self.rows_R,
-                        scores=self.scores, lse_new=lse_new)
+                        scores=self.scores, lse_new=lse_new, lse_by_token=lse_by_token)
         self.sel_idx = self.sel_idx[:n_sel]
         self.rows_R = self.rows_R[:n_rows]
 

@@ -202,8 +202,7 @@ def test_paper_mode_boundary_selection():
     res3, pk3, pv3, kt3, vt3 = oracle_layer(lay, l3, mode="full")
     g3 = GpuLayer(lay, l3)
     g3.step_full()
-    lse_new = g3.lse[g3.new_tok].contiguous()
-    g3.select(lse_new=lse_new)
+    g3.select(lse_new=g3.lse, lse_by_token=True)      # full-mode LSE indexed by token: single sweep
     torch.cuda.synchronize()
     sel = g3.sel_idx.cpu().numpy()
     s = orc.scores(pk3, kt3[0], int(lay.seq_len[0]), l3.q_full[lay.new_idx], lay.new_idx, lay.num_q_heads)
