@@ -154,18 +154,14 @@ def run_ours(args):
     from paper_2606_01751_b200 import build as sxbuild
     from paper_2606_01751_b200.layer import GpuLayer
 
-    rank = int(os.environ.get("RANK", "0"))
-    world = int(os.environ.get("WORLD_SIZE", "1"))
-    local = int(os.environ.get("LOCAL_RANK", "0"))
-    if world > 1:
-        import torch.distributed as dist
-        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+    from paper_2606_01751_b200 import dist_util as du
+    rank, world, local = du.env_rank()
     torch.cuda.set_device(local)
     dev = torch.device("cuda", local)
+    du.init("nccl", dev)
     if rank == 0:
         sxbuild.build()
-    if world > 1:
-        dist.barrier()
+    du.barrier()
     sx.load()
     peaks = load_peaks()
     cfg = args.config
@@ -259,8 +255,7 @@ def run_ours(args):
             sparse_layer(layers[0], own_select=True)
 
     def barrier():
-        if world > 1:
-            dist.barrier()
+        du.barrier()
         torch.cuda.synchronize()
 
     # L2 note: one step touches > 10 GB (C3 stack) resp. every stage streams its own pool region; for the
@@ -290,10 +285,7 @@ def run_ours(args):
     ev["on"] = False
     launches = sx.LAUNCHES
     t_ms = float(np.sum(step_ms))
-    if world > 1:
-        tt = torch.tensor([t_ms], device=dev, dtype=torch.float64)
-        dist.all_reduce(tt, op=dist.ReduceOp.MAX)
-        t_ms = float(tt.item())
+    t_ms = du.max_over_ranks(t_ms, dev)
     ms_per_step = t_ms / args.steps
     stage_ms = {k: float(sum(x.elapsed_time(y) for x, y in v)) / args.steps for k, v in ev.items() if k != "on"}
     stage_n = {k: len(v) // args.steps for k, v in ev.items() if k != "on"}
@@ -321,10 +313,10 @@ def run_ours(args):
     hbm = {"realign_gbs": round(re_bytes / (stage_ms["realign"] * 1e-3) / 1e9, 1),
            "realign_frac": round(re_bytes / (stage_ms["realign"] * 1e-3) / 1e9 / peaks["hbm_gbs"], 4)}
 
-    value = world * T * n_layers / (ms_per_step * 1e-3)
+    value = du.job_throughput(T * n_layers, ms_per_step, world)
 
     # ---- e2e: host (pinned) per-row inputs in, O out, inside the timed region
-    e2e = run_e2e(torch, sx, lay, layers, batch, all_rows, sel_holder, stack, args, dev, world, barrier)
+    e2e = run_e2e(torch, sx, du, lay, layers, batch, all_rows, sel_holder, stack, args, dev, world, barrier)
 
     if rank != 0:
         return
@@ -347,7 +339,7 @@ def run_ours(args):
     print(json.dumps(line), flush=True)
 
 
-def run_e2e(torch, sx, lay, layers, batch, all_rows, sel_holder, stack, args, dev, world, barrier):
+def run_e2e(torch, sx, du, lay, layers, batch, all_rows, sel_holder, stack, args, dev, world, barrier):
     """Same step with per-row inputs in pinned HOST memory and outputs copied back, all on the stream."""
     hq = lay.num_q_heads
     T = lay.total_tokens
@@ -399,12 +391,8 @@ def run_e2e(torch, sx, lay, layers, batch, all_rows, sel_holder, stack, args, de
     b.record()
     barrier()
     ms = a.elapsed_time(b) / n
-    if world > 1:
-        import torch.distributed as dist
-        tt = torch.tensor([ms], device=dev, dtype=torch.float64)
-        dist.all_reduce(tt, op=dist.ReduceOp.MAX)
-        ms = float(tt.item())
-    return {"value": round(world * T * len(layers) / (ms * 1e-3), 1), "unit": UNIT, "ms_per_step": round(ms, 3),
+    ms = du.max_over_ranks(ms, dev)
+    return {"value": round(du.job_throughput(T * len(layers), ms, world), 1), "unit": UNIT, "ms_per_step": round(ms, 3),
             "h2d_bytes_per_step": int(h2d), "d2h_bytes_per_step": int(d2h), "steps": n,
             "note": "per-row inputs (Q, fresh K/V) from pinned host memory, O read back; paged pool resident"}
 
