@@ -4,20 +4,25 @@
 // and, with kWithPV = false, the first sweep of stage (b): the softmax normaliser (log-sum-exp) of
 // the Sparse-Q rows of Eq. (1).
 //
-// tcgen05 design (one CTA per (request, KV head, tile of R rows)):
-//   * GQA packing: the M = 128 rows of a tile are (row of R, query head of the KV group) pairs,
-//     rows_per_tile = 128 / g consecutive rows of R times g heads -> one K/V tile feeds g heads.
-//     Q arrives by one 3-D TMA box per 64-column half, already in the 128-B-swizzled K-major layout.
+// tcgen05 design, one CTA per (request, KV head, PAIR of 128-row query tiles):
+//   * GQA packing: the M = 128 rows of a query tile are (row of R, query head of the KV group)
+//     pairs: rows_per_tile = 128 / g consecutive rows of R times g heads, so one K/V tile feeds the
+//     g heads of the group. A CTA owns two such tiles (2 * rows_per_tile rows of R): every K/V tile
+//     it stages in shared memory is used by 256 query rows.
 //   * K/V tiles of 128 keys = 8 pages: the producer warp reads 8 block-table entries and issues
-//     16 TMA boxes (64 columns x 16 rows, 128-B swizzle) per tile; the 8 boxes of a half stack into
-//     a 128-row operand. K is the K-major B operand of S = Q K^T, V the MN-major B operand of O += P V.
-//   * warp 0 = TMA producer, warp 1 = MMA issuer (one elected lane), warps 2-5 = softmax: thread =
-//     one row of S in TMEM (tcgen05.ld), fp32 online softmax in the exp2 domain with lazy rescale
-//     (O in TMEM is rescaled only when the row maximum grew by more than 2^8), P rounded to bf16
-//     into swizzled shared memory as the A operand of the PV MMA. S is double-buffered in TMEM so
-//     QK^T of tile t+1 overlaps the softmax of tile t.
+//     16 TMA boxes (64 columns x 16 rows, 128-B swizzle) per tile into a 5-slot ring (K(0), V(0),
+//     K(1), V(1), ...). K is the K-major B operand of S = Q K^T, V the MN-major B operand of O += P V.
+//   * TMEM (512 columns): S_0, S_1 (128 fp32 columns each), O_0, O_1 (128 each). P (bf16) is written
+//     by the softmax threads back into the first 64 columns of its S and is the TMEM A operand of
+//     the PV MMA, so P never touches shared memory.
+//   * warp 0 = TMA producer, warp 1 = MMA issuer (one elected lane); warps 4-7 / 8-11 = softmax
+//     warpgroups of query tile 0 / 1: thread = one row of S (tcgen05.ld), fp32 online softmax in the
+//     exp2 domain with lazy rescale (O is rescaled only when the row maximum grew by more than 2^8),
+//     a fixed fraction of the exponentials evaluated on the FMA pipe (Cody-Waite + cubic) because
+//     MUFU.EX2 (16/clk/SM) would otherwise co-limit the tensor pipe. The two tiles ping-pong:
+//     while one tile's softmax runs, the tensor pipe executes the other tile's PV and next QK^T.
 //   * causality with a sparse, sorted row list: key tiles run up to the largest position of the
-//     tile; each row masks keys beyond its own position.
+//     query tile; each row masks keys beyond its own position.
 #include <math.h>
 
 #include "sx_internal.h"
@@ -25,9 +30,13 @@
 
 namespace sx {
 
-constexpr int kAttnThreads = 192;
+constexpr int kAttnThreads = 384;
 constexpr int kTileBytes = kTile * kHeadDim * 2;  // 32 KB: two 16-KB halves [half][row][64 bf16]
 constexpr int kHalfBytes = kTileBytes / 2;
+constexpr int kKvStages = 5;
+#ifndef SX_ATTN_POLY
+#define SX_ATTN_POLY 2  // of every 8 exponentials, this many go to the FMA pipe (0, 2, 4, 6 or 8)
+#endif
 
 struct AttnParams {
   const int32_t *rows;      // [total_rows] positions, or nullptr (row n of request r = position n - rows_off[r])
@@ -42,56 +51,81 @@ struct AttnParams {
   float scale;       // 1 / sqrt(128)
 };
 
-template <bool kWithPV>
 struct AttnCfg {
-  static constexpr int kStagesK = kWithPV ? 2 : 4;
-  static constexpr int kStagesV = kWithPV ? 2 : 0;
-  static constexpr int kOffQ = 0;
-  static constexpr int kOffK = kOffQ + kTileBytes;
-  static constexpr int kOffV = kOffK + kStagesK * kTileBytes;
-  static constexpr int kOffP = kOffV + kStagesV * kTileBytes;
-  static constexpr int kOffBar = kOffP + (kWithPV ? kTileBytes : 0);
-  static constexpr int kSmemBytes = kOffBar + 512 + 1024;  // + alignment slack
-  static constexpr uint32_t kTmemCols = kWithPV ? 512 : 256;
+  static constexpr int kOffQ = 0;                                  // 2 query tiles
+  static constexpr int kOffKV = kOffQ + 2 * kTileBytes;            // ring
+  static constexpr int kOffBar = kOffKV + kKvStages * kTileBytes;
+  static constexpr int kSmemBytes = kOffBar + 256 + 1024;  // + alignment slack
 };
 
 struct AttnBars {
   uint64_t q_full;
-  uint64_t k_full[4], k_empty[4];
-  uint64_t v_full[2], v_empty[2];
-  uint64_t s_full[2], s_empty[2];
-  uint64_t p_full, pv_done;
+  uint64_t kv_full[kKvStages], kv_empty[kKvStages];
+  uint64_t s_full[2][2];  // [query tile][buffer]: S = Q K^T landed in TMEM   (buffer 1: LSE-only variant)
+  uint64_t s_free[2][2];  // softmax -> MMA: P written (PV variant) / S consumed (LSE-only); 128 arrivals
+  uint64_t o_full[2];     // last PV of the query tile completed
   uint32_t tmem_base;
 };
+
+// exp2 on the FMA pipe for two values at once: x = n + f, n = rint(x), |f| <= 1/2;
+// 2^f by a cubic (max relative error 7.5e-5, below the bf16 rounding of P), 2^n by exponent arithmetic.
+__device__ __forceinline__ float2 ex2_poly2(float2 x) {
+  const float kMagic = 12582912.f;  // 1.5 * 2^23: adding it leaves rint(x) in the low mantissa bits
+  x.x = fmaxf(x.x, -126.f);
+  x.y = fmaxf(x.y, -126.f);
+  const float2 t = __fadd2_rn(x, make_float2(kMagic, kMagic));
+  const float2 n = __fadd2_rn(t, make_float2(-kMagic, -kMagic));
+  const float2 f = __ffma2_rn(n, make_float2(-1.f, -1.f), x);
+  float2 p = __ffma2_rn(make_float2(0.0551716648f, 0.0551716648f), f, make_float2(0.2426111251f, 0.2426111251f));
+  p = __ffma2_rn(p, f, make_float2(0.6932609677f, 0.6932609677f));
+  p = __ffma2_rn(p, f, make_float2(0.9999280572f, 0.9999280572f));
+  float2 r;
+  r.x = __int_as_float(__float_as_int(p.x) + (__float_as_int(t.x) << 23));
+  r.y = __int_as_float(__float_as_int(p.y) + (__float_as_int(t.y) << 23));
+  return r;
+}
 
 template <bool kWithPV>
 __global__ void __launch_bounds__(kAttnThreads, 1)
 attn_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_constant__ CUtensorMap tm_k,
             const __grid_constant__ CUtensorMap tm_v, const AttnParams p) {
-  using Cfg = AttnCfg<kWithPV>;
+  using Cfg = AttnCfg;
   extern __shared__ uint8_t smem_raw[];
   uint8_t *smem = reinterpret_cast<uint8_t *>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~uintptr_t(1023));
   AttnBars *bars = reinterpret_cast<AttnBars *>(smem + Cfg::kOffBar);
 
-  // ---- which (request, KV head, row tile) is this CTA; heavy (late) tiles of a request first
-  const int g = p.group, rpt = p.rows_per_tile;
-  int req = 0, base = 0, tiles = 0, n_r = 0;
+  // ---- which (request, KV head, pair of row tiles) is this CTA; heavy (late) pairs of a request first
+  const int g = p.group, rpt = p.rows_per_tile, rpc = 2 * rpt;
+  int req = 0, base = 0, pairs = 0, n_r = 0;
   for (; req < p.num_reqs; ++req) {
     n_r = p.rows_off[req + 1] - p.rows_off[req];
-    tiles = (n_r + rpt - 1) / rpt;
-    if ((int)blockIdx.x < base + tiles * p.num_kv_heads) break;
-    base += tiles * p.num_kv_heads;
+    pairs = (n_r + rpc - 1) / rpc;
+    if ((int)blockIdx.x < base + pairs * p.num_kv_heads) break;
+    base += pairs * p.num_kv_heads;
   }
   if (req >= p.num_reqs) return;
   const int local = blockIdx.x - base;
   const int kvh = local % p.num_kv_heads;
-  const int tile = tiles - 1 - local / p.num_kv_heads;
-  const int row_base = p.rows_off[req] + tile * rpt;     // first row (batch-wide index) of this tile
-  const int nrows = min(rpt, n_r - tile * rpt);          // valid rows of R in this tile
+  const int pair = pairs - 1 - local / p.num_kv_heads;
+  const int row_base = p.rows_off[req] + pair * rpc;  // first row (batch-wide index) of query tile 0
+  const int nrows_cta = min(rpc, n_r - pair * rpc);   // valid rows of R in this CTA (>= 1)
   const int T = p.seq_len[req];
-  const int pos_max = p.rows ? p.rows[row_base + nrows - 1] : tile * rpt + nrows - 1;
-  const int n_tiles = pos_max / kTile + 1;
   const int n_pages = (T + kPage - 1) / kPage;
+  // valid rows and number of key tiles of each query tile
+  int nrows[2], n_t[2];
+  nrows[0] = min(rpt, nrows_cta);
+  nrows[1] = nrows_cta - nrows[0];
+#pragma unroll
+  for (int i = 0; i < 2; ++i) {
+    if (nrows[i] > 0) {
+      const int last = row_base + i * rpt + nrows[i] - 1;
+      const int pos_max = p.rows ? p.rows[last] : last - p.rows_off[req];
+      n_t[i] = pos_max / kTile + 1;
+    } else {
+      n_t[i] = 0;
+    }
+  }
+  const int n_tiles = max(n_t[0], n_t[1]);
 
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
 
@@ -100,131 +134,169 @@ attn_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_constant__ CU
     tma_prefetch_desc(&tm_k);
     if (kWithPV) tma_prefetch_desc(&tm_v);
     mbar_init(&bars->q_full, 1);
-    for (int i = 0; i < 4; ++i) {
-      mbar_init(&bars->k_full[i], 1);
-      mbar_init(&bars->k_empty[i], 1);
+    for (int i = 0; i < kKvStages; ++i) {
+      mbar_init(&bars->kv_full[i], 1);
+      mbar_init(&bars->kv_empty[i], 1);
     }
     for (int i = 0; i < 2; ++i) {
-      mbar_init(&bars->v_full[i], 1);
-      mbar_init(&bars->v_empty[i], 1);
-      mbar_init(&bars->s_full[i], 1);
-      mbar_init(&bars->s_empty[i], 128);
+      for (int b = 0; b < 2; ++b) {
+        mbar_init(&bars->s_full[i][b], 1);
+        mbar_init(&bars->s_free[i][b], 128);
+      }
+      mbar_init(&bars->o_full[i], 1);
     }
-    mbar_init(&bars->p_full, 128);
-    mbar_init(&bars->pv_done, 1);
     fence_mbar_init();
   }
   if (warp == 1) {
-    tmem_alloc(&bars->tmem_base, Cfg::kTmemCols);
+    tmem_alloc(&bars->tmem_base, 512);
     tmem_relinquish();
+  }
+  // rows of the query tiles that the TMA box never writes (128 - rpt*g of them when g does not divide 128)
+  if (rpt * g < kTile && warp >= 4) {
+    const int pad = kTile - rpt * g;
+    for (int i = threadIdx.x - 128; i < 4 * pad * 8; i += 256) {
+      const int c16 = i & 7, r = (i >> 3) % pad, hs = (i >> 3) / pad;  // hs = tile*2 + half
+      *reinterpret_cast<uint4 *>(smem + Cfg::kOffQ + hs * kHalfBytes + (rpt * g + r) * 128 + c16 * 16) =
+          make_uint4(0, 0, 0, 0);
+    }
+    fence_proxy_async_smem();
   }
   tc_fence_before();
   __syncthreads();
   tc_fence_after();
   const uint32_t tmem = bars->tmem_base;
-  const uint32_t tmem_o = tmem + 256;
 
-  if (warp == 0) {
-    // ================================================================ TMA producer
-    if (lane == 0) {
-      mbar_expect_tx(&bars->q_full, (uint32_t)(2 * rpt * g * 128));
-      tma_load_3d(smem + Cfg::kOffQ, &tm_q, &bars->q_full, 0, kvh * g, row_base);
-      tma_load_3d(smem + Cfg::kOffQ + kHalfBytes, &tm_q, &bars->q_full, 64, kvh * g, row_base);
-    }
-    const int pg_in_tile = lane >> 1, half = lane & 1;
-    for (int t = 0; t < n_tiles; ++t) {
-      int lp = t * 8 + pg_in_tile;
-      if (lp > n_pages - 1) lp = n_pages - 1;  // pages past the sequence: any valid page (keys are masked)
-      {
-        const int s = t % Cfg::kStagesK, u = t / Cfg::kStagesK;
-        mbar_wait(&bars->k_empty[s], (u & 1) ^ 1);
-        if (lane == 0) mbar_expect_tx(&bars->k_full[s], kTileBytes);
-        __syncwarp();
-        if (lane < 16) {
-          const int blk = p.k_table[(size_t)req * p.max_pages + lp];
-          tma_load_2d(smem + Cfg::kOffK + s * kTileBytes + half * kHalfBytes + pg_in_tile * 2048, &tm_k,
-                      &bars->k_full[s], half * 64, (blk * p.num_kv_heads + kvh) * kPage);
-        }
-      }
-      if (kWithPV) {
-        const int s = t % 2, u = t / 2;
-        mbar_wait(&bars->v_empty[s], (u & 1) ^ 1);
-        if (lane == 0) mbar_expect_tx(&bars->v_full[s], kTileBytes);
-        __syncwarp();
-        if (lane < 16) {
-          const int blk = p.v_table[(size_t)req * p.max_pages + lp];
-          tma_load_2d(smem + Cfg::kOffV + s * kTileBytes + half * kHalfBytes + pg_in_tile * 2048, &tm_v,
-                      &bars->v_full[s], half * 64, (blk * p.num_kv_heads + kvh) * kPage);
-        }
-      }
-    }
-  } else if (warp == 1) {
-    // ================================================================ MMA issuer
-    constexpr uint32_t idesc_qk = umma_idesc_bf16(128, 128, 0, 0);
-    constexpr uint32_t idesc_pv = umma_idesc_bf16(128, 128, 0, 1);
-    const uint32_t q_addr = smem_u32(smem + Cfg::kOffQ);
-    const uint32_t p_addr = smem_u32(smem + Cfg::kOffP);
-    mbar_wait(&bars->q_full, 0);
-    auto issue_qk = [&](int t) {
-      const int s = t % Cfg::kStagesK;
-      mbar_wait(&bars->k_full[s], (t / Cfg::kStagesK) & 1);
-      if (t >= 2) mbar_wait(&bars->s_empty[t & 1], ((t >> 1) + 1) & 1);
-      tc_fence_after();
+  if (warp < 4) {
+    setmaxnreg_dec<40>();
+    if (warp == 0) {
+      // ================================================================ TMA producer
       if (lane == 0) {
-        const uint32_t k_addr = smem_u32(smem + Cfg::kOffK + s * kTileBytes);
-#pragma unroll
-        for (int kk = 0; kk < 8; ++kk) {
-          const uint32_t o = (kk >> 2) * kHalfBytes + (kk & 3) * 32;
-          umma_ss(tmem + (t & 1) * 128, umma_smem_desc(q_addr + o, 16, 1024), umma_smem_desc(k_addr + o, 16, 1024),
-                  idesc_qk, kk > 0);
+        const int nq = nrows[1] > 0 ? 2 : 1;
+        mbar_expect_tx(&bars->q_full, (uint32_t)(nq * 2 * rpt * g * 128));
+        for (int i = 0; i < nq; ++i) {
+          tma_load_3d(smem + Cfg::kOffQ + i * kTileBytes, &tm_q, &bars->q_full, 0, kvh * g, row_base + i * rpt);
+          tma_load_3d(smem + Cfg::kOffQ + i * kTileBytes + kHalfBytes, &tm_q, &bars->q_full, 64, kvh * g,
+                      row_base + i * rpt);
         }
-        umma_commit(&bars->s_full[t & 1]);
-        umma_commit(&bars->k_empty[s]);
       }
-      __syncwarp();
-    };
-    issue_qk(0);
-    for (int t = 0; t < n_tiles; ++t) {
-      if (t + 1 < n_tiles) issue_qk(t + 1);
-      if (kWithPV) {
-        const int s = t & 1;
-        mbar_wait(&bars->v_full[s], (t >> 1) & 1);
-        mbar_wait(&bars->p_full, t & 1);
-        tc_fence_after();
+      const int pg_in_tile = lane >> 1, half = lane & 1;
+      const int n_items = kWithPV ? 2 * n_tiles : n_tiles;
+      for (int it = 0; it < n_items; ++it) {
+        const int t = kWithPV ? (it >> 1) : it;
+        const bool is_v = kWithPV && (it & 1);
+        int lp = t * 8 + pg_in_tile;
+        if (lp > n_pages - 1) lp = n_pages - 1;  // pages past the sequence: any valid page (keys are masked)
+        const int s = it % kKvStages, u = it / kKvStages;
+        mbar_wait(&bars->kv_empty[s], (u & 1) ^ 1);
+        if (lane == 0) mbar_expect_tx(&bars->kv_full[s], kTileBytes);
+        __syncwarp();
+        if (lane < 16) {
+          const int blk = (is_v ? p.v_table : p.k_table)[(size_t)req * p.max_pages + lp];
+          tma_load_2d(smem + Cfg::kOffKV + s * kTileBytes + half * kHalfBytes + pg_in_tile * 2048,
+                      is_v ? &tm_v : &tm_k, &bars->kv_full[s], half * 64, (blk * p.num_kv_heads + kvh) * kPage);
+        }
+      }
+    } else if (warp == 1) {
+      // ================================================================ MMA issuer
+      constexpr uint32_t idesc_qk = umma_idesc_bf16(128, 128, 0, 0);
+      constexpr uint32_t idesc_pv = umma_idesc_bf16(128, 128, 0, 1);
+      const uint32_t q_addr = smem_u32(smem + Cfg::kOffQ);
+      const uint32_t kv_addr = smem_u32(smem + Cfg::kOffKV);
+      mbar_wait(&bars->q_full, 0);
+      // S_i[buffer b] = Q_i K(slot)^T
+      auto issue_qk = [&](int i, int b, int slot) {
         if (lane == 0) {
-          const uint32_t v_addr = smem_u32(smem + Cfg::kOffV + s * kTileBytes);
+          const uint32_t k_addr = kv_addr + slot * kTileBytes;
+          const uint32_t d = tmem + (kWithPV ? i * 128 : (i * 2 + b) * 128);
 #pragma unroll
-          for (int kk = 0; kk < 8; ++kk) {  // 16 keys per MMA
-            const uint32_t po = (kk >> 2) * kHalfBytes + (kk & 3) * 32;
-            umma_ss(tmem_o, umma_smem_desc(p_addr + po, 16, 1024),
-                    umma_smem_desc(v_addr + kk * 2048, kHalfBytes, 1024), idesc_pv, (t > 0 || kk > 0));
+          for (int kk = 0; kk < 8; ++kk) {
+            const uint32_t o = (kk >> 2) * kHalfBytes + (kk & 3) * 32;
+            umma_ss(d, umma_smem_desc(q_addr + i * kTileBytes + o, 16, 1024), umma_smem_desc(k_addr + o, 16, 1024),
+                    idesc_qk, kk > 0);
           }
-          umma_commit(&bars->pv_done);
-          umma_commit(&bars->v_empty[s]);
+          umma_commit(&bars->s_full[i][b]);
         }
         __syncwarp();
+      };
+      if (kWithPV) {
+        auto kv_wait = [&](int it) { mbar_wait(&bars->kv_full[it % kKvStages], (it / kKvStages) & 1); };
+        auto kv_release = [&](int it) {
+          if (lane == 0) umma_commit(&bars->kv_empty[it % kKvStages]);
+          __syncwarp();
+        };
+        kv_wait(0);
+        tc_fence_after();
+        issue_qk(0, 0, 0);
+        if (n_t[1] > 0) issue_qk(1, 0, 0);
+        kv_release(0);
+        for (int t = 0; t < n_tiles; ++t) {
+          kv_wait(2 * t + 1);                       // V(t)
+          if (t + 1 < n_tiles) kv_wait(2 * t + 2);  // K(t+1)
+#pragma unroll
+          for (int i = 0; i < 2; ++i) {
+            if (t < n_t[i]) {
+              mbar_wait(&bars->s_free[i][0], t & 1);  // P_i(t) is in TMEM
+              tc_fence_after();
+              if (lane == 0) {
+                const uint32_t v_addr = kv_addr + ((2 * t + 1) % kKvStages) * kTileBytes;
+#pragma unroll
+                for (int kk = 0; kk < 8; ++kk)  // 16 keys per MMA: 8 TMEM columns of packed bf16 P
+                  umma_ts(tmem + 256 + i * 128, tmem + i * 128 + kk * 8,
+                          umma_smem_desc(v_addr + kk * 2048, kHalfBytes, 1024), idesc_pv, (t > 0 || kk > 0));
+                if (t == n_t[i] - 1) umma_commit(&bars->o_full[i]);
+              }
+              __syncwarp();
+              if (t + 1 < n_t[i]) issue_qk(i, 0, (2 * t + 2) % kKvStages);
+            }
+          }
+          kv_release(2 * t + 1);
+          if (t + 1 < n_tiles) kv_release(2 * t + 2);
+        }
+      } else {
+        for (int t = 0; t < n_tiles; ++t) {
+          const int slot = t % kKvStages, b = t & 1;
+          mbar_wait(&bars->kv_full[slot], (t / kKvStages) & 1);
+#pragma unroll
+          for (int i = 0; i < 2; ++i) {
+            if (t < n_t[i]) {
+              if (t >= 2) mbar_wait(&bars->s_free[i][b], ((t >> 1) + 1) & 1);
+              tc_fence_after();
+              issue_qk(i, b, slot);
+            }
+          }
+          if (lane == 0) umma_commit(&bars->kv_empty[slot]);
+          __syncwarp();
+        }
       }
     }
   } else {
-    // ================================================================ softmax / epilogue (128 threads)
-    const int quarter = warp & 3;              // TMEM lane quarter this warp may access
-    const int row = quarter * 32 + lane;       // row of the tile = TMEM lane
+    // ================================================================ softmax / epilogue (2 x 128 threads)
+    setmaxnreg_inc<232>();
+    const int qt = (warp >> 2) - 1;           // query tile of this warpgroup
+    const int quarter = warp & 3;             // TMEM lane quarter this warp may access
+    const int row = quarter * 32 + lane;      // row of the tile = TMEM lane
     const int n_local = row / g, hh = row - n_local * g;
-    const bool valid = n_local < nrows;
-    const int pos = valid ? (p.rows ? p.rows[row_base + n_local] : tile * rpt + n_local) : 0;
+    const bool valid = n_local < (qt ? nrows[1] : nrows[0]);
+    const int grow = row_base + qt * rpt + n_local;  // batch-wide row index
+    const int pos = valid ? (p.rows ? p.rows[grow] : grow - p.rows_off[req]) : 0;
     const uint32_t lane_addr = (uint32_t)(quarter * 32) << 16;
+    const uint32_t tmem_s = tmem + lane_addr + (kWithPV ? qt * 128 : qt * 256);
+    const uint32_t tmem_o = tmem + lane_addr + 256 + qt * 128;
+    const int my_tiles = qt ? n_t[1] : n_t[0];
     float m_used = -INFINITY, l = 0.f;
 
-    for (int t = 0; t < n_tiles; ++t) {
-      const int b = t & 1;
-      mbar_wait(&bars->s_full[b], (t >> 1) & 1);
+    for (int t = 0; t < my_tiles; ++t) {
+      const int b = kWithPV ? 0 : (t & 1);
+      mbar_wait(&bars->s_full[qt][b], kWithPV ? (t & 1) : ((t >> 1) & 1));
       tc_fence_after();
       uint32_t sr[4][32];
 #pragma unroll
-      for (int c = 0; c < 4; ++c) tmem_ld32(tmem + lane_addr + b * 128 + c * 32, sr[c]);
+      for (int c = 0; c < 4; ++c) tmem_ld32(tmem_s + b * 128 + c * 32, sr[c]);
       tmem_wait_ld();
-      tc_fence_before();
-      mbar_arrive(&bars->s_empty[b]);
+      if (!kWithPV) {
+        tc_fence_before();
+        mbar_arrive(&bars->s_free[qt][b]);
+      }
 
       const int nvalid = pos - t * kTile + 1;  // keys [0, nvalid) of this tile are visible to this row
       if (nvalid < kTile) {
@@ -238,7 +310,8 @@ attn_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_constant__ CU
 #pragma unroll
       for (int c = 0; c < 4; ++c)
 #pragma unroll
-        for (int i = 0; i < 32; ++i) tmax = fmaxf(tmax, __uint_as_float(sr[c][i]));
+        for (int i = 0; i < 32; i += 2)
+          tmax = fmaxf(tmax, fmaxf(__uint_as_float(sr[c][i]), __uint_as_float(sr[c][i + 1])));
       const float m_new = fmaxf(m_used, tmax);
       const bool upd = (m_new - m_used) * p.scale_log2 > 8.0f;  // lazy rescale threshold: 2^8
       float alpha = 1.f;
@@ -246,95 +319,97 @@ attn_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_constant__ CU
         alpha = ex2_approx((m_used - m_new) * p.scale_log2);
         m_used = m_new;
       }
+      if (kWithPV && t > 0 && __any_sync(0xffffffffu, upd)) {
+        // s_full(t) was committed after PV(t-1): O is quiescent until this thread arrives on s_free
+#pragma unroll
+        for (int c = 0; c < 4; ++c) {
+          uint32_t o[32];
+          tmem_ld32(tmem_o + c * 32, o);
+          tmem_wait_ld();
+#pragma unroll
+          for (int i = 0; i < 32; ++i) o[i] = __float_as_uint(__uint_as_float(o[i]) * alpha);
+          tmem_st32(tmem_o + c * 32, o);
+        }
+      }
       const float neg_m = -m_used * p.scale_log2;
-      float rsum = 0.f;
+      const float2 sc2 = make_float2(p.scale_log2, p.scale_log2), nm2 = make_float2(neg_m, neg_m);
+      float2 rsum2 = make_float2(0.f, 0.f);
+      uint32_t pk[kWithPV ? 64 : 1];
 #pragma unroll
       for (int c = 0; c < 4; ++c)
 #pragma unroll
-        for (int i = 0; i < 32; ++i) {
-          float e = ex2_approx(fmaf(__uint_as_float(sr[c][i]), p.scale_log2, neg_m));
-          rsum += e;
-          sr[c][i] = __float_as_uint(e);
+        for (int i = 0; i < 32; i += 2) {
+          float2 x = __ffma2_rn(make_float2(__uint_as_float(sr[c][i]), __uint_as_float(sr[c][i + 1])), sc2, nm2);
+          float2 e;
+          if ((i & 7) < SX_ATTN_POLY) {
+            e = ex2_poly2(x);
+          } else {
+            e.x = ex2_approx(x.x);
+            e.y = ex2_approx(x.y);
+          }
+          rsum2 = __fadd2_rn(rsum2, e);
+          if (kWithPV) pk[c * 16 + (i >> 1)] = pack_bf16x2(e.x, e.y);
         }
-      l = l * alpha + rsum;
+      l = l * alpha + (rsum2.x + rsum2.y);
 
       if (kWithPV) {
-        if (t > 0) mbar_wait(&bars->pv_done, (t - 1) & 1);  // P buffer free, O accumulator quiescent
-        if (t > 0 && __any_sync(0xffffffffu, upd)) {
-          tc_fence_after();
-#pragma unroll
-          for (int c = 0; c < 4; ++c) {
-            uint32_t o[32];
-            tmem_ld32(tmem_o + lane_addr + c * 32, o);
-            tmem_wait_ld();
-#pragma unroll
-            for (int i = 0; i < 32; ++i) o[i] = __float_as_uint(__uint_as_float(o[i]) * alpha);
-            tmem_st32(tmem_o + lane_addr + c * 32, o);
-          }
-          tmem_wait_st();
-        }
         // V rows of keys beyond the sequence may hold anything (even NaN patterns): zero them
-        if (t == n_tiles - 1 && (t + 1) * kTile > T) {
-          mbar_wait(&bars->v_full[t & 1], (t >> 1) & 1);
+        if ((t + 1) * kTile > T) {
+          const int it = 2 * t + 1;
+          mbar_wait(&bars->kv_full[it % kKvStages], (it / kKvStages) & 1);
           if (t * kTile + row >= T) {
-            uint4 z = make_uint4(0, 0, 0, 0);
-            uint8_t *v0 = smem + Cfg::kOffV + (t & 1) * kTileBytes + row * 128;
+            const uint4 z = make_uint4(0, 0, 0, 0);
+            uint8_t *v0 = smem + Cfg::kOffKV + (it % kKvStages) * kTileBytes + row * 128;
 #pragma unroll
             for (int i = 0; i < 8; ++i) {
               *reinterpret_cast<uint4 *>(v0 + i * 16) = z;
               *reinterpret_cast<uint4 *>(v0 + kHalfBytes + i * 16) = z;
             }
           }
+          fence_proxy_async_smem();
         }
-        // P (bf16) -> swizzled K-major A operand: chunk j = keys [8j, 8j+8) of this row
-        uint8_t *prow = smem + Cfg::kOffP + row * 128;
-#pragma unroll
-        for (int j = 0; j < 16; ++j) {
-          const int c = j >> 2, i0 = (j & 3) * 8;
-          uint4 v;
-          v.x = pack_bf16x2(__uint_as_float(sr[c][i0 + 0]), __uint_as_float(sr[c][i0 + 1]));
-          v.y = pack_bf16x2(__uint_as_float(sr[c][i0 + 2]), __uint_as_float(sr[c][i0 + 3]));
-          v.z = pack_bf16x2(__uint_as_float(sr[c][i0 + 4]), __uint_as_float(sr[c][i0 + 5]));
-          v.w = pack_bf16x2(__uint_as_float(sr[c][i0 + 6]), __uint_as_float(sr[c][i0 + 7]));
-          *reinterpret_cast<uint4 *>(prow + (j >> 3) * kHalfBytes + (((j & 7) ^ (row & 7)) << 4)) = v;
-        }
-        fence_proxy_async_smem();
+        // P (bf16 pairs) -> TMEM columns [0, 64) of this tile's S: the A operand of the PV MMA
+        tmem_st32(tmem_s, *reinterpret_cast<uint32_t(*)[32]>(&pk[0]));
+        tmem_st32(tmem_s + 32, *reinterpret_cast<uint32_t(*)[32]>(&pk[32]));
+        tmem_wait_st();
         tc_fence_before();
-        mbar_arrive(&bars->p_full);
+        mbar_arrive(&bars->s_free[qt][0]);
       }
     }
 
     // ---- epilogue
-    const size_t out_row = (size_t)(row_base + n_local) * p.num_q_heads + kvh * g + hh;
-    if (kWithPV) {
-      mbar_wait(&bars->pv_done, (n_tiles - 1) & 1);
-      tc_fence_after();
-      const float inv = 1.f / l;
+    if (my_tiles > 0) {
+      const size_t out_row = (size_t)grow * p.num_q_heads + kvh * g + hh;
+      if (kWithPV) {
+        mbar_wait(&bars->o_full[qt], 0);
+        tc_fence_after();
+        const float inv = 1.f / l;
 #pragma unroll
-      for (int c = 0; c < 4; ++c) {
-        uint32_t o[32];
-        tmem_ld32(tmem_o + lane_addr + c * 32, o);
-        tmem_wait_ld();
-        if (valid) {
-          uint4 *dst = reinterpret_cast<uint4 *>(p.out + out_row * kHeadDim + c * 32);
+        for (int c = 0; c < 4; ++c) {
+          uint32_t o[32];
+          tmem_ld32(tmem_o + c * 32, o);
+          tmem_wait_ld();
+          if (valid) {
+            uint4 *dst = reinterpret_cast<uint4 *>(p.out + out_row * kHeadDim + c * 32);
 #pragma unroll
-          for (int v4 = 0; v4 < 4; ++v4) {
-            uint4 v;
-            v.x = pack_bf16x2(__uint_as_float(o[v4 * 8 + 0]) * inv, __uint_as_float(o[v4 * 8 + 1]) * inv);
-            v.y = pack_bf16x2(__uint_as_float(o[v4 * 8 + 2]) * inv, __uint_as_float(o[v4 * 8 + 3]) * inv);
-            v.z = pack_bf16x2(__uint_as_float(o[v4 * 8 + 4]) * inv, __uint_as_float(o[v4 * 8 + 5]) * inv);
-            v.w = pack_bf16x2(__uint_as_float(o[v4 * 8 + 6]) * inv, __uint_as_float(o[v4 * 8 + 7]) * inv);
-            dst[v4] = v;
+            for (int v4 = 0; v4 < 4; ++v4) {
+              uint4 v;
+              v.x = pack_bf16x2(__uint_as_float(o[v4 * 8 + 0]) * inv, __uint_as_float(o[v4 * 8 + 1]) * inv);
+              v.y = pack_bf16x2(__uint_as_float(o[v4 * 8 + 2]) * inv, __uint_as_float(o[v4 * 8 + 3]) * inv);
+              v.z = pack_bf16x2(__uint_as_float(o[v4 * 8 + 4]) * inv, __uint_as_float(o[v4 * 8 + 5]) * inv);
+              v.w = pack_bf16x2(__uint_as_float(o[v4 * 8 + 6]) * inv, __uint_as_float(o[v4 * 8 + 7]) * inv);
+              dst[v4] = v;
+            }
           }
         }
       }
+      if (p.lse && valid) p.lse[out_row] = m_used * p.scale + logf(l);
     }
-    if (p.lse && valid) p.lse[out_row] = m_used * p.scale + logf(l);
   }
 
   tc_fence_before();
   __syncthreads();
-  if (warp == 1) tmem_dealloc(tmem, Cfg::kTmemCols);
+  if (warp == 1) tmem_dealloc(tmem, 512);
 }
 
 sx_status launch_attn(const sx_pool *pool, const sx_batch *b, bool with_pv, const void *q, const int32_t *rows,
@@ -364,16 +439,16 @@ sx_status launch_attn(const sx_pool *pool, const sx_batch *b, bool with_pv, cons
   p.rows_per_tile = rpt;
   p.scale = (float)(1.0 / sqrt((double)kHeadDim));
   p.scale_log2 = (float)(kLog2e / sqrt((double)kHeadDim));
-  const int grid = (total_rows / rpt + b->num_reqs) * pool->num_kv_heads;
+  const int grid = (total_rows / (2 * rpt) + b->num_reqs) * pool->num_kv_heads;  // >= sum_r ceil(n_r / 2rpt) * Hkv
   cudaError_t e;
   if (with_pv) {
-    e = cudaFuncSetAttribute(attn_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, AttnCfg<true>::kSmemBytes);
+    e = cudaFuncSetAttribute(attn_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, AttnCfg::kSmemBytes);
     if (e != cudaSuccess) return set_error(SX_ERR_CUDA, "attn smem attr: %s", cudaGetErrorString(e));
-    attn_kernel<true><<<grid, kAttnThreads, AttnCfg<true>::kSmemBytes, st>>>(tm_q, tm_k, tm_v, p);
+    attn_kernel<true><<<grid, kAttnThreads, AttnCfg::kSmemBytes, st>>>(tm_q, tm_k, tm_v, p);
   } else {
-    e = cudaFuncSetAttribute(attn_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, AttnCfg<false>::kSmemBytes);
+    e = cudaFuncSetAttribute(attn_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, AttnCfg::kSmemBytes);
     if (e != cudaSuccess) return set_error(SX_ERR_CUDA, "lse smem attr: %s", cudaGetErrorString(e));
-    attn_kernel<false><<<grid, kAttnThreads, AttnCfg<false>::kSmemBytes, st>>>(tm_q, tm_k, tm_v, p);
+    attn_kernel<false><<<grid, kAttnThreads, AttnCfg::kSmemBytes, st>>>(tm_q, tm_k, tm_v, p);
   }
   return check_launch(with_pv ? "attn_kernel<pv>" : "attn_kernel<lse>");
 }
