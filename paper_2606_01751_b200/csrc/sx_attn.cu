@@ -323,7 +323,7 @@ attn_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_constant__ CU
       tmem_ld32(tmem_s + b * 128 + 96, sr[3]);
 
       const int nvalid = pos - t * kTile + 1;  // keys [0, nvalid) of this tile are visible to this row
-      float tm[4] = {-INFINITY, -INFINITY, -INFINITY, -INFINITY};  // independent chains
+      float tm[2] = {-INFINITY, -INFINITY};  // two independent 3-input max chains
 #pragma unroll
       for (int c = 0; c < 4; ++c) {
         if (c == 2) {
@@ -343,12 +343,8 @@ attn_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_constant__ CU
           tm[0] = fmaxf(tm[0], fmaxf(__uint_as_float(sr[c][i]), __uint_as_float(sr[c][i + 1])));
           tm[1] = fmaxf(tm[1], fmaxf(__uint_as_float(sr[c][i + 2]), __uint_as_float(sr[c][i + 3])));
         }
-        if (c & 1) {  // fold every 64 columns to keep the chains short but independent
-          tm[2] = fmaxf(tm[2], fmaxf(tm[0], tm[1]));
-          tm[0] = tm[1] = -INFINITY;
-        }
       }
-      const float tmax = tm[2];
+      const float tmax = fmaxf(tm[0], tm[1]);
       const float m_new = fmaxf(m_used, tmax);
       const bool upd = (m_new - m_used) * p.scale_log2 > 8.0f;  // lazy rescale threshold: 2^8
       float alpha = 1.f;
