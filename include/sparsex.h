@@ -151,8 +151,12 @@ sx_status sx_score_select(const sx_pool *pool, const sx_batch *batch, const void
  *   lse  device fp32 [total_rows][Hq] natural-log normaliser, or NULL.
  *   total_rows (host) = rows_off[num_reqs] (mode 0) or total_tokens (mode 1).
  * O[n][h] = sum_{j <= pos(n)} softmax_j(<q, k_j>/sqrt(128)) v_j with kv head h / g, K and V read
- * through the block tables. bf16 x bf16 -> fp32 tensor-core accumulate, fp32 softmax, P rounded to
- * bf16 before PV. */
+ * through the block tables. Two paths, chosen from host-visible sizes only:
+ *   - total_rows * g >= 64 * num_reqs (at least 64 query rows per KV head on average; g = Hq/Hkv):
+ *     tcgen05 tensor-core tiles, bf16 x bf16 -> fp32 accumulate, fp32 softmax, P rounded to bf16 before PV;
+ *   - fewer rows (and g <= 32): CUDA-core split-KV path, fp32 FMA throughout, partial results of the
+ *     key-range splits combined in a fixed order. Uses ws (sx_workspace_size covers it).
+ * Both are deterministic and meet the same tolerance against fp64. */
 sx_status sx_sparse_attn(const sx_pool *pool, const sx_batch *batch, int32_t mode, const void *q,
                          const int32_t *rows_R, const int32_t *rows_off, int32_t total_rows,
                          void *out, float *lse, void *ws, size_t ws_bytes, sx_stream stream);

@@ -201,7 +201,9 @@ def sparse_attn(pool: DevicePool, batch: DeviceBatch, q: torch.Tensor, out: torc
     global LAUNCHES
     ws = batch.workspace(pool)
     n = int(q.shape[0]) if total_rows is None else int(total_rows)
-    LAUNCHES += 1 if n else 0
+    g = pool.c.num_q_heads // pool.c.num_kv_heads
+    small = g <= 32 and n * g < 64 * batch.c.num_reqs       # CUDA-core path: split kernel + merge kernel
+    LAUNCHES += (2 if small else 1) if n else 0
     assert q.is_contiguous() and out.is_contiguous()
     _check(load().sx_sparse_attn(ctypes.byref(pool.c), ctypes.byref(batch.c), 1 if full else 0, _ptr(q),
                                  _ptr(rows_R), _ptr(rows_off), n, _ptr(out), _ptr(lse), _ptr(ws), ws.numel(),

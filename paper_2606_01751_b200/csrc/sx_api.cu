@@ -37,6 +37,8 @@ WsLayout ws_layout(const sx_pool *pool, const sx_batch *b) {
   off = align_up(off + sizeof(float) * (size_t)pool->num_kv_heads * b->total_tokens, 256);
   w.scores = off;
   off = align_up(off + sizeof(float) * (size_t)b->total_tokens, 256);
+  w.small_part = off;
+  off = align_up(off + small_ws_bytes(b->num_reqs, pool->num_kv_heads, pool->num_q_heads / pool->num_kv_heads), 256);
   w.total = off;
   return w;
 }
@@ -221,8 +223,6 @@ sx_status sx_sparse_attn(const sx_pool *pool, const sx_batch *batch, int32_t mod
                          void *ws, size_t ws_bytes, sx_stream stream) {
   sx_status st = validate(pool, batch);
   if (st != SX_OK) return st;
-  (void)ws;
-  (void)ws_bytes;
   if (mode != 0 && mode != 1) return set_error(SX_ERR_INVALID_ARG, "mode must be 0 (sparse rows) or 1 (full)");
   if (total_rows < 0) return set_error(SX_ERR_INVALID_ARG, "total_rows < 0");
   if (total_rows == 0) return SX_OK;
@@ -232,9 +232,21 @@ sx_status sx_sparse_attn(const sx_pool *pool, const sx_batch *batch, int32_t mod
   if (mode == 1) {
     if (total_rows != batch->total_tokens)
       return set_error(SX_ERR_INVALID_ARG, "full mode: total_rows must equal total_tokens");
-    return launch_attn(pool, batch, true, q, nullptr, batch->tok_off, total_rows, out, lse, s);
+    rows_R = nullptr;
+    rows_off = batch->tok_off;
+  } else if (!rows_R || !rows_off) {
+    return set_error(SX_ERR_INVALID_ARG, "rows_R / rows_off is NULL");
   }
-  if (!rows_R || !rows_off) return set_error(SX_ERR_INVALID_ARG, "rows_R / rows_off is NULL");
+  // Dispatch (BASELINE.json north_star): tcgen05 tiles only where GQA packing gives at least 64 query
+  // rows per KV head; with fewer (on average over the batch) the CUDA-core split-KV path streams K/V.
+  const int g = pool->num_q_heads / pool->num_kv_heads;
+  if (g <= 32 && (int64_t)total_rows * g < (int64_t)64 * batch->num_reqs) {
+    st = validate_ws(pool, batch, ws, ws_bytes);
+    if (st != SX_OK) return st;
+    WsLayout w = ws_layout(pool, batch);
+    return launch_attn_small(pool, batch, q, rows_R, rows_off, total_rows, out, lse,
+                             reinterpret_cast<float *>(static_cast<char *>(ws) + w.small_part), s);
+  }
   return launch_attn(pool, batch, true, q, rows_R, rows_off, total_rows, out, lse, s);
 }
 

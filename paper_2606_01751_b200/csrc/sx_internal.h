@@ -20,6 +20,7 @@ struct WsLayout {
   size_t lse_new;      // float  [total_new][Hq]          sweep-1 normaliser (natural log)
   size_t partial;      // float  [Hkv][total_tokens]      per-kv-head column sums of A_sq
   size_t scores;       // float  [total_tokens]           head-summed scores when the caller passes none
+  size_t small_part;   // float  split-KV partials of the CUDA-core attention path (sx_attn_small.cu)
   size_t total;
 };
 WsLayout ws_layout(const sx_pool *pool, const sx_batch *batch);
@@ -37,6 +38,11 @@ sx_status launch_select(const sx_pool *pool, const sx_batch *b, const float *par
 // tcgen05 kernels. q_rows: bf16 [total_rows][Hq][128]; rows == nullptr => row n is position n - off[req].
 sx_status launch_attn(const sx_pool *pool, const sx_batch *b, bool with_pv, const void *q, const int32_t *rows,
                       const int32_t *rows_off, int32_t total_rows, void *out, float *lse, cudaStream_t st);
+// CUDA-core split-KV attention for fewer than 64 (row, head) pairs per KV head; part = ws.small_part
+sx_status launch_attn_small(const sx_pool *pool, const sx_batch *b, const void *q, const int32_t *rows,
+                            const int32_t *rows_off, int32_t total_rows, void *out, float *lse, float *part,
+                            cudaStream_t st);
+size_t small_ws_bytes(int num_reqs, int num_kv_heads, int group);
 sx_status launch_colsum(const sx_pool *pool, const sx_batch *b, const void *q_new, const float *lse_new,
                         int lse_by_token, float *partial, cudaStream_t st);
 

@@ -92,6 +92,10 @@ class GpuLayer:
         self.kf_sel = self.k_fresh[ts].contiguous()
         self.vf_sel = self.v_fresh[ts].contiguous()
         self.q_R = self.q_full[tr].contiguous()
+        # all recomputed rows at once (R is known before the layer starts when an earlier boundary
+        # selection is reused: one scatter of K/V_fresh[R], Alg. 1 l.544)
+        self.kf_R = self.k_fresh[tr].contiguous()
+        self.vf_R = self.v_fresh[tr].contiguous()
 
     def scatter_sel(self):
         if self.sel_idx.numel():
@@ -111,13 +115,15 @@ class GpuLayer:
         """rows_given: (sel_idx, rows_R) device tensors from an earlier boundary selection (paper mode)."""
         if do_realign:
             self.realign()
-        self.scatter_new()
         if rows_given is None:
+            self.scatter_new()
             self.select(want_scores=want_scores)
             self.stage_rows(self.sel_idx, self.rows_R)
+            self.scatter_sel()
         else:
             self.stage_rows(*rows_given)
-        self.scatter_sel()
+            sx.scatter_kv(self.pool, self.batch, self.kf_R, self.vf_R, self.rows_R, self.rows_off,
+                          max_rows=int(self.rows_R.numel()))
         self.attend()
 
     def step_full(self, do_realign: bool = True, want_lse: bool = True):

@@ -1,0 +1,40 @@
+#!/usr/bin/env python
+"""Writes tests/golden/carve_<cfg>.txt: the top-k margin carve (readings A9/A10) of the FULL-SIZE
+seeded workloads C2..C5, layer 0, so that the full-size GPU parity tests replay it instead of iterating
+the fp64 oracle (minutes per config). Calls only oracle/ (through tests/helpers.py) and the seeded input
+generator; nothing here touches the CUDA path.
+
+    python tests/golden/make_carve.py [C2 C3 C4 C5]
+
+Each line: physical block, row in block, scale applied to that key row (all KV heads), in application order.
+"""
+import os
+import sys
+import time
+
+HERE = os.path.dirname(os.path.abspath(__file__))
+sys.path.insert(0, os.path.dirname(HERE))
+sys.path.insert(0, os.path.dirname(os.path.dirname(HERE)))
+
+from helpers import carve_margins  # noqa: E402
+from paper_2606_01751_b200 import workloads as wl  # noqa: E402
+
+
+def main():
+    for name in (sys.argv[1:] or ["C2", "C3", "C4", "C5"]):
+        t0 = time.time()
+        lay = wl.CONFIGS[name]()
+        lt = wl.build_layer(lay, 0)
+        log = []
+        hist = carve_margins(lay, lt, log=log)
+        with open(os.path.join(HERE, "carve_%s.txt" % name), "w") as f:
+            f.write("# margin carve of workloads.CONFIGS[%r](), layer 0, tau = 1e-3; band sizes per iteration %r\n"
+                    % (name, hist))
+            f.write("# written by tests/golden/make_carve.py (fp64 oracle only); columns: block row scale\n")
+            for blk, row, scale in log:
+                f.write("%d %d %.2f\n" % (blk, row, scale))
+        print(name, hist, len(log), "ops, %.0f s" % (time.time() - t0), flush=True)
+
+
+if __name__ == "__main__":
+    main()

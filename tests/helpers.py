@@ -49,19 +49,25 @@ def oracle_scores_after_realign(lay: wl.LayerTensors, lt: wl.LayerTensors):
     return out
 
 
-def carve_margins(lay: wl.Layout, lt: wl.LayerTensors, tau: float = 1e-3, max_iter: int = 12):
+def carve_margins(lay: wl.Layout, lt: wl.LayerTensors, tau: float = 1e-3, max_iter: int = 12, log=None):
     """Reading A9/A10: the x4 salient tokens alone do not make the rank-k cut unambiguous
     (ratio > salient fraction, the cut falls among ordinary tokens). Enforce a relative margin at the
     cut: every cached token whose fp64 score lies within tau of the midpoint c between ranks k and k+1
     has its SOURCE key row rescaled (x1.25 above the cut, x0.8 below), re-rounded to bf16; repeat until
     the band is empty and the gap is >= 2 tau. Modifies lt.pool_k in place; returns per-iteration band
-    sizes. Uses the oracle, hence lives in tests/.
+    sizes. Uses the oracle, hence lives in tests/. `log` (a list) receives every (block, row, scale)
+    applied, in order, so that the result can be replayed with apply_carve (tests/golden/carve_*.txt).
     """
     hist = []
     bs = wl.PAGE
-    for _ in range(max_iter):
+    for it in range(max_iter):
+        # every rescaled key also moves the softmax normalisers, hence the cut itself, by a few 1e-4
+        # relative: clear a wider band (3 tau first, 1.5 tau later) than the one that must end up empty
+        widen = 3.0 if it == 0 else 1.5
         sc = oracle_scores_after_realign(lay, lt)
         band_total = 0
+        touched = set()     # a source row shared by two requests is moved once per iteration (else a row that
+                            # sits above one request's cut and below another's is scaled x1.25 x0.8 = x1)
         for r in range(lay.num_reqs):
             k = int(lay.k_per_req[r])
             is_new = lay.is_new_mask(r)
@@ -72,9 +78,9 @@ def carve_margins(lay: wl.Layout, lt: wl.LayerTensors, tau: float = 1e-3, max_it
             order = np.lexsort((cand, -s))
             c = 0.5 * (s[order[k - 1]] + s[order[k]])
             gap_ok = (s[order[k - 1]] - s[order[k]]) >= 2 * tau * c
-            band = np.nonzero(np.abs(s - c) <= tau * c)[0]
-            if gap_ok and len(band) == 0:
+            if gap_ok and not np.any(np.abs(s - c) <= tau * c):
                 continue
+            band = np.nonzero(np.abs(s - c) <= widen * tau * c)[0]
             if len(band) == 0:          # gap too small but nobody inside the band: push the two neighbours
                 band = np.asarray([order[k - 1], order[k]])
             band_total += len(band)
@@ -87,13 +93,36 @@ def carve_margins(lay: wl.Layout, lt: wl.LayerTensors, tau: float = 1e-3, max_it
                     if rq == r and new_pos <= pos < new_pos + ln:
                         j = pos - new_pos
                         blk = int(lay.src_blocks[src_off + j // bs])
+                        if (blk, j % bs) in touched:
+                            break
+                        touched.add((blk, j % bs))
                         row = orc.bf16_to_f64(lt.pool_k[blk, :, j % bs, :]) * scale
                         lt.pool_k[blk, :, j % bs, :] = orc.f64_to_bf16(row)
+                        if log is not None:
+                            log.append((blk, j % bs, scale))
                         break
         hist.append(band_total)
         if band_total == 0:
             return hist
     raise RuntimeError("margin carving did not converge: %r" % hist)
+
+
+def apply_carve(lt: wl.LayerTensors, ops):
+    """Replay a carve log: key row (block, row) of every KV head times scale, re-rounded to bf16, in order."""
+    for blk, row, scale in ops:
+        v = orc.bf16_to_f64(lt.pool_k[blk, :, row, :]) * scale
+        lt.pool_k[blk, :, row, :] = orc.f64_to_bf16(v)
+
+
+def load_carve(path):
+    ops = []
+    with open(path) as f:
+        for ln in f:
+            if ln.startswith("#") or not ln.strip():
+                continue
+            a, b, c = ln.split()
+            ops.append((int(a), int(b), float(c)))
+    return ops
 
 
 def check_close(name, got, ref64, max_abs=MAX_ABS, mean_abs=MEAN_ABS, ulp_floor=False):

@@ -262,3 +262,49 @@ def test_determinism():
         outs.append((g.scores.cpu().numpy().copy(), dev_to_bits(g.out).copy(), g.rows_R.cpu().numpy().copy()))
     for a, b in zip(outs[0], outs[1]):
         assert np.array_equal(a, b)
+
+
+SMALL_CASES = {
+    # name: (prepared case, rows per request as a function of (T, request index))
+    "tiny-last3": ("tiny", lambda t, r: np.arange(t - 3, t)),
+    "tiny-ragged-mixed": ("tiny-ragged", lambda t, r: np.asarray([0, 1, t // 2, t - 1])),
+    "tiny-g7-5rows": ("tiny-g7", lambda t, r: np.asarray([0, 17, t // 3, t - 2, t - 1])),
+    "tiny-g1": ("tiny-g1", lambda t, r: np.arange(t - 9, t)),
+    "C1-last8": ("C1", lambda t, r: np.arange(t - 8, t)),                   # 32 pairs per KV head
+    "C1-15-scattered": ("C1", lambda t, r: np.unique(np.linspace(0, t - 1, 15).astype(np.int64))),
+    "C2q-chunked": ("C2-quarter", lambda t, r: np.arange(t - (7 if r == 0 else 1), t) if r else
+                    np.unique(np.linspace(5, t - 1, 7).astype(np.int64))),
+    "C4e-one-row-each": ("C4-eighth", lambda t, r: np.asarray([t - 1])),    # decode-like: 4 pairs per KV head
+    "C5-last2": ("C5-1/16", lambda t, r: np.arange(t - 2, t)),               # g = 7: 14 pairs per KV head
+}
+
+
+@pytest.mark.parametrize("case", list(SMALL_CASES))
+def test_small_row_sets_cuda_core_path(case):
+    """Fewer than 64 (row, head) pairs per KV head: sx_sparse_attn takes the CUDA-core split-KV path
+    (north_star); same definition O-c, same tolerance."""
+    GpuLayer, dev_to_bits = _gpu()
+    name, pick = SMALL_CASES[case]
+    lay, lt, res, pk, pv, kt, vt = prepared(name)
+    g = GpuLayer(lay, lt)
+    g.step_sparse()
+    rows, off = [], [0]
+    for r in range(lay.num_reqs):
+        rr = np.asarray(pick(int(lay.seq_len[r]), r), dtype=np.int32)
+        rows.append(rr)
+        off.append(off[-1] + len(rr))
+    gq = lay.num_q_heads // lay.num_kv_heads
+    assert off[-1] * gq < 64 * lay.num_reqs          # the dispatch rule of include/sparsex.h
+    g.rows_off = torch.tensor(off, dtype=torch.int32, device=g.dev)
+    g.sel_off = torch.zeros(lay.num_reqs + 1, dtype=torch.int32, device=g.dev)
+    g.stage_rows(torch.zeros(0, dtype=torch.int32, device=g.dev), torch.from_numpy(np.concatenate(rows)).to(g.dev))
+    g.attend()
+    torch.cuda.synchronize()
+    out = orc.bf16_to_f64(dev_to_bits(g.out))
+    lse = g.lse.cpu().numpy().astype(np.float64)
+    for r in range(lay.num_reqs):
+        o, t = int(lay.tok_off[r]), int(lay.seq_len[r])
+        ref_o, ref_l = orc.attention(pk, pv, kt[r], vt[r], t, lt.q_full[o + rows[r]], rows[r], lay.num_q_heads,
+                                     want_lse=True)
+        check_close("%s req %d O" % (case, r), out[off[r]:off[r + 1]], ref_o)
+        assert np.max(np.abs(lse[off[r]:off[r + 1]] - ref_l)) < 2e-3
