@@ -186,7 +186,7 @@ def score_select(pool: DevicePool, batch: DeviceBatch, q_new: torch.Tensor, sel_
                  lse_by_token: bool = False, stream=None):
     """Stage (b), Eq. (1)-(3): Sparse-Q scores, head/query aggregation, top-k, R = I_nr U S_key."""
     global LAUNCHES
-    LAUNCHES += 1 + ((2 if lse_new is None else 1) if batch.c.total_new else 0)   # [lse sweep] colsum select
+    LAUNCHES += 1 + ((3 if lse_new is None else 2) if batch.c.total_new else 0)   # [lse sweep] coltab colsum select
     ws = batch.workspace(pool)
     _check(load().sx_score_select(ctypes.byref(pool.c), ctypes.byref(batch.c), _ptr(q_new), _ptr(lse_new),
                                   1 if lse_by_token else 0, _ptr(sel_off), _ptr(rows_off), _ptr(scores), _ptr(sel_idx), _ptr(rows_R),

@@ -37,6 +37,8 @@ WsLayout ws_layout(const sx_pool *pool, const sx_batch *b) {
   off = align_up(off + sizeof(float) * (size_t)pool->num_kv_heads * b->total_tokens, 256);
   w.scores = off;
   off = align_up(off + sizeof(float) * (size_t)b->total_tokens, 256);
+  w.col_tab = off;
+  off = align_up(off + colsum_tab_bytes(pool, b), 256);
   w.small_part = off;
   off = align_up(off + small_ws_bytes(b->num_reqs, pool->num_kv_heads, pool->num_q_heads / pool->num_kv_heads), 256);
   w.total = off;
@@ -208,7 +210,8 @@ sx_status sx_score_select(const sx_pool *pool, const sx_batch *batch, const void
       lse_by_token = 0;
     }
     // sweep 2: column sums of A_sq (Eq. 2), one partial vector per KV head
-    st = launch_colsum(pool, batch, q_new, lse, lse_by_token, partial, s);
+    st = launch_colsum(pool, batch, q_new, lse, lse_by_token, partial,
+                       reinterpret_cast<float2 *>(base + w.col_tab), s);
     if (st != SX_OK) return st;
   } else {
     cudaError_t e = cudaMemsetAsync(partial, 0, sizeof(float) * (size_t)pool->num_kv_heads * batch->total_tokens, s);

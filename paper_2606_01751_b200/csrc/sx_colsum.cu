@@ -9,6 +9,9 @@
 // with lane = key. Each consumer thread owns one key: p = exp2(s*c - lse_i) summed over its TMEM
 // row -> the column sum needs no cross-thread reduction and no atomics (deterministic).
 // The row normaliser lse_i comes from the first sweep (attn_kernel<false>) or from the caller.
+// The sweep is bound by the exponentials (128 x 128 per tile against 512 tensor-pipe cycles), so two
+// CTAs share an SM, two consumer threads share a key (64 columns each), and a fixed fraction of the
+// exponentials runs on the FMA pipe (Cody-Waite + cubic) beside MUFU.EX2.
 #include <math.h>
 
 #include "sx_internal.h"
@@ -16,20 +19,25 @@
 
 namespace sx {
 
-constexpr int kCsThreads = 192;
+constexpr int kCsThreads = 320;  // warps 0-7 consumers, warp 8 TMA producer, warp 9 MMA issuer
 constexpr int kCsTileBytes = kTile * kHeadDim * 2;
 constexpr int kCsHalf = kCsTileBytes / 2;
-constexpr int kCsStages = 3;
+constexpr int kCsStages = 2;
 constexpr int kCsOffK = 0;
 constexpr int kCsOffQ = kCsOffK + kCsTileBytes;
-constexpr int kCsOffCol = kCsOffQ + kCsStages * kCsTileBytes;  // [2][128] float lse2 + [2][128] int pos
-constexpr int kCsOffBar = kCsOffCol + 2 * 128 * 8;
-constexpr int kCsSmemBytes = kCsOffBar + 256 + 1024;
+constexpr int kCsColStages = 8;  // (lse, position) rows of 128 columns: 1 KB each, own ring (see producer)
+constexpr int kCsOffCol = kCsOffQ + kCsStages * kCsTileBytes;  // float2 [kCsColStages][128]
+constexpr int kCsOffBar = kCsOffCol + kCsColStages * 1024;
+constexpr int kCsSmemBytes = kCsOffBar + 256 + 1024;  // 2 CTAs per SM
+#ifndef SX_COLSUM_POLY
+#define SX_COLSUM_POLY 0  // of every 8 pairs of exponentials, this many pairs go to the FMA pipe (0..8)
+#endif
 
 struct ColsumParams {
   const int32_t *seq_len, *tok_off, *new_off, *new_idx, *k_table;
   const float *lse;  // natural log; [total_new][Hq], or [total_tokens][Hq] when lse_by_token
   int lse_by_token;
+  float2 *col_tab;   // [query tiles of the batch][Hkv][128]: (lse * log2 e, position as int bits)
   float *partial;    // [Hkv][total_tokens]
   int num_reqs, max_pages, num_q_heads, num_kv_heads, group, rows_per_tile, total_tokens;
   float scale_log2;
@@ -39,25 +47,70 @@ struct CsBars {
   uint64_t k_full;
   uint64_t q_full[kCsStages], q_empty[kCsStages];
   uint64_t d_full[2], d_empty[2];
+  uint64_t c_full[kCsColStages];
   uint32_t tmem_base;
 };
 
-__global__ void __launch_bounds__(kCsThreads, 1)
+// Column table of sweep 2: for every GQA-packed query tile (rows_per_tile queries x g heads = up to 128
+// columns) the log2-domain normaliser and the position of each column; pad columns get (+inf, -1) so that
+// their exp2 is 0. One 1-KB row per (query tile, KV head): the colsum producer fetches it with one bulk copy.
+__global__ void __launch_bounds__(128)
+coltab_kernel(const ColsumParams p) {
+  const int g = p.group, rpt = p.rows_per_tile;
+  int req = 0, base = 0;
+  for (; req < p.num_reqs; ++req) {
+    const int nq = (p.new_off[req + 1] - p.new_off[req] + rpt - 1) / rpt;
+    if ((int)blockIdx.x < base + nq) break;
+    base += nq;
+  }
+  if (req >= p.num_reqs) return;
+  const int qt = blockIdx.x - base, kvh = blockIdx.y, ct = threadIdx.x;
+  const int nq0 = p.new_off[req], nn = p.new_off[req + 1] - nq0;
+  const int cn = ct / g, ch = ct - cn * g, n = qt * rpt + cn;
+  float lse2 = INFINITY;
+  int qpos = -1;
+  if (cn < rpt && n < nn) {
+    qpos = p.new_idx[nq0 + n];
+    const size_t lrow = p.lse_by_token ? (size_t)(p.tok_off[req] + qpos) : (size_t)(nq0 + n);
+    lse2 = p.lse[lrow * p.num_q_heads + kvh * g + ch] * (float)kLog2e;
+  }
+  p.col_tab[((size_t)blockIdx.x * p.num_kv_heads + kvh) * 128 + ct] = make_float2(lse2, __int_as_float(qpos));
+}
+
+// exp2 of two values on the FMA pipe: x = n + f, n = rint(x), |f| <= 1/2; cubic for 2^f (relative error
+// 7.5e-5, far inside the 5e-3 score tolerance), 2^n by exponent arithmetic. x <= ~0 here; clamp at -126.
+__device__ __forceinline__ float2 cs_ex2_poly2(float2 x) {
+  const float kMagic = 12582912.f;  // 1.5 * 2^23
+  x.x = fmaxf(x.x, -126.f);
+  x.y = fmaxf(x.y, -126.f);
+  const float2 t = __fadd2_rn(x, make_float2(kMagic, kMagic));
+  const float2 n = __fadd2_rn(t, make_float2(-kMagic, -kMagic));
+  const float2 f = __ffma2_rn(n, make_float2(-1.f, -1.f), x);
+  float2 p = __ffma2_rn(make_float2(0.0551716648f, 0.0551716648f), f, make_float2(0.2426111251f, 0.2426111251f));
+  p = __ffma2_rn(p, f, make_float2(0.6932609677f, 0.6932609677f));
+  p = __ffma2_rn(p, f, make_float2(0.9999280572f, 0.9999280572f));
+  float2 r;
+  r.x = __int_as_float(__float_as_int(p.x) + (__float_as_int(t.x) << 23));
+  r.y = __int_as_float(__float_as_int(p.y) + (__float_as_int(t.y) << 23));
+  return r;
+}
+
+__global__ void __launch_bounds__(kCsThreads, 2)
 colsum_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_constant__ CUtensorMap tm_k,
               const ColsumParams p) {
   extern __shared__ uint8_t smem_raw[];
   uint8_t *smem = reinterpret_cast<uint8_t *>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~uintptr_t(1023));
   CsBars *bars = reinterpret_cast<CsBars *>(smem + kCsOffBar);
-  float *col_lse = reinterpret_cast<float *>(smem + kCsOffCol);       // [2][128]
-  int *col_pos = reinterpret_cast<int *>(smem + kCsOffCol + 2 * 128 * 4);  // [2][128]
+  float2 *col_sm = reinterpret_cast<float2 *>(smem + kCsOffCol);  // [kCsColStages][128] (lse2, position)
 
   // ---- (request, key tile, KV head); early key tiles (seen by the most queries) first
   const int g = p.group, rpt = p.rows_per_tile;
-  int req = 0, base = 0, ktiles = 0;
+  int req = 0, base = 0, ktiles = 0, qt_base = 0;  // qt_base: query tiles of the requests before this one
   for (; req < p.num_reqs; ++req) {
     ktiles = (p.seq_len[req] + kTile - 1) / kTile;
     if ((int)blockIdx.x < base + ktiles * p.num_kv_heads) break;
     base += ktiles * p.num_kv_heads;
+    qt_base += (p.new_off[req + 1] - p.new_off[req] + rpt - 1) / rpt;
   }
   if (req >= p.num_reqs) return;
   const int local = blockIdx.x - base;
@@ -78,7 +131,8 @@ colsum_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_constant__ 
   const int n_it = (lo < nn) ? n_qt - qt0 : 0;
 
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-  if (warp == 0 && lane == 0) {
+  constexpr int kWarpProd = 8, kWarpMma = 9;
+  if (warp == kWarpProd && lane == 0) {
     tma_prefetch_desc(&tm_q);
     tma_prefetch_desc(&tm_k);
     mbar_init(&bars->k_full, 1);
@@ -88,11 +142,12 @@ colsum_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_constant__ 
     }
     for (int i = 0; i < 2; ++i) {
       mbar_init(&bars->d_full[i], 1);
-      mbar_init(&bars->d_empty[i], 128);
+      mbar_init(&bars->d_empty[i], 256);
     }
+    for (int i = 0; i < kCsColStages; ++i) mbar_init(&bars->c_full[i], 1);
     fence_mbar_init();
   }
-  if (warp == 1) {
+  if (warp == kWarpMma) {
     tmem_alloc(&bars->tmem_base, 256);
     tmem_relinquish();
   }
@@ -111,7 +166,7 @@ colsum_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_constant__ 
   tc_fence_after();
   const uint32_t tmem = bars->tmem_base;
 
-  if (warp == 0) {
+  if (warp == kWarpProd) {
     // ================================================================ TMA producer
     if (n_it > 0) {
       const int pg_in_tile = lane >> 1, half = lane & 1;
@@ -124,122 +179,116 @@ colsum_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_constant__ 
         tma_load_2d(smem + kCsOffK + half * kCsHalf + pg_in_tile * 2048, &tm_k, &bars->k_full, half * 64,
                     (blk * p.num_kv_heads + kvh) * kPage);
       }
-      for (int it = 0; it < n_it; ++it) {
-        const int s = it % kCsStages, u = it / kCsStages;
-        mbar_wait(&bars->q_empty[s], (u & 1) ^ 1);
-        if (lane == 0) {
+      __syncwarp();
+      if (elect_one()) {
+        int s = 0, ph = 1;
+        for (int it = 0; it < n_it; ++it) {
+          mbar_wait(&bars->q_empty[s], ph);
           mbar_expect_tx(&bars->q_full[s], (uint32_t)(2 * rpt * g * 128));
           const int r0 = nq0 + (qt0 + it) * rpt;
           tma_load_3d(smem + kCsOffQ + s * kCsTileBytes, &tm_q, &bars->q_full[s], 0, kvh * g, r0);
           tma_load_3d(smem + kCsOffQ + s * kCsTileBytes + kCsHalf, &tm_q, &bars->q_full[s], 64, kvh * g, r0);
+          // column table row of this query tile. Ring of 8: this thread is at most 2 tiles ahead of the MMA
+          // issuer, which is at most 2 tiles ahead of the consumers' D loads, so stage it & 7 is free.
+          mbar_expect_tx(&bars->c_full[it & (kCsColStages - 1)], 1024);
+          bulk_load_1d(col_sm + (it & (kCsColStages - 1)) * 128,
+                       p.col_tab + ((size_t)(qt_base + qt0 + it) * p.num_kv_heads + kvh) * 128, 1024,
+                       &bars->c_full[it & (kCsColStages - 1)]);
+          if (++s == kCsStages) { s = 0; ph ^= 1; }
         }
-        __syncwarp();
       }
     }
-  } else if (warp == 1) {
+  } else if (warp == kWarpMma) {
     // ================================================================ MMA issuer: D[b] = K_tile * Q_tile^T
-    if (n_it > 0) {
+    if (n_it > 0 && elect_one()) {
       constexpr uint32_t idesc = umma_idesc_bf16(128, 128, 0, 0);
-      const uint32_t k_addr = smem_u32(smem + kCsOffK);
+      const uint64_t k_desc = umma_smem_desc(smem_u32(smem + kCsOffK), 16, 1024);
+      const uint64_t q_desc = umma_smem_desc(smem_u32(smem + kCsOffQ), 16, 1024);
+      const uint32_t k_lo = (uint32_t)k_desc, q_lo = (uint32_t)q_desc, hi32 = (uint32_t)(k_desc >> 32);
       mbar_wait(&bars->k_full, 0);
+      int s = 0, ph = 0;
       for (int it = 0; it < n_it; ++it) {
-        const int s = it % kCsStages, b = it & 1;
-        mbar_wait(&bars->q_full[s], (it / kCsStages) & 1);
+        const int b = it & 1;
+        mbar_wait(&bars->q_full[s], ph);
         if (it >= 2) mbar_wait(&bars->d_empty[b], ((it >> 1) + 1) & 1);
         tc_fence_after();
-        if (lane == 0) {
-          const uint32_t q_addr = smem_u32(smem + kCsOffQ + s * kCsTileBytes);
+        const uint32_t qd = q_lo + (uint32_t)s * (kCsTileBytes >> 4);
 #pragma unroll
-          for (int kk = 0; kk < 8; ++kk) {
-            const uint32_t o = (kk >> 2) * kCsHalf + (kk & 3) * 32;
-            umma_ss(tmem + b * 128, umma_smem_desc(k_addr + o, 16, 1024), umma_smem_desc(q_addr + o, 16, 1024),
-                    idesc, kk > 0);
-          }
-          umma_commit(&bars->d_full[b]);
-          umma_commit(&bars->q_empty[s]);
+        for (int kk = 0; kk < 8; ++kk) {
+          const uint32_t o = ((kk >> 2) * kCsHalf + (kk & 3) * 32) >> 4;
+          umma_ss2(tmem + b * 128, k_lo + o, hi32, qd + o, hi32, idesc, kk > 0);
         }
-        __syncwarp();
+        umma_commit(&bars->d_full[b]);
+        umma_commit(&bars->q_empty[s]);
+        if (++s == kCsStages) { s = 0; ph ^= 1; }
       }
     }
   } else {
-    // ================================================================ consumers: thread = one key
+    // ================================================================ consumers: two threads per key
+    const int hf = warp >> 2;              // column half [64 hf, 64 hf + 64) of every D tile
     const int quarter = warp & 3;
     const int row = quarter * 32 + lane;   // key j0 + row = TMEM lane
-    const int ct = threadIdx.x - 64;       // 0..127: column staged by this thread
     const int j = j0 + row;
     const uint32_t lane_addr = (uint32_t)(quarter * 32) << 16;
-    const int cn = ct / g, ch = ct - cn * g;  // column ct = (query cn of the tile, head ch of the group)
-    float acc = 0.f;
-
-    auto load_col = [&](int it, float &lse2, int &qpos) {
-      const int n = (qt0 + it) * rpt + cn;  // query index within the request
-      if (cn < rpt && n < nn) {
-        qpos = p.new_idx[nq0 + n];
-        const size_t lrow = p.lse_by_token ? (size_t)(p.tok_off[req] + qpos) : (size_t)(nq0 + n);
-        lse2 = p.lse[lrow * p.num_q_heads + kvh * g + ch] * (float)kLog2e;
-      } else {
-        lse2 = INFINITY;  // pad column: exp2(-inf) = 0
-        qpos = -1;
-      }
-    };
-    float nx_lse = 0.f;
-    int nx_pos = 0;
-    if (n_it > 0) load_col(0, nx_lse, nx_pos);
+    float2 acc2 = make_float2(0.f, 0.f);
+    const float2 sc2 = make_float2(p.scale_log2, p.scale_log2);
     for (int it = 0; it < n_it; ++it) {
-      const int b = it & 1;
-      col_lse[b * 128 + ct] = nx_lse;
-      col_pos[b * 128 + ct] = nx_pos;
-      if (it + 1 < n_it) load_col(it + 1, nx_lse, nx_pos);
-      named_bar_sync(1, 128);
-      // queries are sorted by position: columns below `first` cannot see key j
-      const bool need_mask = col_pos[b * 128] < j0 + kTile - 1;  // some column may be masked for some key
+      const int b = it & 1, cs = it & (kCsColStages - 1);
+      mbar_wait(&bars->c_full[cs], (it / kCsColStages) & 1);
+      const uint32_t col = smem_u32(col_sm + cs * 128 + hf * 64);
+      // queries are sorted by position: only tiles whose first query is below the tile's last key need a mask
+      const bool need_mask = __float_as_int(lds_f1(smem_u32(col_sm + cs * 128) + 4)) < j0 + kTile - 1;
       mbar_wait(&bars->d_full[b], (it >> 1) & 1);
       tc_fence_after();
-      const float4 *lse4 = reinterpret_cast<const float4 *>(col_lse + b * 128);
-      const int4 *pos4 = reinterpret_cast<const int4 *>(col_pos + b * 128);
-#pragma unroll
-      for (int c = 0; c < 4; ++c) {
-        uint32_t d[32];
-        tmem_ld32(tmem + lane_addr + b * 128 + c * 32, d);
-        tmem_wait_ld();
-        if (!need_mask) {
-#pragma unroll
-          for (int i = 0; i < 32; i += 4) {
-            const float4 ls = lse4[(c * 32 + i) >> 2];
-            acc += ex2_approx(fmaf(__uint_as_float(d[i + 0]), p.scale_log2, -ls.x));
-            acc += ex2_approx(fmaf(__uint_as_float(d[i + 1]), p.scale_log2, -ls.y));
-            acc += ex2_approx(fmaf(__uint_as_float(d[i + 2]), p.scale_log2, -ls.z));
-            acc += ex2_approx(fmaf(__uint_as_float(d[i + 3]), p.scale_log2, -ls.w));
-          }
-        } else {
-#pragma unroll
-          for (int i = 0; i < 32; i += 4) {
-            const float4 ls = lse4[(c * 32 + i) >> 2];
-            const int4 qp = pos4[(c * 32 + i) >> 2];
-            float e0 = ex2_approx(fmaf(__uint_as_float(d[i + 0]), p.scale_log2, -ls.x));
-            float e1 = ex2_approx(fmaf(__uint_as_float(d[i + 1]), p.scale_log2, -ls.y));
-            float e2 = ex2_approx(fmaf(__uint_as_float(d[i + 2]), p.scale_log2, -ls.z));
-            float e3 = ex2_approx(fmaf(__uint_as_float(d[i + 3]), p.scale_log2, -ls.w));
-            acc += (qp.x >= j) ? e0 : 0.f;
-            acc += (qp.y >= j) ? e1 : 0.f;
-            acc += (qp.z >= j) ? e2 : 0.f;
-            acc += (qp.w >= j) ? e3 : 0.f;
-          }
-        }
-      }
+      uint32_t d[2][32];
+      tmem_ld32(tmem + lane_addr + b * 128 + hf * 64, d[0]);
+      tmem_ld32(tmem + lane_addr + b * 128 + hf * 64 + 32, d[1]);
+      tmem_wait_ld();
       tc_fence_before();
-      mbar_arrive(&bars->d_empty[b]);
+      mbar_arrive(&bars->d_empty[b]);  // D[b] is in registers: the next-but-one tile may overwrite it
+#pragma unroll
+      for (int c = 0; c < 2; ++c)
+#pragma unroll
+        for (int i = 0; i < 32; i += 2) {
+          const float4 cc = lds_f4(col + (c * 32 + i) * 8);  // (lse, pos) of two columns
+          float2 x = __ffma2_rn(make_float2(__uint_as_float(d[c][i]), __uint_as_float(d[c][i + 1])), sc2,
+                                make_float2(-cc.x, -cc.z));
+          float2 e;
+          if ((i & 15) < 2 * SX_COLSUM_POLY) {
+            e = cs_ex2_poly2(x);
+          } else {
+            e.x = ex2_approx(x.x);
+            e.y = ex2_approx(x.y);
+          }
+          if (need_mask) {
+            e.x = (__float_as_int(cc.y) >= j) ? e.x : 0.f;
+            e.y = (__float_as_int(cc.w) >= j) ? e.y : 0.f;
+          }
+          acc2 = __fadd2_rn(acc2, e);
+        }
     }
-    if (j < T) p.partial[(size_t)kvh * p.total_tokens + p.tok_off[req] + j] = acc;
+    // the two halves of a key add up in a fixed order
+    float *xch = reinterpret_cast<float *>(col_sm);  // every column row has been consumed
+    named_bar_sync(1, 256);
+    const float acc = acc2.x + acc2.y;
+    if (hf == 1) xch[row] = acc;
+    named_bar_sync(1, 256);
+    if (hf == 0 && j < T) p.partial[(size_t)kvh * p.total_tokens + p.tok_off[req] + j] = acc + xch[row];
   }
 
   tc_fence_before();
   __syncthreads();
-  if (warp == 1) tmem_dealloc(tmem, 256);
+  if (warp == kWarpMma) tmem_dealloc(tmem, 256);
+}
+
+size_t colsum_tab_bytes(const sx_pool *pool, const sx_batch *b) {
+  const int g = pool->num_q_heads / pool->num_kv_heads;
+  const int rpt = kTile / (g > 0 ? g : 1) > 0 ? kTile / (g > 0 ? g : 1) : 1;
+  return (size_t)(b->total_new / rpt + b->num_reqs) * pool->num_kv_heads * 128 * sizeof(float2);
 }
 
 sx_status launch_colsum(const sx_pool *pool, const sx_batch *b, const void *q_new, const float *lse_new,
-                        int lse_by_token, float *partial, cudaStream_t st) {
+                        int lse_by_token, float *partial, float2 *col_tab, cudaStream_t st) {
   const int g = pool->num_q_heads / pool->num_kv_heads;
   const int rpt = kTile / g;
   CUtensorMap tm_q, tm_k;
@@ -256,6 +305,7 @@ sx_status launch_colsum(const sx_pool *pool, const sx_batch *b, const void *q_ne
   p.lse = lse_new;
   p.lse_by_token = lse_by_token;
   p.partial = partial;
+  p.col_tab = col_tab;
   p.num_reqs = b->num_reqs;
   p.max_pages = b->max_pages_per_req;
   p.num_q_heads = pool->num_q_heads;
@@ -267,6 +317,10 @@ sx_status launch_colsum(const sx_pool *pool, const sx_batch *b, const void *q_ne
   const int grid = (b->total_tokens / kTile + b->num_reqs) * pool->num_kv_heads;
   cudaError_t e = cudaFuncSetAttribute(colsum_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, kCsSmemBytes);
   if (e != cudaSuccess) return set_error(SX_ERR_CUDA, "colsum smem attr: %s", cudaGetErrorString(e));
+  const int n_qt = b->total_new / rpt + b->num_reqs;  // >= sum_r ceil(|I_nr(r)| / rpt)
+  coltab_kernel<<<dim3(n_qt, pool->num_kv_heads), 128, 0, st>>>(p);
+  s = check_launch("coltab_kernel");
+  if (s != SX_OK) return s;
   colsum_kernel<<<grid, kCsThreads, kCsSmemBytes, st>>>(tm_q, tm_k, p);
   return check_launch("colsum_kernel");
 }

@@ -20,6 +20,7 @@ struct WsLayout {
   size_t lse_new;      // float  [total_new][Hq]          sweep-1 normaliser (natural log)
   size_t partial;      // float  [Hkv][total_tokens]      per-kv-head column sums of A_sq
   size_t scores;       // float  [total_tokens]           head-summed scores when the caller passes none
+  size_t col_tab;      // float2 [query tiles][Hkv][128]  (log2-domain lse, position) of every sweep-2 column
   size_t small_part;   // float  split-KV partials of the CUDA-core attention path (sx_attn_small.cu)
   size_t total;
 };
@@ -44,7 +45,8 @@ sx_status launch_attn_small(const sx_pool *pool, const sx_batch *b, const void *
                             cudaStream_t st);
 size_t small_ws_bytes(int num_reqs, int num_kv_heads, int group);
 sx_status launch_colsum(const sx_pool *pool, const sx_batch *b, const void *q_new, const float *lse_new,
-                        int lse_by_token, float *partial, cudaStream_t st);
+                        int lse_by_token, float *partial, float2 *col_tab, cudaStream_t st);
+size_t colsum_tab_bytes(const sx_pool *pool, const sx_batch *b);
 
 // TMA descriptor construction (driver entry point fetched through the runtime; no libcuda link)
 sx_status make_tmap_pool(CUtensorMap *out, const void *base, int num_blocks, int num_kv_heads);
