@@ -32,7 +32,7 @@ WsLayout ws_layout(const sx_pool *pool, const sx_batch *b) {
   w.rope_table = off;
   off = align_up(off + sizeof(float2) * 64 * (size_t)(b->num_segments > 0 ? b->num_segments : 1), 256);
   w.lse_new = off;
-  off = align_up(off + sizeof(float) * (size_t)(b->total_new > 0 ? b->total_new : 1) * pool->num_q_heads, 256);
+  off = align_up(off + 8 * sizeof(float) * (size_t)(b->total_new > 0 ? b->total_new : 1) * pool->num_q_heads, 256);
   w.partial = off;
   off = align_up(off + sizeof(float) * (size_t)pool->num_kv_heads * b->total_tokens, 256);
   w.scores = off;
@@ -200,17 +200,19 @@ sx_status sx_score_select(const sx_pool *pool, const sx_batch *batch, const void
   float *partial = reinterpret_cast<float *>(base + w.partial);
   const float *lse = lse_new;
   if (lse_by_token != 0 && lse_by_token != 1) return set_error(SX_ERR_INVALID_ARG, "lse_by_token must be 0 or 1");
+  int lse_splits = 1;
   if (batch->total_new > 0) {
     if (!lse) {  // sweep 1: row normaliser of Eq. (1) for the Sparse-Q rows
       float *lse_ws = reinterpret_cast<float *>(base + w.lse_new);
+      lse_splits = attn_lse_splits(pool, batch, batch->total_new);
       st = launch_attn(pool, batch, /*with_pv=*/false, q_new, batch->new_idx, batch->new_off, batch->total_new,
-                       nullptr, lse_ws, s);
+                       nullptr, lse_ws, lse_splits, s);
       if (st != SX_OK) return st;
       lse = lse_ws;
       lse_by_token = 0;
     }
     // sweep 2: column sums of A_sq (Eq. 2), one partial vector per KV head
-    st = launch_colsum(pool, batch, q_new, lse, lse_by_token, partial,
+    st = launch_colsum(pool, batch, q_new, lse, lse_by_token, lse_splits, partial,
                        reinterpret_cast<float2 *>(base + w.col_tab), s);
     if (st != SX_OK) return st;
   } else {
@@ -250,7 +252,7 @@ sx_status sx_sparse_attn(const sx_pool *pool, const sx_batch *batch, int32_t mod
     return launch_attn_small(pool, batch, q, rows_R, rows_off, total_rows, out, lse,
                              reinterpret_cast<float *>(static_cast<char *>(ws) + w.small_part), s);
   }
-  return launch_attn(pool, batch, true, q, rows_R, rows_off, total_rows, out, lse, s);
+  return launch_attn(pool, batch, true, q, rows_R, rows_off, total_rows, out, lse, 1, s);
 }
 
 }  // extern "C"

@@ -47,6 +47,8 @@ struct AttnParams {
   __nv_bfloat16 *out;  // [total_rows][Hq][128]
   float *lse;          // [total_rows][Hq] or nullptr
   int num_reqs, max_pages, num_q_heads, num_kv_heads, group, rows_per_tile;
+  int total_rows;
+  int kv_splits;     // LSE-only variant: the key range of a CTA is cut into this many contiguous parts
   float scale_log2;  // log2(e) / sqrt(128)
   float scale;       // 1 / sqrt(128)
 };
@@ -97,15 +99,18 @@ attn_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_constant__ CU
 
   // ---- which (request, KV head, pair of row tiles) is this CTA; heavy (late) pairs of a request first
   const int g = p.group, rpt = p.rows_per_tile, rpc = 2 * rpt;
+  // LSE-only variant: consecutive blocks share a (request, KV head, row pair) and take one key split each
+  const int split = kWithPV ? 0 : (int)blockIdx.x % p.kv_splits;
+  const int bid = kWithPV ? (int)blockIdx.x : (int)blockIdx.x / p.kv_splits;
   int req = 0, base = 0, pairs = 0, n_r = 0;
   for (; req < p.num_reqs; ++req) {
     n_r = p.rows_off[req + 1] - p.rows_off[req];
     pairs = (n_r + rpc - 1) / rpc;
-    if ((int)blockIdx.x < base + pairs * p.num_kv_heads) break;
+    if (bid < base + pairs * p.num_kv_heads) break;
     base += pairs * p.num_kv_heads;
   }
   if (req >= p.num_reqs) return;
-  const int local = blockIdx.x - base;
+  const int local = bid - base;
   const int kvh = local % p.num_kv_heads;
   const int pair = pairs - 1 - local / p.num_kv_heads;
   const int row_base = p.rows_off[req] + pair * rpc;  // first row (batch-wide index) of query tile 0
@@ -125,6 +130,15 @@ attn_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_constant__ CU
     } else {
       n_t[i] = 0;
     }
+  }
+  // key tiles [t0, t0 + n_tiles) of this CTA; n_t[i] and every loop below count tiles from t0
+  int t0 = 0;
+  if (!kWithPV && p.kv_splits > 1) {
+    const int all = max(n_t[0], n_t[1]);
+    const int per = (all + p.kv_splits - 1) / p.kv_splits;
+    t0 = split * per;
+    n_t[0] = max(0, min(n_t[0], t0 + per) - t0);
+    n_t[1] = max(0, min(n_t[1], t0 + per) - t0);
   }
   const int n_tiles = max(n_t[0], n_t[1]);
 
@@ -191,7 +205,7 @@ attn_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_constant__ CU
       const int pg_in_tile = lane >> 1, half = lane & 1;
       const int n_items = kWithPV ? 2 * n_tiles : n_tiles;
       auto table_entry = [&](int it) -> int {
-        const int t = kWithPV ? (it >> 1) : it;
+        const int t = kWithPV ? (it >> 1) : t0 + it;
         const bool is_v = kWithPV && (it & 1);
         int lp = t * 8 + pg_in_tile;
         if (lp > n_pages - 1) lp = n_pages - 1;  // pages past the sequence: any valid page (keys are masked)
@@ -322,7 +336,7 @@ attn_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_constant__ CU
       tmem_ld32(tmem_s + b * 128 + 64, sr[2]);
       tmem_ld32(tmem_s + b * 128 + 96, sr[3]);
 
-      const int nvalid = pos - t * kTile + 1;  // keys [0, nvalid) of this tile are visible to this row
+      const int nvalid = pos - (t0 + t) * kTile + 1;  // keys [0, nvalid) of this tile are visible to this row
       float tm[2] = {-INFINITY, -INFINITY};  // two independent 3-input max chains
 #pragma unroll
       for (int c = 0; c < 4; ++c) {
@@ -364,7 +378,8 @@ attn_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_constant__ CU
           tmem_st32(tmem_o + c * 32, o);
         }
       }
-      const float neg_m = -m_used * p.scale_log2;
+      // a row that has seen no key yet (possible only in a later key split) keeps exp2(-inf) = 0
+      const float neg_m = (m_used == -INFINITY) ? 0.f : -m_used * p.scale_log2;
       const float2 sc2 = make_float2(p.scale_log2, p.scale_log2), nm2 = make_float2(neg_m, neg_m);
       float2 rsum2 = make_float2(0.f, 0.f);
 
@@ -418,7 +433,7 @@ attn_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_constant__ CU
     }
 
     // ---- epilogue
-    if (my_tiles > 0) {
+    if (my_tiles > 0 || !kWithPV) {  // (a key split that holds no tile of the row still reports lse = -inf)
       const size_t out_row = (size_t)grow * p.num_q_heads + kvh * g + hh;
       if (kWithPV) {
         mbar_wait(&bars->o_full[qt], 0);
@@ -443,7 +458,8 @@ attn_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_constant__ CU
           }
         }
       }
-      if (p.lse && valid) p.lse[out_row] = m_used * p.scale + logf(l);
+      if (p.lse && valid)
+        p.lse[(size_t)split * p.total_rows * p.num_q_heads + out_row] = m_used * p.scale + logf(l);
     }
   }
 
@@ -452,8 +468,18 @@ attn_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_constant__ CU
   if (warp == kWarpMma) tmem_dealloc(tmem, 512);
 }
 
+// Key splits of the LSE-only sweep: enough CTAs for about four waves (a long single request gives few row
+// pairs: C5 has 57 x 4 KV heads), at most 8. The partial normalisers are merged by coltab_kernel.
+int attn_lse_splits(const sx_pool *pool, const sx_batch *b, int32_t total_rows) {
+  const int g = pool->num_q_heads / pool->num_kv_heads;
+  const int grid = (total_rows / (2 * (kTile / g)) + b->num_reqs) * pool->num_kv_heads;
+  int s = (4 * 148 + grid - 1) / grid;
+  return s < 1 ? 1 : (s > 8 ? 8 : s);
+}
+
 sx_status launch_attn(const sx_pool *pool, const sx_batch *b, bool with_pv, const void *q, const int32_t *rows,
-                      const int32_t *rows_off, int32_t total_rows, void *out, float *lse, cudaStream_t st) {
+                      const int32_t *rows_off, int32_t total_rows, void *out, float *lse, int kv_splits,
+                      cudaStream_t st) {
   const int g = pool->num_q_heads / pool->num_kv_heads;
   const int rpt = kTile / g;
   CUtensorMap tm_q, tm_k, tm_v;
@@ -477,6 +503,8 @@ sx_status launch_attn(const sx_pool *pool, const sx_batch *b, bool with_pv, cons
   p.num_kv_heads = pool->num_kv_heads;
   p.group = g;
   p.rows_per_tile = rpt;
+  p.total_rows = total_rows;
+  p.kv_splits = with_pv ? 1 : kv_splits;
   p.scale = (float)(1.0 / sqrt((double)kHeadDim));
   p.scale_log2 = (float)(kLog2e / sqrt((double)kHeadDim));
   const int grid = (total_rows / (2 * rpt) + b->num_reqs) * pool->num_kv_heads;  // >= sum_r ceil(n_r / 2rpt) * Hkv
@@ -488,7 +516,7 @@ sx_status launch_attn(const sx_pool *pool, const sx_batch *b, bool with_pv, cons
   } else {
     e = cudaFuncSetAttribute(attn_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, AttnCfg::kSmemBytes);
     if (e != cudaSuccess) return set_error(SX_ERR_CUDA, "lse smem attr: %s", cudaGetErrorString(e));
-    attn_kernel<false><<<grid, kAttnThreads, AttnCfg::kSmemBytes, st>>>(tm_q, tm_k, tm_v, p);
+    attn_kernel<false><<<grid * p.kv_splits, kAttnThreads, AttnCfg::kSmemBytes, st>>>(tm_q, tm_k, tm_v, p);
   }
   return check_launch(with_pv ? "attn_kernel<pv>" : "attn_kernel<lse>");
 }

@@ -37,6 +37,8 @@ struct ColsumParams {
   const int32_t *seq_len, *tok_off, *new_off, *new_idx, *k_table;
   const float *lse;  // natural log; [total_new][Hq], or [total_tokens][Hq] when lse_by_token
   int lse_by_token;
+  int lse_splits;     // > 1: lse holds that many partial normalisers [split][total_new][Hq] (key splits)
+  size_t lse_stride;  // total_new * Hq
   float2 *col_tab;   // [query tiles of the batch][Hkv][128]: (lse * log2 e, position as int bits)
   float *partial;    // [Hkv][total_tokens]
   int num_reqs, max_pages, num_q_heads, num_kv_heads, group, rows_per_tile, total_tokens;
@@ -72,7 +74,16 @@ coltab_kernel(const ColsumParams p) {
   if (cn < rpt && n < nn) {
     qpos = p.new_idx[nq0 + n];
     const size_t lrow = p.lse_by_token ? (size_t)(p.tok_off[req] + qpos) : (size_t)(nq0 + n);
-    lse2 = p.lse[lrow * p.num_q_heads + kvh * g + ch] * (float)kLog2e;
+    const size_t idx = lrow * p.num_q_heads + kvh * g + ch;
+    float l = p.lse[idx];
+    if (p.lse_splits > 1) {  // log-sum-exp of the key splits, fixed order
+      float mx = l;
+      for (int s = 1; s < p.lse_splits; ++s) mx = fmaxf(mx, p.lse[s * p.lse_stride + idx]);
+      float sum = 0.f;
+      for (int s = 0; s < p.lse_splits; ++s) sum += expf(p.lse[s * p.lse_stride + idx] - mx);
+      l = mx + logf(sum);
+    }
+    lse2 = l * (float)kLog2e;
   }
   p.col_tab[((size_t)blockIdx.x * p.num_kv_heads + kvh) * 128 + ct] = make_float2(lse2, __int_as_float(qpos));
 }
@@ -288,7 +299,7 @@ size_t colsum_tab_bytes(const sx_pool *pool, const sx_batch *b) {
 }
 
 sx_status launch_colsum(const sx_pool *pool, const sx_batch *b, const void *q_new, const float *lse_new,
-                        int lse_by_token, float *partial, float2 *col_tab, cudaStream_t st) {
+                        int lse_by_token, int lse_splits, float *partial, float2 *col_tab, cudaStream_t st) {
   const int g = pool->num_q_heads / pool->num_kv_heads;
   const int rpt = kTile / g;
   CUtensorMap tm_q, tm_k;
@@ -304,6 +315,8 @@ sx_status launch_colsum(const sx_pool *pool, const sx_batch *b, const void *q_ne
   p.k_table = b->k_block_table;
   p.lse = lse_new;
   p.lse_by_token = lse_by_token;
+  p.lse_splits = lse_splits;
+  p.lse_stride = (size_t)b->total_new * pool->num_q_heads;
   p.partial = partial;
   p.col_tab = col_tab;
   p.num_reqs = b->num_reqs;

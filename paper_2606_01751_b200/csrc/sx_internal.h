@@ -17,7 +17,7 @@ constexpr double kLog2e = 1.4426950408889634;
 // Workspace carve-up (all offsets 256-B aligned). Computed from host mirrors only.
 struct WsLayout {
   size_t rope_table;   // float2 [num_segments][64]       (cos, sin)(delta_m * theta_i)
-  size_t lse_new;      // float  [total_new][Hq]          sweep-1 normaliser (natural log)
+  size_t lse_new;      // float  [8][total_new][Hq]       sweep-1 normaliser (natural log) per key split
   size_t partial;      // float  [Hkv][total_tokens]      per-kv-head column sums of A_sq
   size_t scores;       // float  [total_tokens]           head-summed scores when the caller passes none
   size_t col_tab;      // float2 [query tiles][Hkv][128]  (log2-domain lse, position) of every sweep-2 column
@@ -38,14 +38,16 @@ sx_status launch_select(const sx_pool *pool, const sx_batch *b, const float *par
                         cudaStream_t st);
 // tcgen05 kernels. q_rows: bf16 [total_rows][Hq][128]; rows == nullptr => row n is position n - off[req].
 sx_status launch_attn(const sx_pool *pool, const sx_batch *b, bool with_pv, const void *q, const int32_t *rows,
-                      const int32_t *rows_off, int32_t total_rows, void *out, float *lse, cudaStream_t st);
+                      const int32_t *rows_off, int32_t total_rows, void *out, float *lse, int kv_splits,
+                      cudaStream_t st);
+int attn_lse_splits(const sx_pool *pool, const sx_batch *b, int32_t total_rows);
 // CUDA-core split-KV attention for fewer than 64 (row, head) pairs per KV head; part = ws.small_part
 sx_status launch_attn_small(const sx_pool *pool, const sx_batch *b, const void *q, const int32_t *rows,
                             const int32_t *rows_off, int32_t total_rows, void *out, float *lse, float *part,
                             cudaStream_t st);
 size_t small_ws_bytes(int num_reqs, int num_kv_heads, int group);
 sx_status launch_colsum(const sx_pool *pool, const sx_batch *b, const void *q_new, const float *lse_new,
-                        int lse_by_token, float *partial, float2 *col_tab, cudaStream_t st);
+                        int lse_by_token, int lse_splits, float *partial, float2 *col_tab, cudaStream_t st);
 size_t colsum_tab_bytes(const sx_pool *pool, const sx_batch *b);
 
 // TMA descriptor construction (driver entry point fetched through the runtime; no libcuda link)

@@ -26,7 +26,8 @@ def main():
         lay = wl.CONFIGS[name]()
         lt = wl.build_layer(lay, 0)
         log = []
-        hist = carve_margins(lay, lt, log=log)
+        # C4: rows shared by several requests whose cuts fall in the same segment need more, wider rounds
+        hist = carve_margins(lay, lt, log=log, max_iter=40, widen_later=3.0 if name == "C4" else 1.5)
         with open(os.path.join(HERE, "carve_%s.txt" % name), "w") as f:
             f.write("# margin carve of workloads.CONFIGS[%r](), layer 0, tau = 1e-3; band sizes per iteration %r\n"
                     % (name, hist))

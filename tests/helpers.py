@@ -49,7 +49,8 @@ def oracle_scores_after_realign(lay: wl.LayerTensors, lt: wl.LayerTensors):
     return out
 
 
-def carve_margins(lay: wl.Layout, lt: wl.LayerTensors, tau: float = 1e-3, max_iter: int = 12, log=None):
+def carve_margins(lay: wl.Layout, lt: wl.LayerTensors, tau: float = 1e-3, max_iter: int = 12, log=None,
+                  widen_later: float = 1.5):
     """Reading A9/A10: the x4 salient tokens alone do not make the rank-k cut unambiguous
     (ratio > salient fraction, the cut falls among ordinary tokens). Enforce a relative margin at the
     cut: every cached token whose fp64 score lies within tau of the midpoint c between ranks k and k+1
@@ -63,7 +64,7 @@ def carve_margins(lay: wl.Layout, lt: wl.LayerTensors, tau: float = 1e-3, max_it
     for it in range(max_iter):
         # every rescaled key also moves the softmax normalisers, hence the cut itself, by a few 1e-4
         # relative: clear a wider band (3 tau first, 1.5 tau later) than the one that must end up empty
-        widen = 3.0 if it == 0 else 1.5
+        widen = 3.0 if it == 0 else widen_later
         sc = oracle_scores_after_realign(lay, lt)
         band_total = 0
         touched = set()     # a source row shared by two requests is moved once per iteration (else a row that
