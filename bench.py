@@ -193,7 +193,8 @@ def measure(cfg, steps, warmup, ctx, want_e2e=True, want_clocks=True):
     sel_holder = {}
 
     def full_layer(gl, select_after):
-        timed("realign", lambda: sx.rope_realign(gl.pool, batch))
+        if not stack:
+            timed("realign", lambda: sx.rope_realign(gl.pool, batch))
         timed("scatter", lambda: sx.scatter_kv(gl.pool, batch, gl.k_fresh, gl.v_fresh, all_rows, batch.tok_off,
                                                max_rows=T))
         timed("attn_full", lambda: sx.sparse_attn(gl.pool, batch, gl.q_full, gl.out, total_rows=T, lse=gl.lse,
@@ -204,7 +205,8 @@ def measure(cfg, steps, warmup, ctx, want_e2e=True, want_clocks=True):
                                                     lse_by_token=True))
 
     def sparse_layer(gl, own_select):
-        timed("realign", lambda: sx.rope_realign(gl.pool, batch))
+        if not stack:
+            timed("realign", lambda: sx.rope_realign(gl.pool, batch))
         n_rows = int(sel_holder["rows"].numel())
         if own_select:
             timed("scatter", lambda: sx.scatter_kv(gl.pool, batch, gl.kf_new, gl.vf_new, batch.new_idx, batch.new_off,
@@ -225,7 +227,9 @@ def measure(cfg, steps, warmup, ctx, want_e2e=True, want_clocks=True):
     n_sel, n_rows_total = int(g0.sel_off_h[-1]), int(g0.rows_off_h[-1])
     sel_holder["sel"] = torch.zeros(max(n_sel, 1), dtype=torch.int32, device=dev)[:n_sel]
     sel_holder["rows"] = torch.zeros(n_rows_total, dtype=torch.int32, device=dev)
+    pools = [gl.pool for gl in layers]
     if stack:
+        sx.rope_realign_layers(pools, batch)
         for l in range(THRESHOLD):
             full_layer(layers[l], select_after=(l == THRESHOLD - 1))
     else:
@@ -245,6 +249,8 @@ def measure(cfg, steps, warmup, ctx, want_e2e=True, want_clocks=True):
 
     def step():
         if stack:
+            # stage (a) for the whole stack in one launch: it reads cached source pages only
+            timed("realign", lambda: sx.rope_realign_layers(pools, batch))
             for l, gl in enumerate(layers):
                 if gl.is_full:
                     full_layer(gl, select_after=(l == THRESHOLD - 1))
@@ -428,9 +434,12 @@ def run_e2e(torch, sx, du, lay, layers, batch, all_rows, sel_holder, stack, args
                 for n, h in host[l].items():
                     getattr(gl, n).copy_(h, non_blocking=True)
                 ev_in[l].record(s_in)
+        if stack:
+            sx.rope_realign_layers([gl.pool for gl in layers], batch)
         for l, gl in enumerate(layers):
             main.wait_event(ev_in[l])
-            sx.rope_realign(gl.pool, batch)
+            if not stack:
+                sx.rope_realign(gl.pool, batch)
             if gl.is_full:
                 sx.scatter_kv(gl.pool, batch, gl.k_fresh, gl.v_fresh, all_rows, batch.tok_off, max_rows=T)
                 sx.sparse_attn(gl.pool, batch, gl.q_full, gl.out, total_rows=T, lse=gl.lse, full=True)

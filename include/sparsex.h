@@ -112,6 +112,14 @@ sx_status sx_workspace_size(const sx_pool *pool, const sx_batch *batch, size_t *
 sx_status sx_rope_realign(const sx_pool *pool, const sx_batch *batch, void *ws, size_t ws_bytes,
                           sx_stream stream);
 
+/* (a) for a stack of layers in ONE launch: pools[0..num_layers) are the per-layer pools (host array; same
+ * num_blocks / num_kv_heads), all addressed through the same batch descriptor (block tables and segment map
+ * are per request, not per layer). The re-alignment reads only cached source pages, never an output of the
+ * current step, so it can be completed for every layer of the scheduling batch before the first layer runs
+ * ("completes RoPE alignment for all requests in a scheduling batch", 331). */
+sx_status sx_rope_realign_layers(const sx_pool *pools, int32_t num_layers, const sx_batch *batch, void *ws,
+                                 size_t ws_bytes, sx_stream stream);
+
 /* (d) Alg. 1 l.509-510 / 544-545; slot mapping PAPER.md:333. Rows of request r are
  * rows[rows_off[r] .. rows_off[r+1]) (absolute positions, strictly ascending within a request);
  * k_fresh / v_fresh are bf16 [n][Hkv][128] in the same order. For each row p:

@@ -68,6 +68,8 @@ def load():
         lib.sx_workspace_size.argtypes = [PP, PB, ctypes.POINTER(sz)]
         lib.sx_rope_realign.restype = ctypes.c_int
         lib.sx_rope_realign.argtypes = [PP, PB, vp, sz, vp]
+        lib.sx_rope_realign_layers.restype = ctypes.c_int
+        lib.sx_rope_realign_layers.argtypes = [PP, i32, PB, vp, sz, vp]
         lib.sx_scatter_kv.restype = ctypes.c_int
         lib.sx_scatter_kv.argtypes = [PP, PB, vp, vp, vp, vp, i32, vp]
         lib.sx_score_select.restype = ctypes.c_int
@@ -167,6 +169,17 @@ def rope_realign(pool: DevicePool, batch: DeviceBatch, stream=None):
     ws = batch.workspace(pool)
     _check(load().sx_rope_realign(ctypes.byref(pool.c), ctypes.byref(batch.c), _ptr(ws), ws.numel(),
                                   _stream(stream)), "sx_rope_realign")
+
+
+def rope_realign_layers(pools, batch: DeviceBatch, stream=None):
+    """Stage (a) for a stack of layers in one launch (same batch descriptor for all layers)."""
+    global LAUNCHES
+    n = len(pools)
+    LAUNCHES += (1 + (n + 63) // 64) if batch.c.num_segments else 0
+    ws = batch.workspace(pools[0])
+    arr = (SxPool * n)(*[p.c for p in pools])
+    _check(load().sx_rope_realign_layers(arr, n, ctypes.byref(batch.c), _ptr(ws), ws.numel(), _stream(stream)),
+           "sx_rope_realign_layers")
 
 
 def scatter_kv(pool: DevicePool, batch: DeviceBatch, k_fresh: torch.Tensor, v_fresh: torch.Tensor,

@@ -31,6 +31,8 @@ WsLayout ws_layout(const sx_pool *pool, const sx_batch *b) {
   size_t off = 0;
   w.rope_table = off;
   off = align_up(off + sizeof(float2) * 64 * (size_t)(b->num_segments > 0 ? b->num_segments : 1), 256);
+  w.page_desc = off;
+  off = align_up(off + sizeof(int4) * (size_t)(b->total_seg_pages > 0 ? b->total_seg_pages : 1), 256);
   w.lse_new = off;
   off = align_up(off + 8 * sizeof(float) * (size_t)(b->total_new > 0 ? b->total_new : 1) * pool->num_q_heads, 256);
   w.partial = off;
@@ -162,15 +164,26 @@ sx_status sx_workspace_size(const sx_pool *pool, const sx_batch *batch, size_t *
   return SX_OK;
 }
 
-sx_status sx_rope_realign(const sx_pool *pool, const sx_batch *batch, void *ws, size_t ws_bytes, sx_stream stream) {
-  sx_status st = validate(pool, batch);
-  if (st != SX_OK) return st;
-  st = validate_ws(pool, batch, ws, ws_bytes);
+sx_status sx_rope_realign_layers(const sx_pool *pools, int32_t num_layers, const sx_batch *batch, void *ws,
+                                 size_t ws_bytes, sx_stream stream) {
+  if (!pools || num_layers <= 0) return set_error(SX_ERR_INVALID_ARG, "pools is NULL or num_layers <= 0");
+  for (int l = 0; l < num_layers; ++l) {
+    sx_status st = validate(&pools[l], batch);
+    if (st != SX_OK) return st;
+    if (pools[l].num_kv_heads != pools[0].num_kv_heads || pools[l].num_blocks != pools[0].num_blocks)
+      return set_error(SX_ERR_INVALID_ARG, "layer %d: pool shape differs from layer 0", l);
+  }
+  sx_status st = validate_ws(&pools[0], batch, ws, ws_bytes);
   if (st != SX_OK) return st;
   if (batch->num_segments == 0 || batch->total_seg_pages == 0) return SX_OK;
-  WsLayout w = ws_layout(pool, batch);
-  return launch_realign(pool, batch, reinterpret_cast<float2 *>(static_cast<char *>(ws) + w.rope_table),
+  WsLayout w = ws_layout(&pools[0], batch);
+  return launch_realign(pools, num_layers, batch, reinterpret_cast<float2 *>(static_cast<char *>(ws) + w.rope_table),
+                        reinterpret_cast<int4 *>(static_cast<char *>(ws) + w.page_desc),
                         reinterpret_cast<cudaStream_t>(stream));
+}
+
+sx_status sx_rope_realign(const sx_pool *pool, const sx_batch *batch, void *ws, size_t ws_bytes, sx_stream stream) {
+  return sx_rope_realign_layers(pool, 1, batch, ws, ws_bytes, stream);
 }
 
 sx_status sx_scatter_kv(const sx_pool *pool, const sx_batch *batch, const void *k_fresh, const void *v_fresh,

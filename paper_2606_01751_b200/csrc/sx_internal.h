@@ -17,6 +17,7 @@ constexpr double kLog2e = 1.4426950408889634;
 // Workspace carve-up (all offsets 256-B aligned). Computed from host mirrors only.
 struct WsLayout {
   size_t rope_table;   // float2 [num_segments][64]       (cos, sin)(delta_m * theta_i)
+  size_t page_desc;    // int4   [total_seg_pages]        (segment, source, destination K, destination V) per page
   size_t lse_new;      // float  [8][total_new][Hq]       sweep-1 normaliser (natural log) per key split
   size_t partial;      // float  [Hkv][total_tokens]      per-kv-head column sums of A_sq
   size_t scores;       // float  [total_tokens]           head-summed scores when the caller passes none
@@ -30,7 +31,8 @@ sx_status set_error(sx_status st, const char *fmt, ...);
 sx_status check_launch(const char *what);
 
 // kernels (one launcher per translation unit)
-sx_status launch_realign(const sx_pool *pool, const sx_batch *b, float2 *table, cudaStream_t st);
+sx_status launch_realign(const sx_pool *pools, int num_layers, const sx_batch *b, float2 *table, int4 *page_desc,
+                         cudaStream_t st);
 sx_status launch_scatter(const sx_pool *pool, const sx_batch *b, const void *k_fresh, const void *v_fresh,
                          const int32_t *rows, const int32_t *rows_off, int32_t max_rows, cudaStream_t st);
 sx_status launch_select(const sx_pool *pool, const sx_batch *b, const float *partial, const int32_t *sel_off,

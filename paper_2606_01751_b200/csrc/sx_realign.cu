@@ -3,8 +3,8 @@
 //
 //   k^_{p'+j} <- R_{p'-p} k^_{p+j},  v^_{p'+j} <- v^_{p+j}
 //
-// HBM-bound: per cached token 8*Hkv*128 bytes (read K,V + write K,V). One CTA per source page
-// (all KV heads, K and V): 16-byte coalesced loads issued up front, rotation in fp32 on
+// HBM-bound: per cached token 8*Hkv*128 bytes (read K,V + write K,V). One CTA per (source page, KV head)
+// = 4 KB of K and of V: 16-byte coalesced loads issued up front, rotation in fp32 on
 // (cos, sin)(Delta_m * theta_i) taken from a per-segment table that a tiny first kernel builds in
 // fp64 (an fp32 product Delta*theta_i loses ~3e-3 in the sine at Delta ~ 1.3e5), one RNE to bf16.
 #include "sx_internal.h"
@@ -12,17 +12,35 @@
 
 namespace sx {
 
-// table[m][i] = (cos, sin)(Delta_m * theta^(-2i/128)), i in [0, 64)
+// One preparatory launch per call: thread idx < num_segments * 64 builds the rotation table
+// table[m][i] = (cos, sin)(Delta_m * theta^(-2i/128)), i in [0, 64), in fp64; thread idx < total pages
+// resolves its page once: (segment, source page, destination K page, destination V page), so that the
+// copy kernel starts streaming after a single 16-byte load instead of a chain of dependent lookups.
 __global__ void rope_table_kernel(const sx_segment *__restrict__ segs, int num_segments, double theta,
-                                  float2 *__restrict__ table) {
+                                  float2 *__restrict__ table, int total_pages,
+                                  const int32_t *__restrict__ src_blocks, const int32_t *__restrict__ k_table,
+                                  const int32_t *__restrict__ v_table, int max_pages, int4 *__restrict__ page_desc) {
   int idx = blockIdx.x * blockDim.x + threadIdx.x;
-  if (idx >= num_segments * 64) return;
-  int m = idx >> 6, i = idx & 63;
-  double delta = (double)(segs[m].new_pos - segs[m].old_pos);
-  double inv_freq = pow(theta, -2.0 * (double)i / (double)kHeadDim);
-  double s, c;
-  sincos(delta * inv_freq, &s, &c);
-  table[idx] = make_float2((float)c, (float)s);
+  if (idx < num_segments * 64) {
+    int m = idx >> 6, i = idx & 63;
+    double delta = (double)(segs[m].new_pos - segs[m].old_pos);
+    double inv_freq = pow(theta, -2.0 * (double)i / (double)kHeadDim);
+    double s, c;
+    sincos(delta * inv_freq, &s, &c);
+    table[idx] = make_float2((float)c, (float)s);
+  }
+  if (idx < total_pages) {
+    // segment m with src_off[m] <= page < src_off[m] + len/16 (src_off ascending: binary search)
+    int lo = 0, hi = num_segments - 1;
+    while (lo < hi) {
+      int mid = (lo + hi + 1) >> 1;
+      if (segs[mid].src_off <= idx) lo = mid; else hi = mid - 1;
+    }
+    const sx_segment sg = segs[lo];
+    const int lpage = sg.new_pos / kPage + (idx - sg.src_off);
+    page_desc[idx] = make_int4(lo, src_blocks[idx], k_table[(size_t)sg.req * max_pages + lpage],
+                               v_table[(size_t)sg.req * max_pages + lpage]);
+  }
 }
 
 __device__ __forceinline__ uint4 ld_stream(const uint4 *p) {
@@ -68,117 +86,107 @@ __device__ __forceinline__ void rotate_inter(uint4 &a, const float2 *cs) {
   }
 }
 
-constexpr int kRealignThreads = 256;
+constexpr int kRealignThreads = 128;
+
+// One CTA per (source page, KV head): 4 KB of K and 4 KB of V in, the same out. Every thread issues its
+// four 16-byte loads (and the rotation coefficients of its column pair) right after the descriptor.
+constexpr int kRealignMaxLayers = 64;
+struct LayerPools {  // K and V pools of the layers of one launch (blockIdx.z = layer), passed by value
+  uint4 *k[kRealignMaxLayers];
+  uint4 *v[kRealignMaxLayers];
+};
 
 template <int STYLE>
 __global__ void __launch_bounds__(kRealignThreads)
-realign_kernel(const uint4 *pool_k_src, uint4 *pool_k_dst, const uint4 *pool_v_src, uint4 *pool_v_dst, int num_kv_heads, const sx_segment *__restrict__ segs, int num_segments,
-               const int32_t *__restrict__ src_blocks, const int32_t *__restrict__ k_table,
-               const int32_t *__restrict__ v_table, int max_pages, const float2 *__restrict__ table) {
-  __shared__ float2 cs_sm[64];
-  __shared__ int sh[4];
-  const int page = blockIdx.x;  // index into src_blocks
-  if (threadIdx.x == 0) {
-    // segment m with src_off[m] <= page < src_off[m] + len/16 (src_off ascending: binary search)
-    int lo = 0, hi = num_segments - 1;
-    while (lo < hi) {
-      int mid = (lo + hi + 1) >> 1;
-      if (segs[mid].src_off <= page) lo = mid; else hi = mid - 1;
-    }
-    const sx_segment s = segs[lo];
-    int pg = page - s.src_off;
-    int lpage = s.new_pos / kPage + pg;
-    sh[0] = lo;
-    sh[1] = src_blocks[page];
-    sh[2] = k_table[(size_t)s.req * max_pages + lpage];
-    sh[3] = v_table[(size_t)s.req * max_pages + lpage];
-  }
-  __syncthreads();
-  const int m = sh[0], src = sh[1], dk = sh[2], dv = sh[3];
-  if (threadIdx.x < 64) cs_sm[threadIdx.x] = table[m * 64 + threadIdx.x];
-  __syncthreads();
-
-  const int chunks = num_kv_heads * kPage * 16;            // 16-byte chunks of one page (all heads)
-  const size_t page_chunks = (size_t)chunks;
-  const uint4 *ks = pool_k_src + (size_t)src * page_chunks;
-  uint4 *kd = pool_k_dst + (size_t)dk * page_chunks;
-  const uint4 *vs = pool_v_src + (size_t)src * page_chunks;
-  uint4 *vd = pool_v_dst + (size_t)dv * page_chunks;
-  const bool copy_v = (dv != src);
-
+realign_kernel(const __grid_constant__ LayerPools pools, int num_kv_heads, const int4 *__restrict__ page_desc,
+               const float2 *__restrict__ table) {
+  const int page = blockIdx.x, h = blockIdx.y;
+  const uint4 *pool_k_src = pools.k[blockIdx.z], *pool_v_src = pools.v[blockIdx.z];
+  uint4 *pool_k_dst = pools.k[blockIdx.z], *pool_v_dst = pools.v[blockIdx.z];
+  const int4 d = __ldg(page_desc + page);  // (segment, source page, destination K page, destination V page)
+  const size_t tile = (size_t)kPage * 16;  // 16-byte chunks of one (page, head) tile
+  const uint4 *ks = pool_k_src + ((size_t)d.y * num_kv_heads + h) * tile;
+  uint4 *kd = pool_k_dst + ((size_t)d.z * num_kv_heads + h) * tile;
+  const uint4 *vs = pool_v_src + ((size_t)d.y * num_kv_heads + h) * tile;
+  uint4 *vd = pool_v_dst + ((size_t)d.w * num_kv_heads + h) * tile;
+  const bool copy_v = (d.w != d.y);
+  const int t = threadIdx.x;
   if (STYLE == 0) {
-    // task = (row, c): chunks c and c+8 of one 256-B row
-    const int tasks = chunks / 2;
-    for (int t0 = threadIdx.x; t0 < tasks; t0 += 4 * kRealignThreads) {
-      uint4 a[4], b[4], v0[4], v1[4];
+    // chunks c and c + 8 of row t >> 3: columns [8c, 8c+8) pair with [64+8c, 64+8c+8)
+    const int row = t >> 3, c = t & 7;
+    uint4 a = ld_stream(ks + row * 16 + c);
+    uint4 b = ld_stream(ks + row * 16 + c + 8);
+    uint4 v0, v1;
+    if (copy_v) {
+      v0 = ld_stream(vs + row * 16 + c);
+      v1 = ld_stream(vs + row * 16 + c + 8);
+    }
+    float2 cs[8];
+    const float4 *tp = reinterpret_cast<const float4 *>(table + d.x * 64 + c * 8);
 #pragma unroll
-      for (int u = 0; u < 4; ++u) {
-        int t = t0 + u * kRealignThreads;
-        if (t < tasks) {
-          int row = t >> 3, c = t & 7;
-          a[u] = ld_stream(ks + row * 16 + c);
-          b[u] = ld_stream(ks + row * 16 + c + 8);
-          if (copy_v) {
-            v0[u] = ld_stream(vs + row * 16 + c);
-            v1[u] = ld_stream(vs + row * 16 + c + 8);
-          }
-        }
-      }
-#pragma unroll
-      for (int u = 0; u < 4; ++u) {
-        int t = t0 + u * kRealignThreads;
-        if (t < tasks) {
-          int row = t >> 3, c = t & 7;
-          rotate_split(a[u], b[u], cs_sm + c * 8);
-          st_stream(kd + row * 16 + c, a[u]);
-          st_stream(kd + row * 16 + c + 8, b[u]);
-          if (copy_v) {
-            st_stream(vd + row * 16 + c, v0[u]);
-            st_stream(vd + row * 16 + c + 8, v1[u]);
-          }
-        }
-      }
+    for (int i = 0; i < 4; ++i) {
+      const float4 f = __ldg(tp + i);
+      cs[2 * i] = make_float2(f.x, f.y);
+      cs[2 * i + 1] = make_float2(f.z, f.w);
+    }
+    rotate_split(a, b, cs);
+    st_stream(kd + row * 16 + c, a);
+    st_stream(kd + row * 16 + c + 8, b);
+    if (copy_v) {
+      st_stream(vd + row * 16 + c, v0);
+      st_stream(vd + row * 16 + c + 8, v1);
     }
   } else {
-    for (int t0 = threadIdx.x; t0 < chunks; t0 += 4 * kRealignThreads) {
-      uint4 a[4], v0[4];
+    // chunks t and t + 128: the 4 interleaved pairs (2i, 2i+1) of each 16-byte chunk
+    uint4 a0 = ld_stream(ks + t), a1 = ld_stream(ks + t + 128);
+    uint4 v0, v1;
+    if (copy_v) {
+      v0 = ld_stream(vs + t);
+      v1 = ld_stream(vs + t + 128);
+    }
+    float2 cs[4];
+    const float4 *tp = reinterpret_cast<const float4 *>(table + d.x * 64 + (t & 15) * 4);
 #pragma unroll
-      for (int u = 0; u < 4; ++u) {
-        int t = t0 + u * kRealignThreads;
-        if (t < chunks) {
-          a[u] = ld_stream(ks + t);
-          if (copy_v) v0[u] = ld_stream(vs + t);
-        }
-      }
-#pragma unroll
-      for (int u = 0; u < 4; ++u) {
-        int t = t0 + u * kRealignThreads;
-        if (t < chunks) {
-          rotate_inter(a[u], cs_sm + (t & 15) * 4);
-          st_stream(kd + t, a[u]);
-          if (copy_v) st_stream(vd + t, v0[u]);
-        }
-      }
+    for (int i = 0; i < 2; ++i) {
+      const float4 f = __ldg(tp + i);
+      cs[2 * i] = make_float2(f.x, f.y);
+      cs[2 * i + 1] = make_float2(f.z, f.w);
+    }
+    rotate_inter(a0, cs);
+    rotate_inter(a1, cs);  // (t + 128) & 15 == t & 15: same column group
+    st_stream(kd + t, a0);
+    st_stream(kd + t + 128, a1);
+    if (copy_v) {
+      st_stream(vd + t, v0);
+      st_stream(vd + t + 128, v1);
     }
   }
 }
 
-sx_status launch_realign(const sx_pool *pool, const sx_batch *b, float2 *table, cudaStream_t st) {
-  int n = b->num_segments * 64;
-  rope_table_kernel<<<(n + 127) / 128, 128, 0, st>>>(b->segments, b->num_segments, b->rope_theta, table);
+sx_status launch_realign(const sx_pool *pools, int num_layers, const sx_batch *b, float2 *table, int4 *page_desc,
+                         cudaStream_t st) {
+  const int n = b->num_segments * 64 > b->total_seg_pages ? b->num_segments * 64 : b->total_seg_pages;
+  rope_table_kernel<<<(n + 127) / 128, 128, 0, st>>>(b->segments, b->num_segments, b->rope_theta, table,
+                                                    b->total_seg_pages, b->src_blocks, b->k_block_table,
+                                                    b->v_block_table, b->max_pages_per_req, page_desc);
   sx_status s = check_launch("rope_table_kernel");
   if (s != SX_OK) return s;
-  const uint4 *k = reinterpret_cast<const uint4 *>(pool->k);
-  const uint4 *v = reinterpret_cast<const uint4 *>(pool->v);
-  if (b->rope_style == 0)
-    realign_kernel<0><<<b->total_seg_pages, kRealignThreads, 0, st>>>(
-        k, reinterpret_cast<uint4 *>(pool->k), v, reinterpret_cast<uint4 *>(pool->v), pool->num_kv_heads, b->segments,
-        b->num_segments, b->src_blocks, b->k_block_table, b->v_block_table, b->max_pages_per_req, table);
-  else
-    realign_kernel<1><<<b->total_seg_pages, kRealignThreads, 0, st>>>(
-        k, reinterpret_cast<uint4 *>(pool->k), v, reinterpret_cast<uint4 *>(pool->v), pool->num_kv_heads, b->segments,
-        b->num_segments, b->src_blocks, b->k_block_table, b->v_block_table, b->max_pages_per_req, table);
-  return check_launch("realign_kernel");
+  for (int l0 = 0; l0 < num_layers; l0 += kRealignMaxLayers) {
+    const int nl = num_layers - l0 < kRealignMaxLayers ? num_layers - l0 : kRealignMaxLayers;
+    LayerPools lp;
+    for (int l = 0; l < nl; ++l) {
+      lp.k[l] = reinterpret_cast<uint4 *>(pools[l0 + l].k);
+      lp.v[l] = reinterpret_cast<uint4 *>(pools[l0 + l].v);
+    }
+    const dim3 grid(b->total_seg_pages, pools[0].num_kv_heads, nl);
+    if (b->rope_style == 0)
+      realign_kernel<0><<<grid, kRealignThreads, 0, st>>>(lp, pools[0].num_kv_heads, page_desc, table);
+    else
+      realign_kernel<1><<<grid, kRealignThreads, 0, st>>>(lp, pools[0].num_kv_heads, page_desc, table);
+    s = check_launch("realign_kernel");
+    if (s != SX_OK) return s;
+  }
+  return SX_OK;
 }
 
 }  // namespace sx

@@ -308,3 +308,24 @@ def test_small_row_sets_cuda_core_path(case):
                                      want_lse=True)
         check_close("%s req %d O" % (case, r), out[off[r]:off[r + 1]], ref_o)
         assert np.max(np.abs(lse[off[r]:off[r + 1]] - ref_l)) < 2e-3
+
+
+def test_realign_all_layers_in_one_launch():
+    """sx_rope_realign_layers (alignment of the whole scheduling batch at once) must give,
+    layer by layer, exactly the bits of the per-layer call."""
+    GpuLayer, dev_to_bits = _gpu()
+    from paper_2606_01751_b200 import binding as sx
+    lay = wl.config_c3(scale=0.125)
+    lts = [wl.build_layer(lay, l) for l in range(3)]
+    single = []
+    for lt in lts:
+        g = GpuLayer(lay, lt)
+        g.realign()
+        torch.cuda.synchronize()
+        single.append((dev_to_bits(g.pool_k).copy(), dev_to_bits(g.pool_v).copy()))
+    gs = [GpuLayer(lay, lt) for lt in lts]
+    sx.rope_realign_layers([g.pool for g in gs], gs[0].batch)
+    torch.cuda.synchronize()
+    for g, (k, v) in zip(gs, single):
+        assert np.array_equal(dev_to_bits(g.pool_k), k)
+        assert np.array_equal(dev_to_bits(g.pool_v), v)
