@@ -152,12 +152,32 @@ sx_status sx_score_select(const sx_pool *pool, const sx_batch *batch, const void
                           float *scores, int32_t *sel_idx, int32_t *rows_R, void *ws,
                           size_t ws_bytes, sx_stream stream);
 
+/* (b) with the two additions that complete the paper's recompute set (Alg. 1 l.535-539):
+ *   R = I_nr U S_key U S_ov U S_tail
+ *   S_ov   (overflow): every maximal contiguous interval of I_nr is expanded by
+ *          overflow_blocks pages (the paper uses 1) on both sides, clipped to the request;
+ *   S_tail (tail fallback): if the last position of the request is a reused token, the last
+ *          tail_tokens (the paper uses 64) positions of the reused segment that holds it.
+ * S_key is still the top-k of ALL cached positions (it may overlap S_ov / S_tail), so |R| depends on the data:
+ *   rows_off      device [num_reqs+1]: CAPACITY offsets; slot r must hold |I_nr(r)| + k_r + |S_ov U S_tail|
+ *                 positions (host-computable from the layout; rows beyond the capacity would be dropped);
+ *   rows_R        device int32 [rows_off[num_reqs]]: R of all requests, packed back to back;
+ *   rows_off_out  device [num_reqs+1]: the actual CSR offsets into rows_R. Pass (rows_R, rows_off_out) to
+ *                 sx_scatter_kv / sx_sparse_attn with max_rows / total_rows = rows_off[num_reqs] (upper bound).
+ * With overflow_blocks = tail_tokens = 0 this is sx_score_select (rows_off_out may then be NULL). */
+sx_status sx_score_select_ex(const sx_pool *pool, const sx_batch *batch, const void *q_new,
+                             const float *lse_new, int32_t lse_by_token, const int32_t *sel_off,
+                             const int32_t *rows_off, int32_t overflow_blocks, int32_t tail_tokens,
+                             float *scores, int32_t *sel_idx, int32_t *rows_R, int32_t *rows_off_out, void *ws,
+                             size_t ws_bytes, sx_stream stream);
+
 /* (c) Alg. 1 l.546-548 (sparse) / l.507-511 (full). mode 0: query rows are rows_R (as produced by
  * sx_score_select); mode 1: rows_R and rows_off are ignored, every position of every request is
  * a query row (R = {0..T-1}, row n of the batch = token tok_off[r]+j).
  *   q    device bf16 [total_rows][Hq][128], compact in rows order; out same shape (bf16);
  *   lse  device fp32 [total_rows][Hq] natural-log normaliser, or NULL.
- *   total_rows (host) = rows_off[num_reqs] (mode 0) or total_tokens (mode 1).
+ *   total_rows (host) >= rows_off[num_reqs] (mode 0; equal unless the row list came from sx_score_select_ex,
+ *   then its capacity) or = total_tokens (mode 1); q / out / lse are sized by total_rows.
  * O[n][h] = sum_{j <= pos(n)} softmax_j(<q, k_j>/sqrt(128)) v_j with kv head h / g, K and V read
  * through the block tables. Two paths, chosen from host-visible sizes only:
  *   - total_rows * g >= 64 * num_reqs (at least 64 query rows per KV head on average; g = Hq/Hkv):

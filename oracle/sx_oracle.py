@@ -224,6 +224,35 @@ def select_topk(s: np.ndarray, is_new: np.ndarray, k: int) -> Tuple[np.ndarray, 
     return sel, rows
 
 
+def recompute_set(is_new: np.ndarray, sel: np.ndarray, seg_ranges, overflow_blocks: int = 1,
+                  tail_tokens: int = 64, block: int = 16) -> np.ndarray:
+    """Alg. 1 l.535-539, one request: R = I_nr U S_key U S_ov U S_tail, sorted.
+    S_ov: every maximal contiguous interval [a, b] of I_nr expanded by `overflow_blocks` blocks of `block`
+    positions on both sides (clipped to the request). S_tail: if the last position is a reused token, the
+    last `tail_tokens` positions of the reused segment that contains it. seg_ranges: [(start, end)) of the
+    reused segments of this request in current positions."""
+    is_new = np.asarray(is_new, dtype=bool)
+    t = len(is_new)
+    r = set(int(i) for i in np.nonzero(is_new)[0]) | set(int(i) for i in sel)
+    a = None
+    for i in range(t + 1):                       # walk the maximal intervals of I_nr
+        inside = i < t and is_new[i]
+        if inside and a is None:
+            a = i
+        if not inside and a is not None:
+            b = i - 1
+            r.update(range(max(0, a - overflow_blocks * block), a))
+            r.update(range(b + 1, min(t, b + 1 + overflow_blocks * block)))
+            a = None
+    if tail_tokens > 0 and not is_new[t - 1]:
+        start = 0
+        for (s0, s1) in seg_ranges:
+            if s0 <= t - 1 < s1:
+                start = s0
+        r.update(range(max(start, t - tail_tokens), t))
+    return np.asarray(sorted(r), dtype=np.int32)
+
+
 # ----------------------------------------------------------------------------- O-c attention
 
 def attention(pool_k: np.ndarray, pool_v: np.ndarray, k_table_row: np.ndarray, v_table_row: np.ndarray,

@@ -24,8 +24,8 @@ _lib = None
 
 SX_OK = 0
 LAUNCHES = 0   # kernels launched through this binding (each stage call adds its known kernel count)
-EXPORTS = ["sx_workspace_size", "sx_rope_realign", "sx_scatter_kv", "sx_score_select", "sx_sparse_attn",
-           "sx_last_error", "sx_version"]
+EXPORTS = ["sx_workspace_size", "sx_rope_realign", "sx_rope_realign_layers", "sx_scatter_kv", "sx_score_select",
+           "sx_score_select_ex", "sx_sparse_attn", "sx_last_error", "sx_version"]
 
 
 class SxPool(ctypes.Structure):
@@ -74,6 +74,8 @@ def load():
         lib.sx_scatter_kv.argtypes = [PP, PB, vp, vp, vp, vp, i32, vp]
         lib.sx_score_select.restype = ctypes.c_int
         lib.sx_score_select.argtypes = [PP, PB, vp, vp, i32, vp, vp, vp, vp, vp, vp, sz, vp]
+        lib.sx_score_select_ex.restype = ctypes.c_int
+        lib.sx_score_select_ex.argtypes = [PP, PB, vp, vp, i32, vp, vp, i32, i32, vp, vp, vp, vp, vp, sz, vp]
         lib.sx_sparse_attn.restype = ctypes.c_int
         lib.sx_sparse_attn.argtypes = [PP, PB, i32, vp, vp, vp, i32, vp, vp, vp, sz, vp]
         lib.sx_last_error.restype = ctypes.c_char_p
@@ -204,6 +206,36 @@ def score_select(pool: DevicePool, batch: DeviceBatch, q_new: torch.Tensor, sel_
     _check(load().sx_score_select(ctypes.byref(pool.c), ctypes.byref(batch.c), _ptr(q_new), _ptr(lse_new),
                                   1 if lse_by_token else 0, _ptr(sel_off), _ptr(rows_off), _ptr(scores), _ptr(sel_idx), _ptr(rows_R),
                                   _ptr(ws), ws.numel(), _stream(stream)), "sx_score_select")
+
+
+def score_select_ex(pool: DevicePool, batch: DeviceBatch, q_new: torch.Tensor, sel_off: torch.Tensor,
+                    rows_cap_off: torch.Tensor, sel_idx: torch.Tensor, rows_R: torch.Tensor,
+                    rows_off_out: torch.Tensor, overflow_blocks: int = 1, tail_tokens: int = 64,
+                    scores: Optional[torch.Tensor] = None, lse_new: Optional[torch.Tensor] = None,
+                    lse_by_token: bool = False, stream=None):
+    """Stage (b) with overflow and tail fallback (Alg. 1 l.535-539): R = I_nr U S_key U S_ov U S_tail; the
+    actual CSR offsets of the packed rows_R come back in rows_off_out (device)."""
+    global LAUNCHES
+    LAUNCHES += 2 + ((3 if lse_new is None else 2) if batch.c.total_new else 0)
+    ws = batch.workspace(pool)
+    _check(load().sx_score_select_ex(ctypes.byref(pool.c), ctypes.byref(batch.c), _ptr(q_new), _ptr(lse_new),
+                                     1 if lse_by_token else 0, _ptr(sel_off), _ptr(rows_cap_off),
+                                     int(overflow_blocks), int(tail_tokens), _ptr(scores), _ptr(sel_idx),
+                                     _ptr(rows_R), _ptr(rows_off_out), _ptr(ws), ws.numel(), _stream(stream)),
+           "sx_score_select_ex")
+
+
+def rows_capacity(lay, overflow_blocks: int, tail_tokens: int) -> np.ndarray:
+    """Host CSR capacity offsets for sx_score_select_ex: |I_nr| + k + 2 * 16 * overflow_blocks per interval of
+    I_nr + tail_tokens per request, clipped to the request length (a sizing bound, not the set itself)."""
+    sel_off, _ = selection_offsets(lay)
+    cap = [0]
+    for r in range(lay.num_reqs):
+        idx = np.asarray(lay.new_idx[lay.new_off[r]:lay.new_off[r + 1]])
+        n_int = (1 + int(np.sum(np.diff(idx) != 1))) if len(idx) else 0
+        c = len(idx) + int(sel_off[r + 1] - sel_off[r]) + 2 * 16 * overflow_blocks * n_int + tail_tokens
+        cap.append(cap[-1] + min(c, int(lay.seq_len[r])))
+    return np.asarray(cap, dtype=np.int32)
 
 
 def sparse_attn(pool: DevicePool, batch: DeviceBatch, q: torch.Tensor, out: torch.Tensor,

@@ -41,6 +41,10 @@ WsLayout ws_layout(const sx_pool *pool, const sx_batch *b) {
   off = align_up(off + sizeof(float) * (size_t)b->total_tokens, 256);
   w.col_tab = off;
   off = align_up(off + colsum_tab_bytes(pool, b), 256);
+  w.rows_tmp = off;
+  off = align_up(off + sizeof(int32_t) * (size_t)b->total_tokens, 256);
+  w.rows_cnt = off;
+  off = align_up(off + sizeof(int32_t) * (size_t)b->num_reqs, 256);
   w.small_part = off;
   off = align_up(off + small_ws_bytes(b->num_reqs, pool->num_kv_heads, pool->num_q_heads / pool->num_kv_heads), 256);
   w.total = off;
@@ -197,14 +201,19 @@ sx_status sx_scatter_kv(const sx_pool *pool, const sx_batch *batch, const void *
   return launch_scatter(pool, batch, k_fresh, v_fresh, rows, rows_off, max_rows, reinterpret_cast<cudaStream_t>(stream));
 }
 
-sx_status sx_score_select(const sx_pool *pool, const sx_batch *batch, const void *q_new, const float *lse_new,
-                          int32_t lse_by_token, const int32_t *sel_off, const int32_t *rows_off, float *scores, int32_t *sel_idx,
-                          int32_t *rows_R, void *ws, size_t ws_bytes, sx_stream stream) {
+sx_status sx_score_select_ex(const sx_pool *pool, const sx_batch *batch, const void *q_new, const float *lse_new,
+                             int32_t lse_by_token, const int32_t *sel_off, const int32_t *rows_off,
+                             int32_t overflow_blocks, int32_t tail_tokens, float *scores, int32_t *sel_idx,
+                             int32_t *rows_R, int32_t *rows_off_out, void *ws, size_t ws_bytes, sx_stream stream) {
   sx_status st = validate(pool, batch);
   if (st != SX_OK) return st;
   st = validate_ws(pool, batch, ws, ws_bytes);
   if (st != SX_OK) return st;
   if (!sel_off || !rows_off || !sel_idx || !rows_R) return set_error(SX_ERR_INVALID_ARG, "score_select: NULL array");
+  if (overflow_blocks < 0 || tail_tokens < 0)
+    return set_error(SX_ERR_INVALID_ARG, "overflow_blocks / tail_tokens must be >= 0");
+  if ((overflow_blocks > 0 || tail_tokens > 0) && !rows_off_out)
+    return set_error(SX_ERR_INVALID_ARG, "rows_off_out is required with overflow / tail fallback (|R| is data dependent)");
   if (batch->total_new > 0 && !q_new) return set_error(SX_ERR_INVALID_ARG, "q_new is NULL");
   if (q_new && misaligned(q_new)) return set_error(SX_ERR_MISALIGNED, "q_new not 16-B aligned");
   cudaStream_t s = reinterpret_cast<cudaStream_t>(stream);
@@ -233,7 +242,16 @@ sx_status sx_score_select(const sx_pool *pool, const sx_batch *batch, const void
     if (e != cudaSuccess) return set_error(SX_ERR_CUDA, "memset: %s", cudaGetErrorString(e));
   }
   float *sc = scores ? scores : reinterpret_cast<float *>(base + w.scores);
-  return launch_select(pool, batch, partial, sel_off, rows_off, sc, sel_idx, rows_R, s);
+  return launch_select(pool, batch, partial, sel_off, rows_off, sc, sel_idx, rows_R, overflow_blocks, tail_tokens,
+                       reinterpret_cast<int32_t *>(base + w.rows_tmp), reinterpret_cast<int32_t *>(base + w.rows_cnt),
+                       rows_off_out, s);
+}
+
+sx_status sx_score_select(const sx_pool *pool, const sx_batch *batch, const void *q_new, const float *lse_new,
+                          int32_t lse_by_token, const int32_t *sel_off, const int32_t *rows_off, float *scores, int32_t *sel_idx,
+                          int32_t *rows_R, void *ws, size_t ws_bytes, sx_stream stream) {
+  return sx_score_select_ex(pool, batch, q_new, lse_new, lse_by_token, sel_off, rows_off, 0, 0, scores, sel_idx, rows_R,
+                            nullptr, ws, ws_bytes, stream);
 }
 
 sx_status sx_sparse_attn(const sx_pool *pool, const sx_batch *batch, int32_t mode, const void *q,

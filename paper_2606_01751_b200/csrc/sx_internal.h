@@ -22,6 +22,8 @@ struct WsLayout {
   size_t partial;      // float  [Hkv][total_tokens]      per-kv-head column sums of A_sq
   size_t scores;       // float  [total_tokens]           head-summed scores when the caller passes none
   size_t col_tab;      // float2 [query tiles][Hkv][128]  (log2-domain lse, position) of every sweep-2 column
+  size_t rows_tmp;     // int32  [total_tokens]           capacity-slotted R of the extended selection
+  size_t rows_cnt;     // int32  [num_reqs]
   size_t small_part;   // float  split-KV partials of the CUDA-core attention path (sx_attn_small.cu)
   size_t total;
 };
@@ -36,7 +38,8 @@ sx_status launch_realign(const sx_pool *pools, int num_layers, const sx_batch *b
 sx_status launch_scatter(const sx_pool *pool, const sx_batch *b, const void *k_fresh, const void *v_fresh,
                          const int32_t *rows, const int32_t *rows_off, int32_t max_rows, cudaStream_t st);
 sx_status launch_select(const sx_pool *pool, const sx_batch *b, const float *partial, const int32_t *sel_off,
-                        const int32_t *rows_off, float *scores, int32_t *sel_idx, int32_t *rows_R,
+                        const int32_t *rows_off, float *scores, int32_t *sel_idx, int32_t *rows_R, int ov_blocks,
+                        int tail_tokens, int32_t *rows_tmp, int32_t *rows_cnt, int32_t *rows_off_out,
                         cudaStream_t st);
 // tcgen05 kernels. q_rows: bf16 [total_rows][Hq][128]; rows == nullptr => row n is position n - off[req].
 sx_status launch_attn(const sx_pool *pool, const sx_batch *b, bool with_pv, const void *q, const int32_t *rows,

@@ -54,8 +54,9 @@ select_kernel(int num_kv_heads, int total_tokens, const int32_t *__restrict__ se
               const int32_t *__restrict__ tok_off, const int32_t *__restrict__ new_off,
               const int32_t *__restrict__ new_idx, const float *__restrict__ partial,
               const int32_t *__restrict__ sel_off, const int32_t *__restrict__ rows_off, float *__restrict__ scores,
-              int32_t *__restrict__ sel_idx, int32_t *__restrict__ rows_R) {
-  extern __shared__ uint32_t is_new[];  // bitmap over positions
+              int32_t *__restrict__ sel_idx, int32_t *__restrict__ rows_R, int ov_tokens, int tail_tokens,
+              const sx_segment *__restrict__ segs, int num_segments, int32_t *__restrict__ rows_cnt) {
+  extern __shared__ uint32_t is_new[];  // bitmap over positions; a second bitmap (forced rows) follows it
   __shared__ int hist[256];
   __shared__ int warp_tot[3][kSelWarps];
   __shared__ int tot[3];
@@ -72,11 +73,36 @@ select_kernel(int num_kv_heads, int total_tokens, const int32_t *__restrict__ se
   if (k > n_cached) k = n_cached;
   if (k < 0) k = 0;
 
-  for (int i = threadIdx.x; i < words; i += kSelThreads) is_new[i] = 0u;
+  uint32_t *forced = is_new + words;  // S_ov U S_tail (Alg. 1 l.535-536), cached positions only
+  for (int i = threadIdx.x; i < 2 * words; i += kSelThreads) is_new[i] = 0u;
   __syncthreads();
   for (int i = threadIdx.x; i < nn; i += kSelThreads) {
     int p = new_idx[n0 + i];
     atomicOr(&is_new[p >> 5], 1u << (p & 31));
+  }
+  if (ov_tokens > 0 || tail_tokens > 0) {
+    __syncthreads();
+    // overflow (Alg. 1 l.535): every maximal interval [a, b] of I_nr grows by one block
+    // on both sides; only positions that are not new themselves are recorded
+    for (int i = threadIdx.x; i < nn; i += kSelThreads) {
+      const int p = new_idx[n0 + i];
+      if (i == 0 || new_idx[n0 + i - 1] != p - 1)
+        for (int q = max(0, p - ov_tokens); q < p; ++q)
+          if (!((is_new[q >> 5] >> (q & 31)) & 1u)) atomicOr(&forced[q >> 5], 1u << (q & 31));
+      if (i == nn - 1 || new_idx[n0 + i + 1] != p + 1)
+        for (int q = p + 1; q <= min(T - 1, p + ov_tokens); ++q)
+          if (!((is_new[q >> 5] >> (q & 31)) & 1u)) atomicOr(&forced[q >> 5], 1u << (q & 31));
+    }
+    // tail fallback (Alg. 1 l.536): the prompt ends inside a reused segment -> its last
+    // tail_tokens positions are recomputed
+    if (tail_tokens > 0 && !((is_new[(T - 1) >> 5] >> ((T - 1) & 31)) & 1u)) {
+      int seg_start = 0;  // start of the reused segment that contains position T - 1
+      for (int m = 0; m < num_segments; ++m)
+        if (segs[m].req == req && segs[m].new_pos <= T - 1 && T - 1 < segs[m].new_pos + segs[m].len)
+          seg_start = segs[m].new_pos;
+      for (int q = max(seg_start, T - tail_tokens) + threadIdx.x; q < T; q += kSelThreads)
+        atomicOr(&forced[q >> 5], 1u << (q & 31));
+    }
   }
   // head aggregation in fixed order kvh = 0..Hkv-1 (global score across heads)
   for (int j = threadIdx.x; j < T; j += kSelThreads) {
@@ -145,9 +171,10 @@ select_kernel(int num_kv_heads, int total_tokens, const int32_t *__restrict__ se
   const int so = sel_off[req], ro = rows_off[req];
   for (int j0 = 0; j0 < T; j0 += kSelThreads) {
     const int j = j0 + threadIdx.x;
-    bool isn = false, gt = false, eq = false;
+    bool isn = false, gt = false, eq = false, frc = false;
     if (j < T) {
       isn = (is_new[j >> 5] >> (j & 31)) & 1u;
+      frc = (forced[j >> 5] >> (j & 31)) & 1u;
       if (!isn && k > 0) {
         uint32_t u = __float_as_uint(scores[off + j]);
         gt = u > thr;
@@ -159,29 +186,53 @@ select_kernel(int num_kv_heads, int total_tokens, const int32_t *__restrict__ se
     const int tot_eq = tot[0];
     const bool sel = gt || (eq && (base_eq + s1.a) < take_eq);
     __syncthreads();
-    Scan3 s2 = block_scan3(sel, sel || isn, false, warp_tot, tot);
+    const bool in_r = sel || isn || frc;  // R = I_nr U S_key U S_ov U S_tail (Alg. 1 l.537-539)
+    Scan3 s2 = block_scan3(sel, in_r, false, warp_tot, tot);
     if (sel) sel_idx[so + base_sel + s2.a] = j;
-    if (sel || isn) rows_R[ro + base_r + s2.b] = j;
+    if (in_r && base_r + s2.b < rows_off[req + 1] - ro) rows_R[ro + base_r + s2.b] = j;
     const int tsel = tot[0], tr = tot[1];
     __syncthreads();
     base_eq += tot_eq;
     base_sel += tsel;
     base_r += tr;
   }
+  if (rows_cnt && threadIdx.x == 0) rows_cnt[req] = min(base_r, rows_off[req + 1] - ro);
+}
+
+// Extended selection only: per-request row lists sit in capacity-sized slots of `tmp`; pack them into one
+// CSR (rows_R, rows_off_out) so that the scatter and attention stages take them unchanged.
+__global__ void __launch_bounds__(kSelThreads)
+compact_rows_kernel(int num_reqs, const int32_t *__restrict__ cap_off, const int32_t *__restrict__ cnt,
+                    const int32_t *__restrict__ tmp, int32_t *__restrict__ rows_R, int32_t *__restrict__ rows_off_out) {
+  int out = 0;
+  for (int r = 0; r < num_reqs; ++r) {
+    const int n = cnt[r], src = cap_off[r];
+    for (int i = threadIdx.x; i < n; i += kSelThreads) rows_R[out + i] = tmp[src + i];
+    if (threadIdx.x == 0) rows_off_out[r] = out;
+    out += n;
+  }
+  if (threadIdx.x == 0) rows_off_out[num_reqs] = out;
 }
 
 sx_status launch_select(const sx_pool *pool, const sx_batch *b, const float *partial, const int32_t *sel_off,
-                        const int32_t *rows_off, float *scores, int32_t *sel_idx, int32_t *rows_R, cudaStream_t st) {
-  size_t smem = sizeof(uint32_t) * (size_t)((b->max_seq_len + 31) / 32);
-  if (smem > 200 * 1024) return set_error(SX_ERR_UNSUPPORTED, "max_seq_len %d too large for the select bitmap", b->max_seq_len);
+                        const int32_t *rows_off, float *scores, int32_t *sel_idx, int32_t *rows_R, int ov_blocks,
+                        int tail_tokens, int32_t *rows_tmp, int32_t *rows_cnt, int32_t *rows_off_out,
+                        cudaStream_t st) {
+  size_t smem = 2 * sizeof(uint32_t) * (size_t)((b->max_seq_len + 31) / 32);
+  if (smem > 200 * 1024) return set_error(SX_ERR_UNSUPPORTED, "max_seq_len %d too large for the select bitmaps", b->max_seq_len);
   if (smem > 40 * 1024) {
     cudaError_t e = cudaFuncSetAttribute(select_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (e != cudaSuccess) return set_error(SX_ERR_CUDA, "select smem attr: %s", cudaGetErrorString(e));
   }
-  select_kernel<<<b->num_reqs, kSelThreads, smem, st>>>(pool->num_kv_heads, b->total_tokens, b->seq_len, b->tok_off,
-                                                       b->new_off, b->new_idx, partial, sel_off, rows_off, scores,
-                                                       sel_idx, rows_R);
-  return check_launch("select_kernel");
+  const bool ex = rows_off_out != nullptr;  // extended: variable |R|, slots of capacity rows_off, then compaction
+  select_kernel<<<b->num_reqs, kSelThreads, smem, st>>>(
+      pool->num_kv_heads, b->total_tokens, b->seq_len, b->tok_off, b->new_off, b->new_idx, partial, sel_off, rows_off,
+      scores, sel_idx, ex ? rows_tmp : rows_R, ov_blocks * kPage, tail_tokens, b->segments, b->num_segments,
+      ex ? rows_cnt : nullptr);
+  sx_status s = check_launch("select_kernel");
+  if (s != SX_OK || !ex) return s;
+  compact_rows_kernel<<<1, kSelThreads, 0, st>>>(b->num_reqs, rows_off, rows_cnt, rows_tmp, rows_R, rows_off_out);
+  return check_launch("compact_rows_kernel");
 }
 
 }  // namespace sx

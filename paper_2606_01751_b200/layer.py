@@ -84,6 +84,25 @@ class GpuLayer:
         self.sel_idx = self.sel_idx[:n_sel]
         self.rows_R = self.rows_R[:n_rows]
 
+    def select_ex(self, overflow_blocks: int = 1, tail_tokens: int = 64, want_scores: bool = True):
+        """Selection with overflow and tail fallback (Alg. 1 l.535-539): |R| is data dependent, so the row
+        offsets are read back before the per-row inputs are staged."""
+        cap = sx.rows_capacity(self.lay, overflow_blocks, tail_tokens)
+        n_sel = int(self.sel_off_h[-1])
+        self.sel_idx = torch.full((max(n_sel, 1),), -1, dtype=torch.int32, device=self.dev)
+        rows = torch.full((max(int(cap[-1]), 1),), -1, dtype=torch.int32, device=self.dev)
+        self.rows_cap = int(cap[-1])
+        off_out = torch.zeros(self.lay.num_reqs + 1, dtype=torch.int32, device=self.dev)
+        self.scores = (torch.empty(int(self.lay.tok_off[-1]), dtype=torch.float32, device=self.dev)
+                       if want_scores else None)
+        sx.score_select_ex(self.pool, self.batch, self.q_new, self.sel_off, torch.from_numpy(cap).to(self.dev),
+                           self.sel_idx, rows, off_out, overflow_blocks=overflow_blocks, tail_tokens=tail_tokens,
+                           scores=self.scores)
+        self.sel_idx = self.sel_idx[:n_sel]
+        self.rows_off = off_out
+        self.rows_off_h = off_out.cpu().numpy()
+        self.rows_R = rows[:int(self.rows_off_h[-1])]
+
     def stage_rows(self, sel_idx: torch.Tensor, rows_R: torch.Tensor):
         """Input staging for (d) and (c): compact fresh K,V of S_key and Q of R (Alg. 1 l.544)."""
         self.sel_idx, self.rows_R = sel_idx, rows_R

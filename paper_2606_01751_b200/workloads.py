@@ -383,6 +383,20 @@ def config_c5(scale: float = 1.0, ratio: float = 0.05) -> Layout:
 CONFIGS = {"C1": config_c1, "C2": config_c2, "C3": config_c3, "C4": config_c4, "C5": config_c5}
 
 
+def config_tail(seed_id: int = 15) -> Layout:
+    """Requests that END inside a reused segment (tail fallback) and whose new-token intervals
+    touch reused segments on both sides (overflow): request 0 ends with a 96-token segment
+    (tail = its last 64 tokens), request 1 with a 32-token one (tail = all of it), request 2 ends with new
+    tokens (no tail) and starts with new tokens (no block before the first interval)."""
+    pool = [PoolSegment(32, 64), PoolSegment(48, 0), PoolSegment(16, 160), PoolSegment(96, 32)]
+    reqs = [[("new", 16), ("seg", 0), ("new", 16), ("seg", 1), ("seg", 3)],
+            [("seg", 2), ("new", 32), ("seg", 0)],
+            [("new", 32), ("seg", 1), ("new", 16), ("seg", 2), ("new", 16)]]
+    # budgets below the number of cached tokens that some new query can see (the tokens behind the last new
+    # token score exactly 0 and would turn the cut into a pure position tie)
+    return build_layout("tail", seed_id, 4, 2, 10000.0, pool, reqs, [0.2, 0.25, 0.3], 0.1, k_override=[8, 4, 19])
+
+
 def config_tiny(seed_id: int = 9, num_q_heads: int = 4, num_kv_heads: int = 2, tail: int = 0,
                 rope_style: int = 0, cow: bool = False) -> Layout:
     """Two small requests with uneven segments, negative and zero deltas; optional ragged tail (T % 16 != 0)."""

@@ -329,3 +329,49 @@ def test_realign_all_layers_in_one_launch():
     for g, (k, v) in zip(gs, single):
         assert np.array_equal(dev_to_bits(g.pool_k), k)
         assert np.array_equal(dev_to_bits(g.pool_v), v)
+
+
+@pytest.mark.parametrize("ov,tail", [(1, 64), (1, 0), (0, 64), (2, 16)])
+def test_overflow_and_tail_fallback(ov, tail):
+    """sx_score_select_ex: R = I_nr U S_key U S_ov U S_tail (Alg. 1 l.535-539) bit-exact against the oracle,
+    then scatter + attention on that (data-dependent) row list."""
+    GpuLayer, dev_to_bits = _gpu()
+    lay = wl.config_tail()
+    lt = wl.build_layer(lay, 0)
+    carve_margins(lay, lt)
+    g = GpuLayer(lay, lt)
+    g.realign()
+    g.scatter_new()
+    g.select_ex(overflow_blocks=ov, tail_tokens=tail)
+    g.stage_rows(g.sel_idx, g.rows_R)
+    sx_rows_total = int(g.rows_off_h[-1])
+    from paper_2606_01751_b200 import binding as sx
+    sx.scatter_kv(g.pool, g.batch, g.kf_R, g.vf_R, g.rows_R, g.rows_off, max_rows=g.rows_cap)
+    g.attend()
+    torch.cuda.synchronize()
+    # oracle
+    pk, pv = lt.pool_k.copy(), lt.pool_v.copy()
+    kt, vt = lay.k_block_table.copy(), lay.v_block_table.copy()
+    orc.realign(pk, pv, kt, vt, lay.segments, lay.src_blocks, lay.rope_theta, lay.rope_style)
+    sel_g, rows_g = g.sel_idx.cpu().numpy(), g.rows_R.cpu().numpy()
+    out = orc.bf16_to_f64(dev_to_bits(g.out))
+    total = 0
+    for r in range(lay.num_reqs):
+        t, o = int(lay.seq_len[r]), int(lay.tok_off[r])
+        nidx = lay.new_idx[lay.new_off[r]:lay.new_off[r + 1]]
+        orc.scatter_kv(pk, pv, kt, vt, None, r, nidx, lt.k_fresh[o + nidx], lt.v_fresh[o + nidx])
+        s = orc.scores(pk, kt[r], t, lt.q_full[o + nidx], nidx, lay.num_q_heads)
+        is_new = lay.is_new_mask(r)
+        sel, _ = orc.select_topk(s, is_new, int(lay.k_per_req[r]))
+        segr = [(int(n), int(n + ln)) for (rq, ln, _, n, _) in lay.segments.tolist() if rq == r]
+        rows = orc.recompute_set(is_new, sel, segr, ov, tail)
+        r0, r1 = int(g.rows_off_h[r]), int(g.rows_off_h[r + 1])
+        assert np.array_equal(sel_g[g.sel_off_h[r]:g.sel_off_h[r + 1]], sel), (r, ov, tail)
+        assert np.array_equal(rows_g[r0:r1], rows), (r, ov, tail)
+        orc.scatter_kv(pk, pv, kt, vt, None, r, rows, lt.k_fresh[o + rows], lt.v_fresh[o + rows])
+        ref = orc.attention(pk, pv, kt[r], vt[r], t, lt.q_full[o + rows], rows, lay.num_q_heads)
+        check_close("overflow/tail req %d O" % r, out[r0:r1], ref)
+        total += len(rows)
+    assert total == sx_rows_total
+    # tokens behind the last new token have score exactly 0 and are reached only through S_tail / S_key
+    assert np.array_equal(dev_to_bits(g.pool_v), pv)

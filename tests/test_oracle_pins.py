@@ -353,3 +353,38 @@ def test_layer_sparse_structure():
         a = orc.gather_tokens(pk, kt[r], t)[keep]
         b = orc.gather_tokens(pk0, lay.k_block_table[r], t)[keep]
         assert np.array_equal(a, b)
+
+
+# ----------------------------------------------------------------------------- overflow / tail fallback
+
+def test_recompute_set_hand_cases():
+    """Alg. 1 l.535-539 on hand-written cases (block 16): expected lists typed from the definitions of
+    PAPER.md:235 (tail: last 64 tokens of the final reused segment) and PAPER.md:241 (one block on each
+    side of every Sparse-Q interval)."""
+    # T = 96: cached [0,32), new [32,48), cached segment [48,96) which also ends the prompt
+    is_new = np.zeros(96, dtype=bool)
+    is_new[32:48] = True
+    rows = orc.recompute_set(is_new, np.asarray([3]), [(0, 32), (48, 96)], overflow_blocks=1, tail_tokens=64)
+    # S_ov = [16,32) U [48,64); S_tail = last 64 of segment [48,96) -> only 48 long -> [48,96); S_key = {3}
+    assert rows.tolist() == [3] + list(range(16, 96))
+    # tail segment longer than 64: only its last 64 positions
+    is_new = np.zeros(160, dtype=bool)
+    is_new[0:16] = True
+    rows = orc.recompute_set(is_new, np.asarray([], dtype=np.int32), [(16, 160)], overflow_blocks=1, tail_tokens=64)
+    assert rows.tolist() == list(range(0, 32)) + list(range(96, 160))     # new + one block after + tail
+    # prompt ends with new tokens: no tail; interval at position 0 has no block before it
+    is_new = np.zeros(96, dtype=bool)
+    is_new[0:16] = True
+    is_new[80:96] = True
+    rows = orc.recompute_set(is_new, np.asarray([40, 41]), [(16, 80)], overflow_blocks=1, tail_tokens=64)
+    assert rows.tolist() == list(range(0, 32)) + [40, 41] + list(range(64, 96))
+    # two intervals 16 apart share the block between them; overflow 0 and tail 0 reduce to R = I_nr U S_key
+    is_new = np.zeros(80, dtype=bool)
+    is_new[16:32] = True
+    is_new[48:64] = True
+    rows = orc.recompute_set(is_new, np.asarray([70]), [(0, 16), (32, 48), (64, 80)], 1, 0)
+    assert rows.tolist() == list(range(0, 80))
+    rows = orc.recompute_set(is_new, np.asarray([70]), [(0, 16), (32, 48), (64, 80)], 0, 0)
+    assert rows.tolist() == list(range(16, 32)) + list(range(48, 64)) + [70]
+    _, plain = orc.select_topk(np.arange(80, dtype=np.float64), is_new, 0)
+    assert np.array_equal(orc.recompute_set(is_new, np.asarray([], dtype=np.int32), [], 0, 0), plain)
