@@ -339,6 +339,44 @@ def measure(cfg, steps, warmup, ctx, want_e2e=True, want_clocks=True):
     return res
 
 
+def measure_s6(ctx, reps=10):
+    """Supplementary HBM-regime cases: stage (c) alone with fewer than 64 (row, head) pairs per
+    KV head, i.e. the CUDA-core split-KV path; K and V of the whole 32K context are streamed once.
+    Achieved GB/s = 4*T*Hkv*128 B / time, L2 flushed between repetitions."""
+    torch, sx, dev, peaks = ctx["torch"], ctx["sx"], ctx["dev"], ctx["peaks"]
+    from paper_2606_01751_b200.layer import GpuLayer
+    lay = wl.CONFIGS["C3"]()
+    gl = GpuLayer(lay, DevLayer(lay, 4, dev, torch), dev)
+    T, hq, hkv = lay.total_tokens, lay.num_q_heads, lay.num_kv_heads
+    sx.rope_realign(gl.pool, gl.batch)
+    all_rows = torch.arange(T, dtype=torch.int32, device=dev)
+    sx.scatter_kv(gl.pool, gl.batch, gl.k_fresh, gl.v_fresh, all_rows, gl.batch.tok_off, max_rows=T)
+    flush = torch.empty(512 << 20, dtype=torch.uint8, device=dev)
+    out = {}
+    for n in (1, 2, 8):
+        rows = torch.arange(T - n, T, dtype=torch.int32, device=dev)
+        off = torch.tensor([0, n], dtype=torch.int32, device=dev)
+        q = gl.q_full[T - n:T].contiguous()
+        o = torch.empty((n, hq, 128), dtype=torch.int16, device=dev)
+        ms = []
+        for i in range(reps + 3):
+            flush.zero_()
+            a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            a.record()
+            sx.sparse_attn(gl.pool, gl.batch, q, o, rows_R=rows, rows_off=off, total_rows=n)
+            b.record()
+            torch.cuda.synchronize()
+            if i >= 3:
+                ms.append(a.elapsed_time(b))
+        t = float(np.median(ms))
+        gbs = 4.0 * T * hkv * 128 / (t * 1e-3) / 1e9
+        out["last%d_rows_%d_pairs_per_kv_head" % (n, n * hq // hkv)] = {
+            "ms": round(t, 4), "hbm_gbs": round(gbs, 1), "hbm_frac": round(gbs / peaks["hbm_gbs"], 4)}
+    del gl, flush
+    torch.cuda.empty_cache()
+    return out
+
+
 def run_ours(args):
     import torch
     from paper_2606_01751_b200 import binding as sx
@@ -369,6 +407,7 @@ def run_ours(args):
                          "stage_ms": {k: round(v, 4) for k, v in o["stage_ms"].items()},
                          "attn_tflops": o["roofline"]["achieved"], "attn_frac": o["roofline"]["frac"],
                          "attn_peak": o["roofline"]["peak_src"], "hbm_stage": o["hbm"]}
+        others["S6"] = measure_s6(ctx)
     if rank != 0:
         return
     stack, n_layers, T = m["stack"], m["n_layers"], m["T"]
