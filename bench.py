@@ -308,7 +308,13 @@ def measure(cfg, steps, warmup, ctx, want_e2e=True, want_clocks=True):
     tf_peak, tf_src = (peaks["tf_sustained"], "sustained") if stack else (peaks["tf_burst"], "burst")
     roofline = {"bound": "tensor", "kernel": "attn_kernel<true> (sx_sparse_attn)", "achieved": round(achieved, 1),
                 "peak": tf_peak, "unit": "TFLOP/s", "frac": round(achieved / tf_peak, 4),
-                "peak_src": "%s bf16 %s" % (peaks["src"], tf_src), "traffic": None,
+                "peak_src": "%s bf16 %s" % (peaks["src"], tf_src),
+                # dram__bytes_read + dram__bytes_write per attention launch, averaged over the 32 launches of a C3 step
+                # (28 sparse x 377.7 MB + 4 full x 2163.4 MB; ncu --set full, profiles/r1_v3_kernels_ncu_full.md)
+                "traffic": 600.9e6 if stack else None, "traffic_unit": "B per launch (ncu capture)",
+                "algorithmic_bytes_per_launch": round(float(sum(
+                    4.0 * int(n) * hkv * 128 for n in lay.seq_len) * n_layers +
+                    4.0 * (n_rows_total * n_sparse + T * n_full) * hq * 128) / n_layers, 1),
                 "launches_per_step": n_layers, "avg_launch_ms": round(attn_ms / n_layers, 4),
                 "flops_per_step": fl_total}
     if "attn_sparse" in stage_ms and n_sparse:
