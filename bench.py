@@ -406,7 +406,7 @@ def run_ours(args):
         for c in wl.CONFIGS:
             if c == cfg or c not in ("C1", "C2", "C3", "C4", "C5"):
                 continue
-            o = measure(c, 5 if c != "C3" else 2, 3, ctx, want_e2e=False, want_clocks=False)
+            o = measure(c, 30 if c != "C3" else 2, 5, ctx, want_e2e=False, want_clocks=False)
             others[c] = {"context_tokens": o["T"], "rows_R": o["rows_R"], "layers": o["n_layers"],
                          "ms_per_layer": round(o["ms_per_step"] / o["n_layers"], 4),
                          "context_tokens_per_s": round(o["value"], 1),
