@@ -351,34 +351,39 @@ def measure_s6(ctx, reps=10):
     Achieved GB/s = 4*T*Hkv*128 B / time, L2 flushed between repetitions."""
     torch, sx, dev, peaks = ctx["torch"], ctx["sx"], ctx["dev"], ctx["peaks"]
     from paper_2606_01751_b200.layer import GpuLayer
-    lay = wl.CONFIGS["C3"]()
-    gl = GpuLayer(lay, DevLayer(lay, 4, dev, torch), dev)
-    T, hq, hkv = lay.total_tokens, lay.num_q_heads, lay.num_kv_heads
-    sx.rope_realign(gl.pool, gl.batch)
-    all_rows = torch.arange(T, dtype=torch.int32, device=dev)
-    sx.scatter_kv(gl.pool, gl.batch, gl.k_fresh, gl.v_fresh, all_rows, gl.batch.tok_off, max_rows=T)
     flush = torch.empty(512 << 20, dtype=torch.uint8, device=dev)
     out = {}
-    for n in (1, 2, 8):
-        rows = torch.arange(T - n, T, dtype=torch.int32, device=dev)
-        off = torch.tensor([0, n], dtype=torch.int32, device=dev)
-        q = gl.q_full[T - n:T].contiguous()
-        o = torch.empty((n, hq, 128), dtype=torch.int16, device=dev)
-        ms = []
-        for i in range(reps + 3):
-            flush.zero_()
-            a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-            a.record()
-            sx.sparse_attn(gl.pool, gl.batch, q, o, rows_R=rows, rows_off=off, total_rows=n)
-            b.record()
-            torch.cuda.synchronize()
-            if i >= 3:
-                ms.append(a.elapsed_time(b))
-        t = float(np.median(ms))
-        gbs = 4.0 * T * hkv * 128 / (t * 1e-3) / 1e9
-        out["last%d_rows_%d_pairs_per_kv_head" % (n, n * hq // hkv)] = {
-            "ms": round(t, 4), "hbm_gbs": round(gbs, 1), "hbm_frac": round(gbs / peaks["hbm_gbs"], 4)}
-    del gl, flush
+    # (i) C3 pool, last 1 / 2 / 8 positions: 4 / 8 / 32 pairs per KV head -> CUDA-core paths
+    # (ii) C5 pool, last 16 positions: 112 pairs per KV head -> tcgen05 tiles with key splits
+    for cfg, layer, lasts in (("C3", 4, (1, 2, 8)), ("C5", 0, (16,))):
+        lay = wl.CONFIGS[cfg]()
+        gl = GpuLayer(lay, DevLayer(lay, layer, dev, torch), dev)
+        T, hq, hkv = lay.total_tokens, lay.num_q_heads, lay.num_kv_heads
+        sx.rope_realign(gl.pool, gl.batch)
+        all_rows = torch.arange(T, dtype=torch.int32, device=dev)
+        sx.scatter_kv(gl.pool, gl.batch, gl.k_fresh, gl.v_fresh, all_rows, gl.batch.tok_off, max_rows=T)
+        for n in lasts:
+            rows = torch.arange(T - n, T, dtype=torch.int32, device=dev)
+            off = torch.tensor([0, n], dtype=torch.int32, device=dev)
+            q = gl.q_full[T - n:T].contiguous()
+            o = torch.empty((n, hq, 128), dtype=torch.int16, device=dev)
+            ms = []
+            for i in range(reps + 3):
+                flush.zero_()
+                a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+                a.record()
+                sx.sparse_attn(gl.pool, gl.batch, q, o, rows_R=rows, rows_off=off, total_rows=n)
+                b.record()
+                torch.cuda.synchronize()
+                if i >= 3:
+                    ms.append(a.elapsed_time(b))
+            t = float(np.median(ms))
+            gbs = 4.0 * T * hkv * 128 / (t * 1e-3) / 1e9
+            out["%s_last%d_rows_%d_pairs_per_kv_head" % (cfg, n, n * hq // hkv)] = {
+                "ms": round(t, 4), "hbm_gbs": round(gbs, 1), "hbm_frac": round(gbs / peaks["hbm_gbs"], 4)}
+        del gl
+        torch.cuda.empty_cache()
+    del flush
     torch.cuda.empty_cache()
     return out
 

@@ -248,6 +248,9 @@ def sparse_attn(pool: DevicePool, batch: DeviceBatch, q: torch.Tensor, out: torc
     n = int(q.shape[0]) if total_rows is None else int(total_rows)
     g = pool.c.num_q_heads // pool.c.num_kv_heads
     small = g <= 32 and n * g < 64 * batch.c.num_reqs       # CUDA-core path: split kernel + merge kernel
+    if not small and n:          # few CTAs against a long context: key splits + merge kernel (attn_pv_splits)
+        grid = (n // (2 * (128 // g)) + batch.c.num_reqs) * pool.c.num_kv_heads
+        small = grid < 148 and min(148 // grid, ((batch.c.max_seq_len + 127) // 128) // 2) > 1
     LAUNCHES += (2 if small else 1) if n else 0
     assert q.is_contiguous() and out.is_contiguous()
     _check(load().sx_sparse_attn(ctypes.byref(pool.c), ctypes.byref(batch.c), 1 if full else 0, _ptr(q),

@@ -45,6 +45,8 @@ WsLayout ws_layout(const sx_pool *pool, const sx_batch *b) {
   off = align_up(off + sizeof(int32_t) * (size_t)b->total_tokens, 256);
   w.rows_cnt = off;
   off = align_up(off + sizeof(int32_t) * (size_t)b->num_reqs, 256);
+  w.attn_part = off;
+  off = align_up(off + attn_part_bytes(), 256);
   w.small_part = off;
   off = align_up(off + small_ws_bytes(b->num_reqs, pool->num_kv_heads, pool->num_q_heads / pool->num_kv_heads), 256);
   w.total = off;
@@ -228,7 +230,7 @@ sx_status sx_score_select_ex(const sx_pool *pool, const sx_batch *batch, const v
       float *lse_ws = reinterpret_cast<float *>(base + w.lse_new);
       lse_splits = attn_lse_splits(pool, batch, batch->total_new);
       st = launch_attn(pool, batch, /*with_pv=*/false, q_new, batch->new_idx, batch->new_off, batch->total_new,
-                       nullptr, lse_ws, lse_splits, s);
+                       nullptr, lse_ws, lse_splits, nullptr, s);
       if (st != SX_OK) return st;
       lse = lse_ws;
       lse_by_token = 0;
@@ -283,7 +285,14 @@ sx_status sx_sparse_attn(const sx_pool *pool, const sx_batch *batch, int32_t mod
     return launch_attn_small(pool, batch, q, rows_R, rows_off, total_rows, out, lse,
                              reinterpret_cast<float *>(static_cast<char *>(ws) + w.small_part), s);
   }
-  return launch_attn(pool, batch, true, q, rows_R, rows_off, total_rows, out, lse, 1, s);
+  const int splits = attn_pv_splits(pool, batch, total_rows);
+  float *part = nullptr;
+  if (splits > 1) {
+    st = validate_ws(pool, batch, ws, ws_bytes);
+    if (st != SX_OK) return st;
+    part = reinterpret_cast<float *>(static_cast<char *>(ws) + ws_layout(pool, batch).attn_part);
+  }
+  return launch_attn(pool, batch, true, q, rows_R, rows_off, total_rows, out, lse, splits, part, s);
 }
 
 }  // extern "C"

@@ -48,7 +48,9 @@ struct AttnParams {
   float *lse;          // [total_rows][Hq] or nullptr
   int num_reqs, max_pages, num_q_heads, num_kv_heads, group, rows_per_tile;
   int total_rows;
-  int kv_splits;     // LSE-only variant: the key range of a CTA is cut into this many contiguous parts
+  int kv_splits;     // the key range of a CTA is cut into this many contiguous parts (consecutive blocks)
+  float *part_o;     // PV variant with kv_splits > 1: [split][total_rows][Hq][128] normalised partial O (fp32)
+  float *part_lse;   //                                 [split][total_rows][Hq]      partial log-sum-exp
   float scale_log2;  // log2(e) / sqrt(128)
   float scale;       // 1 / sqrt(128)
 };
@@ -99,9 +101,9 @@ attn_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_constant__ CU
 
   // ---- which (request, KV head, pair of row tiles) is this CTA; heavy (late) pairs of a request first
   const int g = p.group, rpt = p.rows_per_tile, rpc = 2 * rpt;
-  // LSE-only variant: consecutive blocks share a (request, KV head, row pair) and take one key split each
-  const int split = kWithPV ? 0 : (int)blockIdx.x % p.kv_splits;
-  const int bid = kWithPV ? (int)blockIdx.x : (int)blockIdx.x / p.kv_splits;
+  // consecutive blocks share a (request, KV head, row pair) and take one key split each
+  const int split = (int)blockIdx.x % p.kv_splits;
+  const int bid = (int)blockIdx.x / p.kv_splits;
   int req = 0, base = 0, pairs = 0, n_r = 0;
   for (; req < p.num_reqs; ++req) {
     n_r = p.rows_off[req + 1] - p.rows_off[req];
@@ -133,7 +135,7 @@ attn_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_constant__ CU
   }
   // key tiles [t0, t0 + n_tiles) of this CTA; n_t[i] and every loop below count tiles from t0
   int t0 = 0;
-  if (!kWithPV && p.kv_splits > 1) {
+  if (p.kv_splits > 1) {
     const int all = max(n_t[0], n_t[1]);
     const int per = (all + p.kv_splits - 1) / p.kv_splits;
     t0 = split * per;
@@ -205,7 +207,7 @@ attn_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_constant__ CU
       const int pg_in_tile = lane >> 1, half = lane & 1;
       const int n_items = kWithPV ? 2 * n_tiles : n_tiles;
       auto table_entry = [&](int it) -> int {
-        const int t = kWithPV ? (it >> 1) : t0 + it;
+        const int t = t0 + (kWithPV ? (it >> 1) : it);
         const bool is_v = kWithPV && (it & 1);
         int lp = t * 8 + pg_in_tile;
         if (lp > n_pages - 1) lp = n_pages - 1;  // pages past the sequence: any valid page (keys are masked)
@@ -254,11 +256,13 @@ attn_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_constant__ CU
         if (kWithPV) {
           // ring item 2t+1 = V(t), 2t+2 = K(t+1): (slot, phase) advanced incrementally
           int sv = 1, sk = 2, phv = 0, phk = 0;
-          mbar_wait(&bars->kv_full[0], 0);
-          tc_fence_after();
-          issue_qk(0, 0, 0);
-          if (n_t[1] > 0) issue_qk(1, 0, 0);
-          umma_commit(&bars->kv_empty[0]);
+          if (n_tiles > 0) {  // (a key split may hold no tile of this CTA's rows)
+            mbar_wait(&bars->kv_full[0], 0);
+            tc_fence_after();
+            if (n_t[0] > 0) issue_qk(0, 0, 0);
+            if (n_t[1] > 0) issue_qk(1, 0, 0);
+            umma_commit(&bars->kv_empty[0]);
+          }
           for (int t = 0; t < n_tiles; ++t) {
             const bool more = t + 1 < n_tiles;
             mbar_wait(&bars->kv_full[sv], phv);            // V(t)
@@ -383,11 +387,11 @@ attn_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_constant__ CU
       const float2 sc2 = make_float2(p.scale_log2, p.scale_log2), nm2 = make_float2(neg_m, neg_m);
       float2 rsum2 = make_float2(0.f, 0.f);
 
-      if (kWithPV && (t + 1) * kTile > T) {
+      if (kWithPV && (t0 + t + 1) * kTile > T) {
         // V rows of keys beyond the sequence may hold anything (even NaN patterns): zero them
         const int it = 2 * t + 1;
         mbar_wait(&bars->kv_full[it % kKvStages], (it / kKvStages) & 1);
-        if (t * kTile + row >= T) {
+        if ((t0 + t) * kTile + row >= T) {
           const uint4 z = make_uint4(0, 0, 0, 0);
           uint8_t *v0 = smem + Cfg::kOffKV + (it % kKvStages) * kTileBytes + row * 128;
 #pragma unroll
@@ -433,8 +437,31 @@ attn_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_constant__ CU
     }
 
     // ---- epilogue
-    if (my_tiles > 0 || !kWithPV) {  // (a key split that holds no tile of the row still reports lse = -inf)
-      const size_t out_row = (size_t)grow * p.num_q_heads + kvh * g + hh;
+    const size_t out_row = (size_t)grow * p.num_q_heads + kvh * g + hh;
+    if (kWithPV && p.kv_splits > 1) {
+      // key split: normalised partial O in fp32 and its log-sum-exp go to the workspace (attn_merge_kernel)
+      const size_t prow = (size_t)split * p.total_rows * p.num_q_heads + out_row;
+      float4 *dst = reinterpret_cast<float4 *>(p.part_o + prow * kHeadDim);
+      if (my_tiles > 0) {
+        mbar_wait(&bars->o_full[qt], 0);
+        tc_fence_after();
+        const float inv = 1.f / l;
+#pragma unroll
+        for (int c = 0; c < 4; ++c) {
+          uint32_t o[32];
+          tmem_ld32(tmem_o + c * 32, o);
+          tmem_wait_ld();
+          if (valid) {
+#pragma unroll
+            for (int v4 = 0; v4 < 8; ++v4)
+              dst[c * 8 + v4] = make_float4(__uint_as_float(o[v4 * 4 + 0]) * inv, __uint_as_float(o[v4 * 4 + 1]) * inv,
+                                            __uint_as_float(o[v4 * 4 + 2]) * inv, __uint_as_float(o[v4 * 4 + 3]) * inv);
+          }
+        }
+      }
+      // a split that holds no visible key of the row reports -inf: the merge skips its (undefined) O
+      if (valid) p.part_lse[prow] = (my_tiles > 0 && m_used > -INFINITY) ? m_used * p.scale + logf(l) : -INFINITY;
+    } else if (my_tiles > 0 || !kWithPV) {  // (an LSE key split that holds no tile of the row still reports -inf)
       if (kWithPV) {
         mbar_wait(&bars->o_full[qt], 0);
         tc_fence_after();
@@ -468,6 +495,69 @@ attn_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_constant__ CU
   if (warp == kWarpMma) tmem_dealloc(tmem, 512);
 }
 
+// Combine the key splits of attn_kernel<true>: out = sum_s exp(lse_s - lse) O_s, in the fixed order 0..splits-1.
+__global__ void __launch_bounds__(256)
+attn_merge_kernel(const float *__restrict__ part_o, const float *__restrict__ part_lse, int splits, int total_rows,
+                  int num_q_heads, const int32_t *__restrict__ rows_off, int num_reqs, __nv_bfloat16 *__restrict__ out,
+                  float *__restrict__ lse) {
+  const size_t rh = (size_t)blockIdx.x * 64 + (threadIdx.x >> 2);  // (row, head) index
+  const int qd = threadIdx.x & 3;                                 // quarter of the head dim
+  if (rh >= (size_t)rows_off[num_reqs] * num_q_heads) return;
+  const size_t stride = (size_t)total_rows * num_q_heads;
+  float mx = -INFINITY;
+  for (int s = 0; s < splits; ++s) mx = fmaxf(mx, part_lse[s * stride + rh]);
+  float o[32], den = 0.f;
+#pragma unroll
+  for (int i = 0; i < 32; ++i) o[i] = 0.f;
+  for (int s = 0; s < splits; ++s) {
+    const float ls = part_lse[s * stride + rh];
+    if (ls == -INFINITY) continue;  // no visible key in this split: its O is undefined
+    const float w = __expf(ls - mx);
+    den += w;
+    const float4 *src = reinterpret_cast<const float4 *>(part_o + (s * stride + rh) * kHeadDim + qd * 32);
+#pragma unroll
+    for (int i = 0; i < 8; ++i) {
+      const float4 v = __ldg(src + i);
+      o[4 * i + 0] = fmaf(v.x, w, o[4 * i + 0]);
+      o[4 * i + 1] = fmaf(v.y, w, o[4 * i + 1]);
+      o[4 * i + 2] = fmaf(v.z, w, o[4 * i + 2]);
+      o[4 * i + 3] = fmaf(v.w, w, o[4 * i + 3]);
+    }
+  }
+  const float inv = 1.f / den;
+  uint4 *dst = reinterpret_cast<uint4 *>(out + rh * kHeadDim + qd * 32);
+#pragma unroll
+  for (int i = 0; i < 4; ++i) {
+    uint4 v;
+    v.x = pack_bf16x2(o[8 * i + 0] * inv, o[8 * i + 1] * inv);
+    v.y = pack_bf16x2(o[8 * i + 2] * inv, o[8 * i + 3] * inv);
+    v.z = pack_bf16x2(o[8 * i + 4] * inv, o[8 * i + 5] * inv);
+    v.w = pack_bf16x2(o[8 * i + 6] * inv, o[8 * i + 7] * inv);
+    dst[i] = v;
+  }
+  if (lse && qd == 0) lse[rh] = mx + logf(den);
+}
+
+// Row sets that fill tensor-core tiles but only a few CTAs (a handful of query tiles against a long context):
+// cut the key range so that ONE wave of CTAs exists (225 KB of shared memory: one CTA per SM; a few CTAs
+// spilling into a second wave would double the time); partial results are merged by attn_merge_kernel.
+// The partial buffer bounds splits * total_rows * Hq (each CTA covers at most 256 (row, head) pairs).
+constexpr int kAttnSplitCtas = 148;
+size_t attn_part_bytes() { return (size_t)2 * kAttnSplitCtas * 256 * (kHeadDim + 1) * sizeof(float); }
+
+int attn_pv_splits(const sx_pool *pool, const sx_batch *b, int32_t total_rows) {
+  const int g = pool->num_q_heads / pool->num_kv_heads;
+  const int grid = (total_rows / (2 * (kTile / g)) + b->num_reqs) * pool->num_kv_heads;
+  if (grid >= 148) return 1;
+  int s = kAttnSplitCtas / grid;
+  const int tiles = (b->max_seq_len + kTile - 1) / kTile;
+  if (s > tiles / 2) s = tiles / 2;  // at least two key tiles per split
+  if (s > 64) s = 64;
+  // splits * total_rows * Hq must fit the partial buffer
+  while (s > 1 && (size_t)s * total_rows * pool->num_q_heads > (size_t)2 * kAttnSplitCtas * 256) --s;
+  return s < 1 ? 1 : s;
+}
+
 // Key splits of the LSE-only sweep: enough CTAs for about four waves (a long single request gives few row
 // pairs: C5 has 57 x 4 KV heads), at most 8. The partial normalisers are merged by coltab_kernel.
 int attn_lse_splits(const sx_pool *pool, const sx_batch *b, int32_t total_rows) {
@@ -479,7 +569,7 @@ int attn_lse_splits(const sx_pool *pool, const sx_batch *b, int32_t total_rows) 
 
 sx_status launch_attn(const sx_pool *pool, const sx_batch *b, bool with_pv, const void *q, const int32_t *rows,
                       const int32_t *rows_off, int32_t total_rows, void *out, float *lse, int kv_splits,
-                      cudaStream_t st) {
+                      float *part, cudaStream_t st) {
   const int g = pool->num_q_heads / pool->num_kv_heads;
   const int rpt = kTile / g;
   CUtensorMap tm_q, tm_k, tm_v;
@@ -504,7 +594,9 @@ sx_status launch_attn(const sx_pool *pool, const sx_batch *b, bool with_pv, cons
   p.group = g;
   p.rows_per_tile = rpt;
   p.total_rows = total_rows;
-  p.kv_splits = with_pv ? 1 : kv_splits;
+  p.kv_splits = kv_splits < 1 ? 1 : kv_splits;
+  p.part_o = part;
+  p.part_lse = part ? part + (size_t)p.kv_splits * total_rows * pool->num_q_heads * kHeadDim : nullptr;
   p.scale = (float)(1.0 / sqrt((double)kHeadDim));
   p.scale_log2 = (float)(kLog2e / sqrt((double)kHeadDim));
   const int grid = (total_rows / (2 * rpt) + b->num_reqs) * pool->num_kv_heads;  // >= sum_r ceil(n_r / 2rpt) * Hkv
@@ -512,7 +604,15 @@ sx_status launch_attn(const sx_pool *pool, const sx_batch *b, bool with_pv, cons
   if (with_pv) {
     e = cudaFuncSetAttribute(attn_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, AttnCfg::kSmemBytes);
     if (e != cudaSuccess) return set_error(SX_ERR_CUDA, "attn smem attr: %s", cudaGetErrorString(e));
-    attn_kernel<true><<<grid, kAttnThreads, AttnCfg::kSmemBytes, st>>>(tm_q, tm_k, tm_v, p);
+    attn_kernel<true><<<grid * p.kv_splits, kAttnThreads, AttnCfg::kSmemBytes, st>>>(tm_q, tm_k, tm_v, p);
+    if (p.kv_splits > 1) {
+      sx_status ms = check_launch("attn_kernel<pv>");
+      if (ms != SX_OK) return ms;
+      const int blocks = (int)(((size_t)total_rows * pool->num_q_heads + 63) / 64);
+      attn_merge_kernel<<<blocks, 256, 0, st>>>(p.part_o, p.part_lse, p.kv_splits, total_rows, pool->num_q_heads, rows_off,
+                                                b->num_reqs, p.out, lse);
+      return check_launch("attn_merge_kernel");
+    }
   } else {
     e = cudaFuncSetAttribute(attn_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, AttnCfg::kSmemBytes);
     if (e != cudaSuccess) return set_error(SX_ERR_CUDA, "lse smem attr: %s", cudaGetErrorString(e));

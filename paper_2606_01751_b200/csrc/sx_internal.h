@@ -24,6 +24,7 @@ struct WsLayout {
   size_t col_tab;      // float2 [query tiles][Hkv][128]  (log2-domain lse, position) of every sweep-2 column
   size_t rows_tmp;     // int32  [total_tokens]           capacity-slotted R of the extended selection
   size_t rows_cnt;     // int32  [num_reqs]
+  size_t attn_part;    // float  key-split partials of the tcgen05 attention (few CTAs, long context)
   size_t small_part;   // float  split-KV partials of the CUDA-core attention path (sx_attn_small.cu)
   size_t total;
 };
@@ -44,7 +45,9 @@ sx_status launch_select(const sx_pool *pool, const sx_batch *b, const float *par
 // tcgen05 kernels. q_rows: bf16 [total_rows][Hq][128]; rows == nullptr => row n is position n - off[req].
 sx_status launch_attn(const sx_pool *pool, const sx_batch *b, bool with_pv, const void *q, const int32_t *rows,
                       const int32_t *rows_off, int32_t total_rows, void *out, float *lse, int kv_splits,
-                      cudaStream_t st);
+                      float *part, cudaStream_t st);
+int attn_pv_splits(const sx_pool *pool, const sx_batch *b, int32_t total_rows);
+size_t attn_part_bytes();
 int attn_lse_splits(const sx_pool *pool, const sx_batch *b, int32_t total_rows);
 // CUDA-core split-KV attention for fewer than 64 (row, head) pairs per KV head; part = ws.small_part
 sx_status launch_attn_small(const sx_pool *pool, const sx_batch *b, const void *q, const int32_t *rows,

@@ -375,3 +375,33 @@ def test_overflow_and_tail_fallback(ov, tail):
     assert total == sx_rows_total
     # tokens behind the last new token have score exactly 0 and are reached only through S_tail / S_key
     assert np.array_equal(dev_to_bits(g.pool_v), pv)
+
+
+@pytest.mark.parametrize("name,nlast", [("C5-1/16", 16), ("C1", 40), ("C3-eighth", 24)])
+def test_few_rows_tensor_core_path_with_key_splits(name, nlast):
+    """At least 64 (row, head) pairs per KV head but only a few query tiles against a long context: the tcgen05
+    kernel cuts the key range into splits (partial O and LSE in the workspace) and merges them."""
+    GpuLayer, dev_to_bits = _gpu()
+    lay, lt, res, pk, pv, kt, vt = prepared(name)
+    g = GpuLayer(lay, lt)
+    g.step_sparse()
+    rows, off = [], [0]
+    for r in range(lay.num_reqs):
+        t = int(lay.seq_len[r])
+        rr = np.unique(np.concatenate([np.arange(t - nlast, t), [3, t // 2]])).astype(np.int32)
+        rows.append(rr)
+        off.append(off[-1] + len(rr))
+    assert off[-1] * (lay.num_q_heads // lay.num_kv_heads) >= 64 * lay.num_reqs
+    g.rows_off = torch.tensor(off, dtype=torch.int32, device=g.dev)
+    g.sel_off = torch.zeros(lay.num_reqs + 1, dtype=torch.int32, device=g.dev)
+    g.stage_rows(torch.zeros(0, dtype=torch.int32, device=g.dev), torch.from_numpy(np.concatenate(rows)).to(g.dev))
+    g.attend()
+    torch.cuda.synchronize()
+    out = orc.bf16_to_f64(dev_to_bits(g.out))
+    lse = g.lse.cpu().numpy().astype(np.float64)
+    for r in range(lay.num_reqs):
+        o, t = int(lay.tok_off[r]), int(lay.seq_len[r])
+        ref_o, ref_l = orc.attention(pk, pv, kt[r], vt[r], t, lt.q_full[o + rows[r]], rows[r], lay.num_q_heads,
+                                     want_lse=True)
+        check_close("%s req %d O" % (name, r), out[off[r]:off[r + 1]], ref_o)
+        assert np.max(np.abs(lse[off[r]:off[r + 1]] - ref_l)) < 2e-3
