@@ -201,7 +201,7 @@ def score_select(pool: DevicePool, batch: DeviceBatch, q_new: torch.Tensor, sel_
                  lse_by_token: bool = False, stream=None):
     """Stage (b), Eq. (1)-(3): Sparse-Q scores, head/query aggregation, top-k, R = I_nr U S_key."""
     global LAUNCHES
-    LAUNCHES += 1 + ((3 if lse_new is None else 2) if batch.c.total_new else 0)   # [lse sweep] coltab colsum select
+    LAUNCHES += 2 + ((3 if lse_new is None else 2) if batch.c.total_new else 0)   # [lse sweep] coltab colsum score_sum select
     ws = batch.workspace(pool)
     _check(load().sx_score_select(ctypes.byref(pool.c), ctypes.byref(batch.c), _ptr(q_new), _ptr(lse_new),
                                   1 if lse_by_token else 0, _ptr(sel_off), _ptr(rows_off), _ptr(scores), _ptr(sel_idx), _ptr(rows_R),
@@ -216,7 +216,7 @@ def score_select_ex(pool: DevicePool, batch: DeviceBatch, q_new: torch.Tensor, s
     """Stage (b) with overflow and tail fallback (Alg. 1 l.535-539): R = I_nr U S_key U S_ov U S_tail; the
     actual CSR offsets of the packed rows_R come back in rows_off_out (device)."""
     global LAUNCHES
-    LAUNCHES += 2 + ((3 if lse_new is None else 2) if batch.c.total_new else 0)
+    LAUNCHES += 3 + ((3 if lse_new is None else 2) if batch.c.total_new else 0)
     ws = batch.workspace(pool)
     _check(load().sx_score_select_ex(ctypes.byref(pool.c), ctypes.byref(batch.c), _ptr(q_new), _ptr(lse_new),
                                      1 if lse_by_token else 0, _ptr(sel_off), _ptr(rows_cap_off),

@@ -49,6 +49,16 @@ __device__ __forceinline__ Scan3 block_scan3(bool fa, bool fb, bool fc, int (*wa
   return r;
 }
 
+// Head aggregation: scores[j] = sum over KV heads of the per-head column sums, fixed order.
+__global__ void __launch_bounds__(256)
+score_sum_kernel(int num_kv_heads, int total_tokens, const float *__restrict__ partial, float *__restrict__ scores) {
+  const int j = blockIdx.x * 256 + threadIdx.x;
+  if (j >= total_tokens) return;
+  float s = 0.f;
+  for (int h = 0; h < num_kv_heads; ++h) s += partial[(size_t)h * total_tokens + j];
+  scores[j] = s;
+}
+
 __global__ void __launch_bounds__(kSelThreads)
 select_kernel(int num_kv_heads, int total_tokens, const int32_t *__restrict__ seq_len,
               const int32_t *__restrict__ tok_off, const int32_t *__restrict__ new_off,
@@ -105,11 +115,7 @@ select_kernel(int num_kv_heads, int total_tokens, const int32_t *__restrict__ se
     }
   }
   // head aggregation in fixed order kvh = 0..Hkv-1 (global score across heads)
-  for (int j = threadIdx.x; j < T; j += kSelThreads) {
-    float s = 0.f;
-    for (int h = 0; h < num_kv_heads; ++h) s += partial[(size_t)h * total_tokens + off + j];
-    scores[off + j] = s;
-  }
+  // (the head sum of PAPER.md:225 was formed by score_sum_kernel, all SMs, before this launch)
   __syncthreads();
 
   // ---- radix select: bit pattern of the k-th largest candidate score
@@ -120,10 +126,23 @@ select_kernel(int num_kv_heads, int total_tokens, const int32_t *__restrict__ se
       const int shift = pass * 8;
       for (int i = threadIdx.x; i < 256; i += kSelThreads) hist[i] = 0;
       __syncthreads();
-      for (int j = threadIdx.x; j < T; j += kSelThreads) {
-        if (!((is_new[j >> 5] >> (j & 31)) & 1u)) {
-          uint32_t u = __float_as_uint(scores[off + j]);
-          if ((u & mask) == prefix) atomicAdd(&hist[(u >> shift) & 255u], 1);
+      // all 32 lanes stay in the loop (warp-aggregated histogram: the top digits of the scores take few
+      // distinct values, a plain shared-memory atomic per lane would serialise 32-fold)
+      for (int j0 = 0; j0 < T; j0 += 8 * kSelThreads) {
+        uint32_t u[8];  // eight independent loads in flight per thread: the pass is bound by load latency
+#pragma unroll
+        for (int q = 0; q < 8; ++q) {
+          const int j = j0 + q * kSelThreads + threadIdx.x;
+          u[q] = j < T ? __float_as_uint(scores[off + j]) : 0u;
+        }
+#pragma unroll
+        for (int q = 0; q < 8; ++q) {
+          const int j = j0 + q * kSelThreads + threadIdx.x;
+          int bin = -1;
+          if (j < T && !((is_new[j >> 5] >> (j & 31)) & 1u) && (u[q] & mask) == prefix)
+            bin = (int)((u[q] >> shift) & 255u);
+          const unsigned peers = __match_any_sync(0xffffffffu, bin);
+          if (bin >= 0 && (threadIdx.x & 31) == __ffs(peers) - 1) atomicAdd(&hist[bin], __popc(peers));
         }
       }
       __syncthreads();
@@ -166,37 +185,104 @@ select_kernel(int num_kv_heads, int total_tokens, const int32_t *__restrict__ se
   const uint32_t thr = prefix;
   const int take_eq = (k > 0) ? remaining : 0;
 
-  // ---- ordered emission
-  int base_eq = 0, base_sel = 0, base_r = 0;
-  const int so = sel_off[req], ro = rows_off[req];
-  for (int j0 = 0; j0 < T; j0 += kSelThreads) {
-    const int j = j0 + threadIdx.x;
-    bool isn = false, gt = false, eq = false, frc = false;
-    if (j < T) {
+  // ---- ordered emission. Every warp owns one contiguous range of positions and walks it 32 at a time
+  // (coalesced); ranks inside a warp come from ballots, ranks across warps from one 32-entry scan per phase:
+  //   A: equals of the threshold per warp -> which of them are taken (lowest positions first, reading A8)
+  //   B: |S_key| and |R| per warp          C: write S_key and R in ascending position order
+  // (three cheap passes over L2-resident scores instead of a block-wide scan per 1024 positions)
+  const int so = sel_off[req], ro = rows_off[req], cap_r = rows_off[req + 1] - ro;
+  const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
+  const unsigned lt = (1u << lane) - 1u;
+  const int seg = (((T + kSelWarps - 1) / kSelWarps) + 127) & ~127;  // positions per warp, multiple of 32 * kB
+  const int j_lo = w * seg, j_hi = min(T, j_lo + seg);
+  constexpr int kB = 4;  // groups of 32 positions whose score loads are issued together
+  auto load4 = [&](int j0, uint32_t (&u)[kB]) {
+#pragma unroll
+    for (int q = 0; q < kB; ++q) {
+      const int j = j0 + q * 32 + lane;
+      u[q] = j < j_hi ? __float_as_uint(scores[off + j]) : 0u;
+    }
+  };
+  auto flags = [&](int j, uint32_t u, bool &isn, bool &gt, bool &eq, bool &frc) {
+    isn = gt = eq = frc = false;
+    if (j < j_hi) {
       isn = (is_new[j >> 5] >> (j & 31)) & 1u;
       frc = (forced[j >> 5] >> (j & 31)) & 1u;
       if (!isn && k > 0) {
-        uint32_t u = __float_as_uint(scores[off + j]);
         gt = u > thr;
         eq = u == thr;
       }
     }
-    // rank among equals decides eq membership; it needs the eq scan first
-    Scan3 s1 = block_scan3(eq, false, false, warp_tot, tot);
-    const int tot_eq = tot[0];
-    const bool sel = gt || (eq && (base_eq + s1.a) < take_eq);
+  };
+  // exclusive scan of one per-warp counter over the 32 warps (all threads get their warp's base)
+  auto warp_base = [&](int mine, int *total) -> int {
     __syncthreads();
-    const bool in_r = sel || isn || frc;  // R = I_nr U S_key U S_ov U S_tail (Alg. 1 l.537-539)
-    Scan3 s2 = block_scan3(sel, in_r, false, warp_tot, tot);
-    if (sel) sel_idx[so + base_sel + s2.a] = j;
-    if (in_r && base_r + s2.b < rows_off[req + 1] - ro) rows_R[ro + base_r + s2.b] = j;
-    const int tsel = tot[0], tr = tot[1];
+    if (lane == 0) warp_tot[0][w] = mine;
     __syncthreads();
-    base_eq += tot_eq;
-    base_sel += tsel;
-    base_r += tr;
+    if (w == 0) {
+      const int v = warp_tot[0][lane];
+      int x = v;
+#pragma unroll
+      for (int d = 1; d < 32; d <<= 1) {
+        const int y = __shfl_up_sync(0xffffffffu, x, d);
+        if (lane >= d) x += y;
+      }
+      warp_tot[1][lane] = x - v;
+      if (lane == 31) tot[0] = x;
+    }
+    __syncthreads();
+    if (total) *total = tot[0];
+    return warp_tot[1][w];
+  };
+  bool isn, gt, eq, frc;
+  int n_eq = 0;
+  uint32_t ub[kB];
+  for (int j0 = j_lo; j0 < j_hi; j0 += 32 * kB) {
+    load4(j0, ub);
+#pragma unroll
+    for (int q = 0; q < kB; ++q) {
+      flags(j0 + q * 32 + lane, ub[q], isn, gt, eq, frc);
+      n_eq += __popc(__ballot_sync(0xffffffffu, eq));
+    }
   }
-  if (rows_cnt && threadIdx.x == 0) rows_cnt[req] = min(base_r, rows_off[req + 1] - ro);
+  const int eq_base = warp_base(n_eq, nullptr);
+  int n_sel = 0, n_r = 0, run_eq = eq_base;
+  for (int j0 = j_lo; j0 < j_hi; j0 += 32 * kB) {
+    load4(j0, ub);
+#pragma unroll
+    for (int q = 0; q < kB; ++q) {
+      flags(j0 + q * 32 + lane, ub[q], isn, gt, eq, frc);
+      const unsigned be = __ballot_sync(0xffffffffu, eq);
+      const bool sel = gt || (eq && run_eq + __popc(be & lt) < take_eq);
+      run_eq += __popc(be);
+      n_sel += __popc(__ballot_sync(0xffffffffu, sel));
+      n_r += __popc(__ballot_sync(0xffffffffu, sel || isn || frc));  // R = I_nr U S_key U S_ov U S_tail
+    }
+  }
+  const int sel_base = warp_base(n_sel, nullptr);
+  int total_r = 0;
+  const int r_base = warp_base(n_r, &total_r);
+  int run_sel = sel_base, run_r = r_base;
+  run_eq = eq_base;
+  for (int j0 = j_lo; j0 < j_hi; j0 += 32 * kB) {
+    load4(j0, ub);
+#pragma unroll
+    for (int q = 0; q < kB; ++q) {
+      const int j = j0 + q * 32 + lane;
+      flags(j, ub[q], isn, gt, eq, frc);
+      const unsigned be = __ballot_sync(0xffffffffu, eq);
+      const bool sel = gt || (eq && run_eq + __popc(be & lt) < take_eq);
+      run_eq += __popc(be);
+      const bool in_r = sel || isn || frc;
+      const unsigned bs = __ballot_sync(0xffffffffu, sel), br = __ballot_sync(0xffffffffu, in_r);
+      if (sel) sel_idx[so + run_sel + __popc(bs & lt)] = j;
+      const int rr = run_r + __popc(br & lt);
+      if (in_r && rr < cap_r) rows_R[ro + rr] = j;
+      run_sel += __popc(bs);
+      run_r += __popc(br);
+    }
+  }
+  if (rows_cnt && threadIdx.x == 0) rows_cnt[req] = min(total_r, cap_r);
 }
 
 // Extended selection only: per-request row lists sit in capacity-sized slots of `tmp`; pack them into one
@@ -224,6 +310,9 @@ sx_status launch_select(const sx_pool *pool, const sx_batch *b, const float *par
     cudaError_t e = cudaFuncSetAttribute(select_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (e != cudaSuccess) return set_error(SX_ERR_CUDA, "select smem attr: %s", cudaGetErrorString(e));
   }
+  score_sum_kernel<<<(b->total_tokens + 255) / 256, 256, 0, st>>>(pool->num_kv_heads, b->total_tokens, partial, scores);
+  sx_status s0 = check_launch("score_sum_kernel");
+  if (s0 != SX_OK) return s0;
   const bool ex = rows_off_out != nullptr;  // extended: variable |R|, slots of capacity rows_off, then compaction
   select_kernel<<<b->num_reqs, kSelThreads, smem, st>>>(
       pool->num_kv_heads, b->total_tokens, b->seq_len, b->tok_off, b->new_off, b->new_idx, partial, sel_off, rows_off,
