@@ -617,6 +617,9 @@ def run_reference(args):
     world = int(os.environ.get("WORLD_SIZE", "1"))
     if rank != 0:
         return
+    # torchrun exports OMP_NUM_THREADS=1 for its workers; the one rank that runs the oracle uses the host's cores
+    if os.environ.get("OMP_NUM_THREADS", "1") == "1":
+        os.environ["OMP_NUM_THREADS"] = str(os.cpu_count() or 1)
     cfg = args.config
     stack = cfg == "C3"
     lay = wl.CONFIGS[cfg]()
