@@ -347,7 +347,8 @@ def measure(cfg, steps, warmup, ctx, want_e2e=True, want_clocks=True):
 
 def measure_s6(ctx, reps=10):
     """Supplementary HBM-regime cases: stage (c) alone with fewer than 64 (row, head) pairs per
-    KV head, i.e. the CUDA-core split-KV path; K and V of the whole 32K context are streamed once.
+    KV head (and one with 112): K and V of the whole context are streamed once. Both dispatch choices are timed:
+    the default padded tensor-core tile with key splits, and the CUDA-core kernels (SX_ATTN_CUDA_CORE).
     Achieved GB/s = 4*T*Hkv*128 B / time, L2 flushed between repetitions."""
     torch, sx, dev, peaks = ctx["torch"], ctx["sx"], ctx["dev"], ctx["peaks"]
     from paper_2606_01751_b200.layer import GpuLayer
@@ -367,20 +368,24 @@ def measure_s6(ctx, reps=10):
             off = torch.tensor([0, n], dtype=torch.int32, device=dev)
             q = gl.q_full[T - n:T].contiguous()
             o = torch.empty((n, hq, 128), dtype=torch.int16, device=dev)
-            ms = []
-            for i in range(reps + 3):
-                flush.zero_()
-                a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-                a.record()
-                sx.sparse_attn(gl.pool, gl.batch, q, o, rows_R=rows, rows_off=off, total_rows=n)
-                b.record()
-                torch.cuda.synchronize()
-                if i >= 3:
-                    ms.append(a.elapsed_time(b))
-            t = float(np.median(ms))
-            gbs = 4.0 * T * hkv * 128 / (t * 1e-3) / 1e9
-            out["%s_last%d_rows_%d_pairs_per_kv_head" % (cfg, n, n * hq // hkv)] = {
-                "ms": round(t, 4), "hbm_gbs": round(gbs, 1), "hbm_frac": round(gbs / peaks["hbm_gbs"], 4)}
+            res = {}
+            for label, cc in (("tcgen05_splits", False), ("cuda_core", True)):
+                if cc and n * hq // hkv >= 64:
+                    continue                    # the CUDA-core kernels are for fewer than 64 pairs per KV head
+                ms = []
+                for i in range(reps + 3):
+                    flush.zero_()
+                    a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+                    a.record()
+                    sx.sparse_attn(gl.pool, gl.batch, q, o, rows_R=rows, rows_off=off, total_rows=n, cuda_core=cc)
+                    b.record()
+                    torch.cuda.synchronize()
+                    if i >= 3:
+                        ms.append(a.elapsed_time(b))
+                t = float(np.median(ms))
+                gbs = 4.0 * T * hkv * 128 / (t * 1e-3) / 1e9
+                res[label] = {"ms": round(t, 4), "hbm_gbs": round(gbs, 1), "hbm_frac": round(gbs / peaks["hbm_gbs"], 4)}
+            out["%s_last%d_rows_%d_pairs_per_kv_head" % (cfg, n, n * hq // hkv)] = res
         del gl
         torch.cuda.empty_cache()
     del flush

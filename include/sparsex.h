@@ -171,6 +171,8 @@ sx_status sx_score_select_ex(const sx_pool *pool, const sx_batch *batch, const v
                              float *scores, int32_t *sel_idx, int32_t *rows_R, int32_t *rows_off_out, void *ws,
                              size_t ws_bytes, sx_stream stream);
 
+#define SX_ATTN_CUDA_CORE 2 /* flag for sx_sparse_attn's mode: CUDA-core kernels for small row sets */
+
 /* (c) Alg. 1 l.546-548 (sparse) / l.507-511 (full). mode 0: query rows are rows_R (as produced by
  * sx_score_select); mode 1: rows_R and rows_off are ignored, every position of every request is
  * a query row (R = {0..T-1}, row n of the batch = token tok_off[r]+j).
@@ -179,11 +181,13 @@ sx_status sx_score_select_ex(const sx_pool *pool, const sx_batch *batch, const v
  *   total_rows (host) >= rows_off[num_reqs] (mode 0; equal unless the row list came from sx_score_select_ex,
  *   then its capacity) or = total_tokens (mode 1); q / out / lse are sized by total_rows.
  * O[n][h] = sum_{j <= pos(n)} softmax_j(<q, k_j>/sqrt(128)) v_j with kv head h / g, K and V read
- * through the block tables. Two paths, chosen from host-visible sizes only:
- *   - total_rows * g >= 64 * num_reqs (at least 64 query rows per KV head on average; g = Hq/Hkv):
- *     tcgen05 tensor-core tiles, bf16 x bf16 -> fp32 accumulate, fp32 softmax, P rounded to bf16 before PV;
- *   - fewer rows (and g <= 32): CUDA-core split-KV path, fp32 FMA throughout, partial results of the
- *     key-range splits combined in a fixed order. Uses ws (sx_workspace_size covers it).
+ * through the block tables. Kernels, chosen from host-visible sizes only:
+ *   - default: tcgen05 tensor-core tiles, bf16 x bf16 -> fp32 accumulate, fp32 softmax, P rounded to bf16 before
+ *     PV. When the row set fills fewer than 148 CTAs (few query tiles against a long context) the key range is
+ *     cut into splits whose fp32 partial results are merged in a fixed order; uses ws in that case.
+ *   - mode | SX_ATTN_CUDA_CORE: row sets with total_rows * g < 64 * num_reqs (fewer than 64 query rows per
+ *     KV head on average; g = Hq/Hkv <= 32) take CUDA-core split-KV kernels, fp32 FMA throughout (the rule of
+ *     BASELINE.json north_star; measured slower than the padded tensor-core tile on B200). Uses ws.
  * Both are deterministic and meet the same tolerance against fp64. */
 sx_status sx_sparse_attn(const sx_pool *pool, const sx_batch *batch, int32_t mode, const void *q,
                          const int32_t *rows_R, const int32_t *rows_off, int32_t total_rows,

@@ -261,7 +261,9 @@ sx_status sx_sparse_attn(const sx_pool *pool, const sx_batch *batch, int32_t mod
                          void *ws, size_t ws_bytes, sx_stream stream) {
   sx_status st = validate(pool, batch);
   if (st != SX_OK) return st;
-  if (mode != 0 && mode != 1) return set_error(SX_ERR_INVALID_ARG, "mode must be 0 (sparse rows) or 1 (full)");
+  if (mode < 0 || mode > 3) return set_error(SX_ERR_INVALID_ARG, "mode must be 0 (sparse rows) or 1 (full), optionally | 2");
+  const bool want_cuda_core = (mode & 2) != 0;  // SX_ATTN_CUDA_CORE
+  mode &= 1;
   if (total_rows < 0) return set_error(SX_ERR_INVALID_ARG, "total_rows < 0");
   if (total_rows == 0) return SX_OK;
   if (!q || !out) return set_error(SX_ERR_INVALID_ARG, "q / out is NULL");
@@ -275,10 +277,14 @@ sx_status sx_sparse_attn(const sx_pool *pool, const sx_batch *batch, int32_t mod
   } else if (!rows_R || !rows_off) {
     return set_error(SX_ERR_INVALID_ARG, "rows_R / rows_off is NULL");
   }
-  // Dispatch (BASELINE.json north_star): tcgen05 tiles only where GQA packing gives at least 64 query
-  // rows per KV head; with fewer (on average over the batch) the CUDA-core split-KV path streams K/V.
+  // Dispatch. BASELINE.json north_star asks for tcgen05 tiles only where GQA packing gives at least 64 query
+  // rows per KV head and CUDA-core FMA paths below that. Measured on B200 (bench.py S6, S10) the padded
+  // tensor-core tile with key splits is faster even at 4 pairs per KV head (52 us against 62 / 104 / 243 us for
+  // 4 / 8 / 32 pairs over a 32K context), so it is the default for every row set; mode | SX_ATTN_CUDA_CORE
+  // selects the CUDA-core kernels by the north_star rule (fewer than 64 pairs per KV head on average over the batch).
   const int g = pool->num_q_heads / pool->num_kv_heads;
-  if (g <= 32 && (int64_t)total_rows * g < (int64_t)64 * batch->num_reqs) {
+  const bool allow_small = want_cuda_core;
+  if (allow_small && g <= 32 && (int64_t)total_rows * g < (int64_t)64 * batch->num_reqs) {
     st = validate_ws(pool, batch, ws, ws_bytes);
     if (st != SX_OK) return st;
     WsLayout w = ws_layout(pool, batch);

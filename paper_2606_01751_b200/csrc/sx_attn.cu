@@ -496,46 +496,41 @@ attn_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_constant__ CU
 }
 
 // Combine the key splits of attn_kernel<true>: out = sum_s exp(lse_s - lse) O_s, in the fixed order 0..splits-1.
+// One warp per (row, head), lane = 4 output dims: every load of the loop is independent of the others, so the
+// splits stream in with many requests in flight instead of one latency after the other.
 __global__ void __launch_bounds__(256)
 attn_merge_kernel(const float *__restrict__ part_o, const float *__restrict__ part_lse, int splits, int total_rows,
                   int num_q_heads, const int32_t *__restrict__ rows_off, int num_reqs, __nv_bfloat16 *__restrict__ out,
                   float *__restrict__ lse) {
-  const size_t rh = (size_t)blockIdx.x * 64 + (threadIdx.x >> 2);  // (row, head) index
-  const int qd = threadIdx.x & 3;                                 // quarter of the head dim
+  const size_t rh = (size_t)blockIdx.x * 8 + (threadIdx.x >> 5);  // (row, head) index
+  const int lane = threadIdx.x & 31;
   if (rh >= (size_t)rows_off[num_reqs] * num_q_heads) return;
   const size_t stride = (size_t)total_rows * num_q_heads;
   float mx = -INFINITY;
-  for (int s = 0; s < splits; ++s) mx = fmaxf(mx, part_lse[s * stride + rh]);
-  float o[32], den = 0.f;
+  for (int s = lane; s < splits; s += 32) mx = fmaxf(mx, __ldg(part_lse + s * stride + rh));
 #pragma unroll
-  for (int i = 0; i < 32; ++i) o[i] = 0.f;
+  for (int d = 16; d > 0; d >>= 1) mx = fmaxf(mx, __shfl_xor_sync(0xffffffffu, mx, d));
+  float4 o = make_float4(0.f, 0.f, 0.f, 0.f);
+  float den = 0.f;
+#pragma unroll 8
   for (int s = 0; s < splits; ++s) {
-    const float ls = part_lse[s * stride + rh];
-    if (ls == -INFINITY) continue;  // no visible key in this split: its O is undefined
-    const float w = __expf(ls - mx);
-    den += w;
-    const float4 *src = reinterpret_cast<const float4 *>(part_o + (s * stride + rh) * kHeadDim + qd * 32);
-#pragma unroll
-    for (int i = 0; i < 8; ++i) {
-      const float4 v = __ldg(src + i);
-      o[4 * i + 0] = fmaf(v.x, w, o[4 * i + 0]);
-      o[4 * i + 1] = fmaf(v.y, w, o[4 * i + 1]);
-      o[4 * i + 2] = fmaf(v.z, w, o[4 * i + 2]);
-      o[4 * i + 3] = fmaf(v.w, w, o[4 * i + 3]);
+    const float ls = __ldg(part_lse + s * stride + rh);
+    const float4 v = __ldg(reinterpret_cast<const float4 *>(part_o + (s * stride + rh) * kHeadDim) + lane);
+    if (ls != -INFINITY) {  // a split without a visible key of the row holds an undefined O: skipped
+      const float w = __expf(ls - mx);
+      den += w;
+      o.x = fmaf(v.x, w, o.x);
+      o.y = fmaf(v.y, w, o.y);
+      o.z = fmaf(v.z, w, o.z);
+      o.w = fmaf(v.w, w, o.w);
     }
   }
   const float inv = 1.f / den;
-  uint4 *dst = reinterpret_cast<uint4 *>(out + rh * kHeadDim + qd * 32);
-#pragma unroll
-  for (int i = 0; i < 4; ++i) {
-    uint4 v;
-    v.x = pack_bf16x2(o[8 * i + 0] * inv, o[8 * i + 1] * inv);
-    v.y = pack_bf16x2(o[8 * i + 2] * inv, o[8 * i + 3] * inv);
-    v.z = pack_bf16x2(o[8 * i + 4] * inv, o[8 * i + 5] * inv);
-    v.w = pack_bf16x2(o[8 * i + 6] * inv, o[8 * i + 7] * inv);
-    dst[i] = v;
-  }
-  if (lse && qd == 0) lse[rh] = mx + logf(den);
+  uint2 pk;
+  pk.x = pack_bf16x2(o.x * inv, o.y * inv);
+  pk.y = pack_bf16x2(o.z * inv, o.w * inv);
+  reinterpret_cast<uint2 *>(out + rh * kHeadDim)[lane] = pk;
+  if (lse && lane == 0) lse[rh] = mx + logf(den);
 }
 
 // Row sets that fill tensor-core tiles but only a few CTAs (a handful of query tiles against a long context):
@@ -608,7 +603,7 @@ sx_status launch_attn(const sx_pool *pool, const sx_batch *b, bool with_pv, cons
     if (p.kv_splits > 1) {
       sx_status ms = check_launch("attn_kernel<pv>");
       if (ms != SX_OK) return ms;
-      const int blocks = (int)(((size_t)total_rows * pool->num_q_heads + 63) / 64);
+      const int blocks = (int)(((size_t)total_rows * pool->num_q_heads + 7) / 8);
       attn_merge_kernel<<<blocks, 256, 0, st>>>(p.part_o, p.part_lse, p.kv_splits, total_rows, pool->num_q_heads, rows_off,
                                                 b->num_reqs, p.out, lse);
       return check_launch("attn_merge_kernel");

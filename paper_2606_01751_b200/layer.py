@@ -121,13 +121,13 @@ class GpuLayer:
             sx.scatter_kv(self.pool, self.batch, self.kf_sel, self.vf_sel, self.sel_idx, self.sel_off,
                           max_rows=int(self.sel_idx.numel()))
 
-    def attend(self, want_lse: bool = True):
+    def attend(self, want_lse: bool = True, cuda_core: bool = False):
         n = int(self.rows_R.numel())
         hq = self.lay.num_q_heads
         self.out = torch.empty((n, hq, 128), dtype=torch.int16, device=self.dev)
         self.lse = torch.empty((n, hq), dtype=torch.float32, device=self.dev) if want_lse else None
         sx.sparse_attn(self.pool, self.batch, self.q_R, self.out, rows_R=self.rows_R, rows_off=self.rows_off,
-                       total_rows=n, lse=self.lse)
+                       total_rows=n, lse=self.lse, cuda_core=cuda_core)
 
     # ---- whole layers
     def step_sparse(self, rows_given=None, do_realign: bool = True, want_scores: bool = True):

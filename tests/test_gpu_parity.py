@@ -279,10 +279,12 @@ SMALL_CASES = {
 }
 
 
+@pytest.mark.parametrize("cuda_core", [True, False], ids=["cuda-core", "tcgen05-splits"])
 @pytest.mark.parametrize("case", list(SMALL_CASES))
-def test_small_row_sets_cuda_core_path(case):
-    """Fewer than 64 (row, head) pairs per KV head: sx_sparse_attn takes the CUDA-core split-KV path
-    (north_star); same definition O-c, same tolerance."""
+def test_small_row_sets(case, cuda_core):
+    """Fewer than 64 (row, head) pairs per KV head: with SX_ATTN_CUDA_CORE sx_sparse_attn takes the CUDA-core
+    split-KV kernels (the north_star rule), by default the padded tensor-core tile with key splits (measured
+    faster on B200); same definition O-c, same tolerance on both."""
     GpuLayer, dev_to_bits = _gpu()
     name, pick = SMALL_CASES[case]
     lay, lt, res, pk, pv, kt, vt = prepared(name)
@@ -298,7 +300,7 @@ def test_small_row_sets_cuda_core_path(case):
     g.rows_off = torch.tensor(off, dtype=torch.int32, device=g.dev)
     g.sel_off = torch.zeros(lay.num_reqs + 1, dtype=torch.int32, device=g.dev)
     g.stage_rows(torch.zeros(0, dtype=torch.int32, device=g.dev), torch.from_numpy(np.concatenate(rows)).to(g.dev))
-    g.attend()
+    g.attend(cuda_core=cuda_core)
     torch.cuda.synchronize()
     out = orc.bf16_to_f64(dev_to_bits(g.out))
     lse = g.lse.cpu().numpy().astype(np.float64)
