@@ -409,6 +409,12 @@ def run_ours(args):
     ctx = {"torch": torch, "sx": sx, "du": du, "dev": dev, "local": local, "rank": rank, "world": world,
            "peaks": load_peaks(), "args": args}
     cfg = args.config
+    if cfg == "S6":   # supplementary: stage (c) alone on small row sets (HBM regime); not the headline metric
+        if rank == 0:
+            print(json.dumps({"metric": "small_row_attention_hbm", "unit": "GB/s", "n_gpus": 1, "dtype": "bf16",
+                              "data": "synthetic", "config": {"workload": "S6: last rows of a 32K / 133K context"},
+                              "cases": measure_s6(ctx, reps=max(args.steps, 3))}), flush=True)
+        return
     m = measure(cfg, args.steps, args.warmup, ctx)
     # the other configs of BASELINE.json (north_star: throughput of all five at 1 GPU): short runs, same code path
     others = {}
@@ -652,7 +658,7 @@ def main():
     ap.add_argument("--gpus", type=int, default=1)
     ap.add_argument("--steps", type=int, default=10)
     ap.add_argument("--warmup", type=int, default=3)
-    ap.add_argument("--config", default="C3", choices=list(wl.CONFIGS))
+    ap.add_argument("--config", default="C3", choices=list(wl.CONFIGS) + ["S6"])
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--cpu-seconds", type=float, default=20.0)
     ap.add_argument("--no-cpu", action="store_true")
