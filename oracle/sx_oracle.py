@@ -16,11 +16,16 @@ What each function is (all fp64; inputs are bf16 bit patterns widened exactly):
                           Pins: sum_j s_j = N_n*Hq, Q=0 harmonic closed form, brute-force python loops.
   select_topk()      O-b  Eq. (3) PAPER.md:207-209 restricted to I_reuse (reading A7), ties -> lower
                           position (A8). Pins: full stable sort on tiny inputs, k=0, k=N_c.
+  recompute_set()    O-b  Alg. 1 l.535-539: R = I_nr U S_key U S_ov U S_tail (overflow by
+                          one block around every Sparse-Q interval, tail fallback of 64 tokens). Pins: hand-typed
+                          expected lists -- tests/test_oracle_pins.py::test_recompute_set_hand_cases.
   attention()        O-c  Alg. 1 line 21 (C loops). Pins: R=all == fp64 torch SDPA,
                           Q=0 prefix mean of V, T=1, constant V, rows-subset == full on those rows.
   layer_sparse()/layer_full()  O-layer driver: order realign -> scatter(new) -> select -> scatter(S_key)
                           -> attention (reading A13: Alg. 1 writes fresh K,V at line 19 before line 21).
                           Pin: ratio 100% == dense causal attention over the fresh tensors.
+
+(The host-side segment index has its own plain-dict reference in oracle/sx_index_oracle.py.)
 
 No function here is "parity unpinned"; no pin comes from numbers printed in the paper (it prints none
 for this path).
