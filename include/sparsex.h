@@ -17,6 +17,8 @@
  *   - Every call is asynchronous on `stream` and never synchronises the device. A non-zero status
  *     means nothing was launched (argument errors) or a launch failed (SX_ERR_CUDA);
  *     sx_last_error() then returns a thread-local description.
+ *   - The workspace `ws` is scratch that calls write: calls that may run concurrently (different streams)
+ *     need their own workspace; consecutive calls on one stream may share it.
  *   - bf16 tensors are raw 16-bit patterns. All device pointers must be 16-byte aligned.
  *   - head_dim must be 128 and block_size 16 (SX_ERR_UNSUPPORTED otherwise);
  *     num_q_heads % num_kv_heads == 0, group size g = Hq/Hkv <= 128.
