@@ -333,7 +333,33 @@ def measure(cfg, steps, warmup, ctx, want_e2e=True, want_clocks=True):
         sel_fl = select_flops(lay, hq, 1 if stack else 2)
         hbm["select_tflops"] = round(sel_fl / (stage_ms["select"] * 1e-3) / 1e12, 1)
 
+    # launch-bound single-layer configs: the same step replayed from a CUDA graph (no host launch gaps)
+    graph_ms = None
+    if not stack:
+        try:
+            gr = torch.cuda.CUDAGraph()
+            with torch.cuda.graph(gr):
+                step()
+            for _ in range(3):
+                gr.replay()
+            torch.cuda.synchronize()
+            gms = []
+            for _ in range(max(steps, 5)):
+                flush.zero_()
+                a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+                a.record()
+                gr.replay()
+                b.record()
+                torch.cuda.synchronize()
+                gms.append(a.elapsed_time(b))
+            graph_ms = float(np.median(gms))
+            del gr
+        except Exception as e:     # capture not possible: report the reason, keep the stream-launched number
+            graph_ms = "capture failed: %s" % str(e).splitlines()[0][:120]
+            torch.cuda.synchronize()
+
     res = {"cfg": cfg, "lay": lay, "stack": stack, "n_layers": n_layers, "T": T, "rows_R": n_rows_total,
+           "graph_ms": graph_ms,
            "n_sparse": n_sparse, "ms_per_step": ms_per_step, "stage_ms": stage_ms, "stage_n": stage_n,
            "roofline": roofline, "hbm": hbm, "clocks": clocks, "launches": launches,
            "value": du.job_throughput(T * n_layers, ms_per_step, world), "bytes_per_step": re_bytes + sc_bytes,
@@ -425,6 +451,8 @@ def run_ours(args):
             o = measure(c, 30 if c != "C3" else 2, 5, ctx, want_e2e=False, want_clocks=False)
             others[c] = {"context_tokens": o["T"], "rows_R": o["rows_R"], "layers": o["n_layers"],
                          "ms_per_layer": round(o["ms_per_step"] / o["n_layers"], 4),
+                         "ms_per_layer_cuda_graph": (round(o["graph_ms"], 4) if isinstance(o["graph_ms"], float)
+                                                     else o["graph_ms"]),
                          "context_tokens_per_s": round(o["value"], 1),
                          "stage_ms": {k: round(v, 4) for k, v in o["stage_ms"].items()},
                          "attn_tflops": o["roofline"]["achieved"], "attn_frac": o["roofline"]["frac"],
