@@ -47,6 +47,8 @@ WsLayout ws_layout(const sx_pool *pool, const sx_batch *b) {
   off = align_up(off + sizeof(int32_t) * (size_t)b->num_reqs, 256);
   w.attn_part = off;
   off = align_up(off + attn_part_bytes(), 256);
+  w.sel_scratch = off;
+  off = align_up(off + select_scratch_bytes(b), 256);
   w.small_part = off;
   off = align_up(off + small_ws_bytes(b->num_reqs, pool->num_kv_heads, pool->num_q_heads / pool->num_kv_heads), 256);
   w.total = off;
@@ -246,7 +248,7 @@ sx_status sx_score_select_ex(const sx_pool *pool, const sx_batch *batch, const v
   float *sc = scores ? scores : reinterpret_cast<float *>(base + w.scores);
   return launch_select(pool, batch, partial, sel_off, rows_off, sc, sel_idx, rows_R, overflow_blocks, tail_tokens,
                        reinterpret_cast<int32_t *>(base + w.rows_tmp), reinterpret_cast<int32_t *>(base + w.rows_cnt),
-                       rows_off_out, s);
+                       rows_off_out, reinterpret_cast<int *>(base + w.sel_scratch), s);
 }
 
 sx_status sx_score_select(const sx_pool *pool, const sx_batch *batch, const void *q_new, const float *lse_new,

@@ -24,6 +24,7 @@ struct WsLayout {
   size_t col_tab;      // float2 [query tiles][Hkv][128]  (log2-domain lse, position) of every sweep-2 column
   size_t rows_tmp;     // int32  [total_tokens]           capacity-slotted R of the extended selection
   size_t rows_cnt;     // int32  [num_reqs]
+  size_t sel_scratch;  // int    [num_reqs][4*256 + 4*64] digit histograms and slice counters of the multi-CTA select
   size_t attn_part;    // float  key-split partials of the tcgen05 attention (few CTAs, long context)
   size_t small_part;   // float  split-KV partials of the CUDA-core attention path (sx_attn_small.cu)
   size_t total;
@@ -40,8 +41,9 @@ sx_status launch_scatter(const sx_pool *pool, const sx_batch *b, const void *k_f
                          const int32_t *rows, const int32_t *rows_off, int32_t max_rows, cudaStream_t st);
 sx_status launch_select(const sx_pool *pool, const sx_batch *b, const float *partial, const int32_t *sel_off,
                         const int32_t *rows_off, float *scores, int32_t *sel_idx, int32_t *rows_R, int ov_blocks,
-                        int tail_tokens, int32_t *rows_tmp, int32_t *rows_cnt, int32_t *rows_off_out,
+                        int tail_tokens, int32_t *rows_tmp, int32_t *rows_cnt, int32_t *rows_off_out, int *scratch,
                         cudaStream_t st);
+size_t select_scratch_bytes(const sx_batch *b);
 // tcgen05 kernels. q_rows: bf16 [total_rows][Hq][128]; rows == nullptr => row n is position n - off[req].
 sx_status launch_attn(const sx_pool *pool, const sx_batch *b, bool with_pv, const void *q, const int32_t *rows,
                       const int32_t *rows_off, int32_t total_rows, void *out, float *lse, int kv_splits,

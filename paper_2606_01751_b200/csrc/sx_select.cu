@@ -6,6 +6,8 @@
 // One CTA per request. Scores are non-negative fp32, so their bit patterns order like unsigned
 // integers: 4-pass 8-bit radix select finds the k-th largest pattern, one ordered pass with block
 // scans then emits S_key and R. Integer atomics only (deterministic).
+#include <cooperative_groups.h>
+
 #include "sx_internal.h"
 #include "sx_ptx.cuh"
 
@@ -65,7 +67,15 @@ select_kernel(int num_kv_heads, int total_tokens, const int32_t *__restrict__ se
               const int32_t *__restrict__ new_idx, const float *__restrict__ partial,
               const int32_t *__restrict__ sel_off, const int32_t *__restrict__ rows_off, float *__restrict__ scores,
               int32_t *__restrict__ sel_idx, int32_t *__restrict__ rows_R, int ov_tokens, int tail_tokens,
-              const sx_segment *__restrict__ segs, int num_segments, int32_t *__restrict__ rows_cnt) {
+              const sx_segment *__restrict__ segs, int num_segments, int32_t *__restrict__ rows_cnt,
+              int *__restrict__ scratch) {
+  // gridDim.y > 1 (cooperative launch, long requests): the positions of a request are cut into gridDim.y
+  // slices, one CTA each; digit histograms and the per-slice counts of the ordered emission meet in `scratch`
+  // (zeroed by the launcher) and the CTAs of the grid synchronise between the phases.
+  namespace cg = cooperative_groups;
+  const int ns = gridDim.y, sl = blockIdx.y;
+  int *ghist = scratch + (size_t)blockIdx.x * (4 * 256 + 4 * 64);  // [4 passes][256] then [4 counters][64 slices]
+  int *gcnt = ghist + 4 * 256;
   extern __shared__ uint32_t is_new[];  // bitmap over positions; a second bitmap (forced rows) follows it
   __shared__ int hist[256];
   __shared__ int warp_tot[3][kSelWarps];
@@ -76,6 +86,9 @@ select_kernel(int num_kv_heads, int total_tokens, const int32_t *__restrict__ se
   const int req = blockIdx.x;
   const int T = seq_len[req];
   const int off = tok_off[req];
+  // slice [jb, je) of this CTA, a multiple of 128 positions long (the emission walks 4 x 32 at a time)
+  const int slen = (((T + ns - 1) / ns) + 127) & ~127;
+  const int jb = min(T, sl * slen), je = min(T, jb + slen);
   const int n0 = new_off[req], nn = new_off[req + 1] - n0;
   const int words = (T + 31) >> 5;
   int k = sel_off[req + 1] - sel_off[req];
@@ -121,31 +134,41 @@ select_kernel(int num_kv_heads, int total_tokens, const int32_t *__restrict__ se
   // ---- radix select: bit pattern of the k-th largest candidate score
   uint32_t prefix = 0, mask = 0;
   int remaining = k;
-  if (k > 0) {
-    for (int pass = 3; pass >= 0; --pass) {
-      const int shift = pass * 8;
-      for (int i = threadIdx.x; i < 256; i += kSelThreads) hist[i] = 0;
-      __syncthreads();
+  for (int pass = 3; pass >= 0; --pass) {  // (every CTA of the grid runs every pass: the grid syncs are collective)
+    const int shift = pass * 8;
+    for (int i = threadIdx.x; i < 256; i += kSelThreads) hist[i] = 0;
+    __syncthreads();
+    if (k > 0) {
       // all 32 lanes stay in the loop (warp-aggregated histogram: the top digits of the scores take few
       // distinct values, a plain shared-memory atomic per lane would serialise 32-fold)
-      for (int j0 = 0; j0 < T; j0 += 8 * kSelThreads) {
+      for (int j0 = jb; j0 < je; j0 += 8 * kSelThreads) {
         uint32_t u[8];  // eight independent loads in flight per thread: the pass is bound by load latency
 #pragma unroll
         for (int q = 0; q < 8; ++q) {
           const int j = j0 + q * kSelThreads + threadIdx.x;
-          u[q] = j < T ? __float_as_uint(scores[off + j]) : 0u;
+          u[q] = j < je ? __float_as_uint(scores[off + j]) : 0u;
         }
 #pragma unroll
         for (int q = 0; q < 8; ++q) {
           const int j = j0 + q * kSelThreads + threadIdx.x;
           int bin = -1;
-          if (j < T && !((is_new[j >> 5] >> (j & 31)) & 1u) && (u[q] & mask) == prefix)
+          if (j < je && !((is_new[j >> 5] >> (j & 31)) & 1u) && (u[q] & mask) == prefix)
             bin = (int)((u[q] >> shift) & 255u);
           const unsigned peers = __match_any_sync(0xffffffffu, bin);
           if (bin >= 0 && (threadIdx.x & 31) == __ffs(peers) - 1) atomicAdd(&hist[bin], __popc(peers));
         }
       }
+    }
+    __syncthreads();
+    if (ns > 1) {  // add up the slices of the request (integer atomics: order does not matter), then read the sum
+      for (int i = threadIdx.x; i < 256; i += kSelThreads)
+        if (hist[i]) atomicAdd(&ghist[pass * 256 + i], hist[i]);
+      __threadfence();
+      cg::this_grid().sync();
+      for (int i = threadIdx.x; i < 256; i += kSelThreads) hist[i] = __ldcg(&ghist[pass * 256 + i]);
       __syncthreads();
+    }
+    if (k > 0) {
       if (threadIdx.x < 32) {
         // bins from high to low; lane l owns bins [255-8l-7, 255-8l]
         const int lane = threadIdx.x;
@@ -178,8 +201,8 @@ select_kernel(int num_kv_heads, int total_tokens, const int32_t *__restrict__ se
       prefix = sh_prefix;
       remaining = sh_remaining;
       mask |= 255u << shift;
-      __syncthreads();
     }
+    __syncthreads();
   }
   // prefix = threshold pattern; `remaining` = how many candidates equal to it are taken (lowest positions)
   const uint32_t thr = prefix;
@@ -193,8 +216,26 @@ select_kernel(int num_kv_heads, int total_tokens, const int32_t *__restrict__ se
   const int so = sel_off[req], ro = rows_off[req], cap_r = rows_off[req + 1] - ro;
   const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
   const unsigned lt = (1u << lane) - 1u;
-  const int seg = (((T + kSelWarps - 1) / kSelWarps) + 127) & ~127;  // positions per warp, multiple of 32 * kB
-  const int j_lo = w * seg, j_hi = min(T, j_lo + seg);
+  const int seg = ((((je - jb) + kSelWarps - 1) / kSelWarps) + 127) & ~127;  // positions per warp, multiple of 32 * kB
+  const int j_lo = min(je, jb + w * seg), j_hi = min(je, j_lo + seg);
+  // counter c of the slices before this one (slice totals meet in gcnt[c][slice]); the grid sync is collective
+  auto slice_base = [&](int c, int mine_total, int *all_total) -> int {
+    if (ns == 1) {
+      if (all_total) *all_total = mine_total;
+      return 0;
+    }
+    if (threadIdx.x == 0) gcnt[c * 64 + sl] = mine_total;
+    __threadfence();
+    cg::this_grid().sync();
+    int b0 = 0, all = 0;
+    for (int i = 0; i < ns; ++i) {
+      const int v = __ldcg(&gcnt[c * 64 + i]);
+      if (i < sl) b0 += v;
+      all += v;
+    }
+    if (all_total) *all_total = all;
+    return b0;
+  };
   constexpr int kB = 4;  // groups of 32 positions whose score loads are issued together
   auto load4 = [&](int j0, uint32_t (&u)[kB]) {
 #pragma unroll
@@ -245,7 +286,9 @@ select_kernel(int num_kv_heads, int total_tokens, const int32_t *__restrict__ se
       n_eq += __popc(__ballot_sync(0xffffffffu, eq));
     }
   }
-  const int eq_base = warp_base(n_eq, nullptr);
+  int cta_eq = 0;
+  int eq_base = warp_base(n_eq, &cta_eq);
+  eq_base += slice_base(0, cta_eq, nullptr);
   int n_sel = 0, n_r = 0, run_eq = eq_base;
   for (int j0 = j_lo; j0 < j_hi; j0 += 32 * kB) {
     load4(j0, ub);
@@ -259,9 +302,13 @@ select_kernel(int num_kv_heads, int total_tokens, const int32_t *__restrict__ se
       n_r += __popc(__ballot_sync(0xffffffffu, sel || isn || frc));  // R = I_nr U S_key U S_ov U S_tail
     }
   }
-  const int sel_base = warp_base(n_sel, nullptr);
-  int total_r = 0;
-  const int r_base = warp_base(n_r, &total_r);
+  int cta_sel = 0, cta_r = 0, total_r = 0;
+  int sel_base = warp_base(n_sel, &cta_sel);
+  int r_base = warp_base(n_r, &cta_r);
+  if (ns > 1 && threadIdx.x == 0) gcnt[1 * 64 + sl] = cta_sel;  // rides on the grid sync of the next call
+  r_base += slice_base(2, cta_r, &total_r);
+  if (ns > 1)
+    for (int i = 0; i < sl; ++i) sel_base += __ldcg(&gcnt[1 * 64 + i]);
   int run_sel = sel_base, run_r = r_base;
   run_eq = eq_base;
   for (int j0 = j_lo; j0 < j_hi; j0 += 32 * kB) {
@@ -282,7 +329,7 @@ select_kernel(int num_kv_heads, int total_tokens, const int32_t *__restrict__ se
       run_r += __popc(br);
     }
   }
-  if (rows_cnt && threadIdx.x == 0) rows_cnt[req] = min(total_r, cap_r);
+  if (rows_cnt && threadIdx.x == 0 && sl == 0) rows_cnt[req] = min(total_r, cap_r);
 }
 
 // Extended selection only: per-request row lists sit in capacity-sized slots of `tmp`; pack them into one
@@ -300,9 +347,11 @@ compact_rows_kernel(int num_reqs, const int32_t *__restrict__ cap_off, const int
   if (threadIdx.x == 0) rows_off_out[num_reqs] = out;
 }
 
+size_t select_scratch_bytes(const sx_batch *b) { return sizeof(int) * (size_t)b->num_reqs * (4 * 256 + 4 * 64); }
+
 sx_status launch_select(const sx_pool *pool, const sx_batch *b, const float *partial, const int32_t *sel_off,
                         const int32_t *rows_off, float *scores, int32_t *sel_idx, int32_t *rows_R, int ov_blocks,
-                        int tail_tokens, int32_t *rows_tmp, int32_t *rows_cnt, int32_t *rows_off_out,
+                        int tail_tokens, int32_t *rows_tmp, int32_t *rows_cnt, int32_t *rows_off_out, int *scratch,
                         cudaStream_t st) {
   size_t smem = 2 * sizeof(uint32_t) * (size_t)((b->max_seq_len + 31) / 32);
   if (smem > 200 * 1024) return set_error(SX_ERR_UNSUPPORTED, "max_seq_len %d too large for the select bitmaps", b->max_seq_len);
@@ -314,10 +363,33 @@ sx_status launch_select(const sx_pool *pool, const sx_batch *b, const float *par
   sx_status s0 = check_launch("score_sum_kernel");
   if (s0 != SX_OK) return s0;
   const bool ex = rows_off_out != nullptr;  // extended: variable |R|, slots of capacity rows_off, then compaction
-  select_kernel<<<b->num_reqs, kSelThreads, smem, st>>>(
-      pool->num_kv_heads, b->total_tokens, b->seq_len, b->tok_off, b->new_off, b->new_idx, partial, sel_off, rows_off,
-      scores, sel_idx, ex ? rows_tmp : rows_R, ov_blocks * kPage, tail_tokens, b->segments, b->num_segments,
-      ex ? rows_cnt : nullptr);
+  // Long requests: several CTAs per request (cooperative launch: every CTA must be resident, one per SM).
+  int ns = 1;
+  if (b->max_seq_len >= 4096 && b->num_reqs <= 74) {
+    ns = (b->max_seq_len + 4095) / 4096;
+    if (ns > 148 / b->num_reqs) ns = 148 / b->num_reqs;
+    if (ns > 32) ns = 32;
+  }
+  int num_kv = pool->num_kv_heads, total_tokens = b->total_tokens, ov_tokens = ov_blocks * kPage, nseg = b->num_segments;
+  const int32_t *seq_len = b->seq_len, *tok_off = b->tok_off, *new_off = b->new_off, *new_idx = b->new_idx;
+  int32_t *rows_dst = ex ? rows_tmp : rows_R, *cnt = ex ? rows_cnt : nullptr;
+  const sx_segment *segs = b->segments;
+  if (ns > 1) {
+    cudaError_t e = cudaMemsetAsync(scratch, 0, select_scratch_bytes(b), st);
+    if (e != cudaSuccess) return set_error(SX_ERR_CUDA, "select scratch memset: %s", cudaGetErrorString(e));
+    void *args[] = {&num_kv, &total_tokens, &seq_len, &tok_off, &new_off, &new_idx, &partial, &sel_off, &rows_off,
+                    &scores, &sel_idx, &rows_dst, &ov_tokens, &tail_tokens, &segs, &nseg, &cnt, &scratch};
+    e = cudaLaunchCooperativeKernel(reinterpret_cast<void *>(select_kernel), dim3(b->num_reqs, ns), dim3(kSelThreads),
+                                    args, smem, st);
+    if (e != cudaSuccess) {
+      cudaGetLastError();
+      ns = 1;  // cooperative launch not possible here (e.g. too few free SMs): one CTA per request
+    }
+  }
+  if (ns == 1)
+    select_kernel<<<dim3(b->num_reqs, 1), kSelThreads, smem, st>>>(num_kv, total_tokens, seq_len, tok_off, new_off,
+                                                                  new_idx, partial, sel_off, rows_off, scores, sel_idx,
+                                                                  rows_dst, ov_tokens, tail_tokens, segs, nseg, cnt, scratch);
   sx_status s = check_launch("select_kernel");
   if (s != SX_OK || !ex) return s;
   compact_rows_kernel<<<1, kSelThreads, 0, st>>>(b->num_reqs, rows_off, rows_cnt, rows_tmp, rows_R, rows_off_out);
