@@ -251,9 +251,10 @@ def test_degenerate_budgets():
             assert np.array_equal(dev_to_bits(g.pool_k)[kt[kt >= 0]], pk[kt[kt >= 0]])
 
 
-def test_determinism():
+@pytest.mark.parametrize("name", ["C2-quarter", "C5-1/16"])   # the second one takes the multi-CTA select
+def test_determinism(name):
     GpuLayer, dev_to_bits = _gpu()
-    lay, lt = prepared("C2-quarter")[:2]
+    lay, lt = prepared(name)[:2]
     outs = []
     for _ in range(2):
         g = GpuLayer(lay, lt)
