@@ -80,3 +80,24 @@ def test_layer_tensors_seeded_and_salient():
     kf = np.linalg.norm(wl.bf16_bits_to_f32(a.k_fresh).reshape(len(m), -1), axis=1)
     assert abs(kf[m].mean() / kf[~m].mean() - 4) < 0.3
     assert not m[lay.is_new_mask(0)].any()
+
+
+def test_tail_layout_and_row_capacity():
+    """config_tail ends two requests inside a reused segment; the capacity offsets handed to sx_score_select_ex
+    must cover R = I_nr U S_key U S_ov U S_tail for ANY S_key of size k (checked with the oracle's set builder)."""
+    import pytest
+    torch = pytest.importorskip("torch")  # noqa: F841  (binding imports torch)
+    from oracle import sx_oracle as orc
+    from paper_2606_01751_b200 import binding as sx
+    lay = wl.config_tail()
+    assert not lay.is_new_mask(0)[-1] and not lay.is_new_mask(1)[-1] and lay.is_new_mask(2)[-1]
+    for ov, tail in [(1, 64), (2, 16), (0, 0)]:
+        cap = sx.rows_capacity(lay, ov, tail)
+        for r in range(lay.num_reqs):
+            is_new = lay.is_new_mask(r)
+            cand = np.nonzero(~is_new)[0]
+            k = int(lay.k_per_req[r])
+            segr = [(int(n), int(n + ln)) for (rq, ln, _, n, _) in lay.segments.tolist() if rq == r]
+            for sel in (cand[:k], cand[-k:] if k else cand[:0]):
+                rows = orc.recompute_set(is_new, sel, segr, ov, tail)
+                assert len(rows) <= cap[r + 1] - cap[r]
