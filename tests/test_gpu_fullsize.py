@@ -58,11 +58,14 @@ def _check_keys(name, lay, lt, gk, pk, kt, kref):
     assert np.array_equal(gk[untouched], lt.pool_k[untouched]), name
 
 
-@pytest.mark.parametrize("name", ["C2", "C4", "C5"])
+@pytest.mark.parametrize("name", ["C2", "C4", "C4-cow", "C5"])
 def test_fullsize_sparse_layer(name):
-    """One sparse-mode layer with its own two-sweep selection (what bench.py --config <name> times)."""
+    """One sparse-mode layer with its own two-sweep selection (what bench.py --config <name> times).
+    C4-cow: the copy-on-write variant of C4 (V pages alias the shared source pages until a row is written,
+    reading A14); keys, scores and index sets are those of C4, so the same carve log applies."""
     GpuLayer, dev_to_bits = _gpu()
-    lay = wl.CONFIGS[name]()
+    lay = wl.config_c4(cow=True) if name == "C4-cow" else wl.CONFIGS[name]()
+    name = name.split("-")[0]
     lt = wl.build_layer(lay, 0)
     apply_carve(lt, load_carve(os.path.join(GOLD, "carve_%s.txt" % name)))
     hq = lay.num_q_heads
