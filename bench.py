@@ -37,6 +37,7 @@ from paper_2606_01751_b200 import workloads as wl  # noqa: E402
 
 METRIC = "sparse_recompute_context_tokens_per_s"
 UNIT = "tokens/s"
+CTA_PAIR = False  # --cta-pair: stage (c) runs with the SX_ATTN_CTA_PAIR flag
 L_STACK, THRESHOLD = 32, 4
 
 
@@ -198,7 +199,7 @@ def measure(cfg, steps, warmup, ctx, want_e2e=True, want_clocks=True):
         timed("scatter", lambda: sx.scatter_kv(gl.pool, batch, gl.k_fresh, gl.v_fresh, all_rows, batch.tok_off,
                                                max_rows=T))
         timed("attn_full", lambda: sx.sparse_attn(gl.pool, batch, gl.q_full, gl.out, total_rows=T, lse=gl.lse,
-                                                  full=True))
+                                                  full=True, cta_pair=CTA_PAIR))
         if select_after:
             timed("select", lambda: sx.score_select(gl.pool, batch, gl.q_new, gl.sel_off, gl.rows_off,
                                                     sel_holder["sel"], sel_holder["rows"], lse_new=gl.lse,
@@ -220,7 +221,8 @@ def measure(cfg, steps, warmup, ctx, want_e2e=True, want_clocks=True):
             timed("scatter", lambda: sx.scatter_kv(gl.pool, batch, gl.kf_R, gl.vf_R, sel_holder["rows"], gl.rows_off,
                                                    max_rows=n_rows))
         timed("attn_sparse", lambda: sx.sparse_attn(gl.pool, batch, gl.q_R, gl.out, rows_R=sel_holder["rows"],
-                                                    rows_off=gl.rows_off, total_rows=n_rows, lse=gl.lse))
+                                                    rows_off=gl.rows_off, total_rows=n_rows, lse=gl.lse,
+                                                    cta_pair=CTA_PAIR))
 
     # ---- untimed pass: fixes R (deterministic) and stages the compact per-row inputs of Alg. 1 l.544
     g0 = layers[0]
@@ -306,7 +308,7 @@ def measure(cfg, steps, warmup, ctx, want_e2e=True, want_clocks=True):
     # a kernel timed alone between L2 flushes (single-layer configs) is held against the burst peak, the
     # attention launches inside the long C3 step against the sustained one (B200_PROFILING.md)
     tf_peak, tf_src = (peaks["tf_sustained"], "sustained") if stack else (peaks["tf_burst"], "burst")
-    roofline = {"bound": "tensor", "kernel": "attn_kernel<true> (sx_sparse_attn)", "achieved": round(achieved, 1),
+    roofline = {"bound": "tensor", "kernel": "attn_kernel<true%s> (sx_sparse_attn)" % (", cta pair" if CTA_PAIR else ""), "achieved": round(achieved, 1),
                 "peak": tf_peak, "unit": "TFLOP/s", "frac": round(achieved / tf_peak, 4),
                 "peak_src": "%s bf16 %s" % (peaks["src"], tf_src),
                 # dram__bytes_read + dram__bytes_write per attention launch, averaged over the 32 launches of a C3 step
@@ -531,7 +533,8 @@ def run_e2e(torch, sx, du, lay, layers, batch, all_rows, sel_holder, stack, args
                 sx.rope_realign(gl.pool, batch)
             if gl.is_full:
                 sx.scatter_kv(gl.pool, batch, gl.k_fresh, gl.v_fresh, all_rows, batch.tok_off, max_rows=T)
-                sx.sparse_attn(gl.pool, batch, gl.q_full, gl.out, total_rows=T, lse=gl.lse, full=True)
+                sx.sparse_attn(gl.pool, batch, gl.q_full, gl.out, total_rows=T, lse=gl.lse, full=True,
+                               cta_pair=CTA_PAIR)
                 if l == THRESHOLD - 1:
                     sx.score_select(gl.pool, batch, gl.q_new, gl.sel_off, gl.rows_off, sel_holder["sel"],
                                     sel_holder["rows"], lse_new=gl.lse, lse_by_token=True)
@@ -548,7 +551,7 @@ def run_e2e(torch, sx, du, lay, layers, batch, all_rows, sel_holder, stack, args
                         sx.scatter_kv(gl.pool, batch, gl.kf_sel, gl.vf_sel, sel_holder["sel"], gl.sel_off,
                                       max_rows=int(sel_holder["sel"].numel()))
                 sx.sparse_attn(gl.pool, batch, gl.q_R, gl.out, rows_R=sel_holder["rows"], rows_off=gl.rows_off,
-                               total_rows=n_rows, lse=gl.lse)
+                               total_rows=n_rows, lse=gl.lse, cta_pair=CTA_PAIR)
             ev_done[l].record(main)
             with torch.cuda.stream(s_out):
                 s_out.wait_event(ev_done[l])
@@ -691,7 +694,11 @@ def main():
     ap.add_argument("--cpu-seconds", type=float, default=20.0)
     ap.add_argument("--no-cpu", action="store_true")
     ap.add_argument("--no-others", action="store_true", help="skip the short runs of the other BASELINE configs")
+    ap.add_argument("--cta-pair", action="store_true",
+                    help="stage (c) with SX_ATTN_CTA_PAIR (2-CTA clusters, tcgen05.mma.cta_group::2)")
     args = ap.parse_args()
+    global CTA_PAIR
+    CTA_PAIR = args.cta_pair
     if args.impl == "reference":
         run_reference(args)
     else:

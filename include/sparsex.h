@@ -174,6 +174,7 @@ sx_status sx_score_select_ex(const sx_pool *pool, const sx_batch *batch, const v
                              size_t ws_bytes, sx_stream stream);
 
 #define SX_ATTN_CUDA_CORE 2 /* flag for sx_sparse_attn's mode: CUDA-core kernels for small row sets */
+#define SX_ATTN_CTA_PAIR 4  /* flag for sx_sparse_attn's mode: 2-CTA clusters with tcgen05.mma.cta_group::2 */
 
 /* (c) Alg. 1 l.546-548 (sparse) / l.507-511 (full). mode 0: query rows are rows_R (as produced by
  * sx_score_select); mode 1: rows_R and rows_off are ignored, every position of every request is
@@ -190,7 +191,12 @@ sx_status sx_score_select_ex(const sx_pool *pool, const sx_batch *batch, const v
  *   - mode | SX_ATTN_CUDA_CORE: row sets with total_rows * g < 64 * num_reqs (fewer than 64 query rows per
  *     KV head on average; g = Hq/Hkv <= 32) take CUDA-core split-KV kernels, fp32 FMA throughout (the rule of
  *     BASELINE.json north_star; measured slower than the padded tensor-core tile on B200). Uses ws.
- * Both are deterministic and meet the same tolerance against fp64. */
+ *   - mode | SX_ATTN_CTA_PAIR: when the tensor-core path runs without key splits, clusters of two CTAs work on
+ *     adjacent pairs of query tiles with M = 256 MMAs (tcgen05.mma.cta_group::2): every K/V tile is fetched once
+ *     per cluster, half into each CTA. Same arithmetic per row, hence the same results as the default; measured
+ *     0.3-0.5 % faster on the power-capped 32-layer stack and 1-7 % slower on single layers (S10), so
+ *     it is opt-in. Ignored where key splits or the CUDA-core kernels apply.
+ * All are deterministic and meet the same tolerance against fp64. */
 sx_status sx_sparse_attn(const sx_pool *pool, const sx_batch *batch, int32_t mode, const void *q,
                          const int32_t *rows_R, const int32_t *rows_off, int32_t total_rows,
                          void *out, float *lse, void *ws, size_t ws_bytes, sx_stream stream);

@@ -232,7 +232,7 @@ sx_status sx_score_select_ex(const sx_pool *pool, const sx_batch *batch, const v
       float *lse_ws = reinterpret_cast<float *>(base + w.lse_new);
       lse_splits = attn_lse_splits(pool, batch, batch->total_new);
       st = launch_attn(pool, batch, /*with_pv=*/false, q_new, batch->new_idx, batch->new_off, batch->total_new,
-                       nullptr, lse_ws, lse_splits, nullptr, s);
+                       nullptr, lse_ws, lse_splits, nullptr, /*cta_pair=*/false, s);
       if (st != SX_OK) return st;
       lse = lse_ws;
       lse_by_token = 0;
@@ -263,8 +263,10 @@ sx_status sx_sparse_attn(const sx_pool *pool, const sx_batch *batch, int32_t mod
                          void *ws, size_t ws_bytes, sx_stream stream) {
   sx_status st = validate(pool, batch);
   if (st != SX_OK) return st;
-  if (mode < 0 || mode > 3) return set_error(SX_ERR_INVALID_ARG, "mode must be 0 (sparse rows) or 1 (full), optionally | 2");
-  const bool want_cuda_core = (mode & 2) != 0;  // SX_ATTN_CUDA_CORE
+  if (mode < 0 || mode > 7)
+    return set_error(SX_ERR_INVALID_ARG, "mode must be 0 (sparse rows) or 1 (full), optionally | SX_ATTN_* flags");
+  const bool want_cuda_core = (mode & SX_ATTN_CUDA_CORE) != 0;
+  const bool want_cta_pair = (mode & SX_ATTN_CTA_PAIR) != 0;
   mode &= 1;
   if (total_rows < 0) return set_error(SX_ERR_INVALID_ARG, "total_rows < 0");
   if (total_rows == 0) return SX_OK;
@@ -300,7 +302,7 @@ sx_status sx_sparse_attn(const sx_pool *pool, const sx_batch *batch, int32_t mod
     if (st != SX_OK) return st;
     part = reinterpret_cast<float *>(static_cast<char *>(ws) + ws_layout(pool, batch).attn_part);
   }
-  return launch_attn(pool, batch, true, q, rows_R, rows_off, total_rows, out, lse, splits, part, s);
+  return launch_attn(pool, batch, true, q, rows_R, rows_off, total_rows, out, lse, splits, part, want_cta_pair, s);
 }
 
 }  // extern "C"

@@ -33,7 +33,8 @@ namespace sx {
 constexpr int kAttnThreads = 384;
 constexpr int kTileBytes = kTile * kHeadDim * 2;  // 32 KB: two 16-KB halves [half][row][64 bf16]
 constexpr int kHalfBytes = kTileBytes / 2;
-constexpr int kKvStages = 5;
+constexpr int kKvStages = 5;      // ring slots of one CTA (32 KB each)
+constexpr int kKvStagesPair = 8;  // CTA-pair variant: each CTA stages half of every K/V tile (16 KB slots)
 #ifndef SX_ATTN_POLY
 #define SX_ATTN_POLY 2  // of every 8 pairs of exponentials, this many pairs go to the FMA pipe (0..8)
 #endif
@@ -64,11 +65,12 @@ struct AttnCfg {
 
 struct AttnBars {
   uint64_t q_full;
-  uint64_t kv_full[kKvStages], kv_empty[kKvStages];
+  uint64_t kv_full[kKvStagesPair], kv_empty[kKvStagesPair];
   uint64_t s_full[2][2];  // [query tile][buffer]: S = Q K^T landed in TMEM   (buffer 1: LSE-only variant)
   uint64_t s_free[2][2];  // softmax -> MMA: P written (PV variant) / S consumed (LSE-only); 128 arrivals
   uint64_t p_half[2];     // softmax -> MMA: keys [0, 64) of P written (PV variant); 128 arrivals
   uint64_t o_full[2];     // last PV of the query tile completed
+  uint64_t v_landed;      // CTA-pair variant: the V tile that holds keys >= T is in shared memory (both CTAs)
   uint32_t tmem_base;
 };
 
@@ -90,52 +92,74 @@ __device__ __forceinline__ float2 ex2_poly2(float2 x) {
   return r;
 }
 
-template <bool kWithPV>
+// kPair (PV variant without key splits): a cluster of two CTAs works on two ADJACENT pairs of query tiles of one
+// (request, KV head) with tcgen05.mma.cta_group::2 (M = 256): every K/V tile is fetched once per cluster, each
+// CTA staging half of it (K: 64 of the 128 keys; V: 64 of the 128 dims), so L2 -> SM traffic and the
+// shared-memory operand reads of B are halved. CTA rank 0 issues all MMAs; both CTAs run the softmax of their own
+// rows over the cluster's common number of key tiles (rows with fewer visible keys see fully masked tiles).
+template <bool kWithPV, bool kPair>
 __global__ void __launch_bounds__(kAttnThreads, 1)
 attn_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_constant__ CUtensorMap tm_k,
             const __grid_constant__ CUtensorMap tm_v, const AttnParams p) {
+  static_assert(kWithPV || !kPair, "the CTA-pair variant exists for the PV kernel only");
   using Cfg = AttnCfg;
+  constexpr int kStages = kPair ? kKvStagesPair : kKvStages;
+  constexpr int kStageBytes = kPair ? kHalfBytes : kTileBytes;  // bytes of one ring item in THIS CTA
   extern __shared__ uint8_t smem_raw[];
   uint8_t *smem = reinterpret_cast<uint8_t *>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~uintptr_t(1023));
   AttnBars *bars = reinterpret_cast<AttnBars *>(smem + Cfg::kOffBar);
 
   // ---- which (request, KV head, pair of row tiles) is this CTA; heavy (late) pairs of a request first
   const int g = p.group, rpt = p.rows_per_tile, rpc = 2 * rpt;
+  const int rank = kPair ? (int)cluster_ctarank() : 0;
   // consecutive blocks share a (request, KV head, row pair) and take one key split each
-  const int split = (int)blockIdx.x % p.kv_splits;
-  const int bid = (int)blockIdx.x / p.kv_splits;
-  int req = 0, base = 0, pairs = 0, n_r = 0;
+  // (kPair: consecutive blocks are the two CTAs of a cluster and take adjacent row pairs)
+  const int split = kPair ? 0 : (int)blockIdx.x % p.kv_splits;
+  const int bid = kPair ? (int)blockIdx.x >> 1 : (int)blockIdx.x / p.kv_splits;
+  int req = 0, base = 0, pairs = 0, n_r = 0, units = 0;
   for (; req < p.num_reqs; ++req) {
     n_r = p.rows_off[req + 1] - p.rows_off[req];
     pairs = (n_r + rpc - 1) / rpc;
-    if (bid < base + pairs * p.num_kv_heads) break;
-    base += pairs * p.num_kv_heads;
+    units = kPair ? (pairs + 1) / 2 : pairs;
+    if (bid < base + units * p.num_kv_heads) break;
+    base += units * p.num_kv_heads;
   }
-  if (req >= p.num_reqs) return;
+  if (req >= p.num_reqs) return;  // (both CTAs of a cluster leave together)
   const int local = bid - base;
   const int kvh = local % p.num_kv_heads;
-  const int pair = pairs - 1 - local / p.num_kv_heads;
-  const int row_base = p.rows_off[req] + pair * rpc;  // first row (batch-wide index) of query tile 0
-  const int nrows_cta = min(rpc, n_r - pair * rpc);   // valid rows of R in this CTA (>= 1)
+  // kPair: rank 0 takes the later pair; with an odd number of pairs the last cluster's rank 1 has no rows
+  // (pair = -1) and only stages its halves of K/V and runs masked softmax tiles
+  const int pair = kPair ? pairs - 1 - (2 * (local / p.num_kv_heads) + rank) : pairs - 1 - local / p.num_kv_heads;
+  const int row_base = pair >= 0 ? p.rows_off[req] + pair * rpc : p.total_rows;  // first row of query tile 0
   const int T = p.seq_len[req];
   const int n_pages = (T + kPage - 1) / kPage;
-  // valid rows and number of key tiles of each query tile
-  int nrows[2], n_t[2];
-  nrows[0] = min(rpt, nrows_cta);
-  nrows[1] = nrows_cta - nrows[0];
+  // valid rows and number of key tiles of each query tile of row pair `pr`
+  auto tile_info = [&](int pr, int (&nr)[2], int (&nt)[2]) {
+    const int cta_rows = pr >= 0 ? min(rpc, n_r - pr * rpc) : 0;
+    nr[0] = min(rpt, cta_rows);
+    nr[1] = cta_rows - nr[0];
 #pragma unroll
-  for (int i = 0; i < 2; ++i) {
-    if (nrows[i] > 0) {
-      const int last = row_base + i * rpt + nrows[i] - 1;
-      const int pos_max = p.rows ? p.rows[last] : last - p.rows_off[req];
-      n_t[i] = pos_max / kTile + 1;
-    } else {
-      n_t[i] = 0;
+    for (int i = 0; i < 2; ++i) {
+      if (nr[i] > 0) {
+        const int last = p.rows_off[req] + pr * rpc + i * rpt + nr[i] - 1;
+        const int pos_max = p.rows ? p.rows[last] : last - p.rows_off[req];
+        nt[i] = pos_max / kTile + 1;
+      } else {
+        nt[i] = 0;
+      }
     }
+  };
+  int nrows[2], n_t[2];
+  tile_info(pair, nrows, n_t);
+  if (kPair) {  // the cluster's common tile counts (rank 0 holds the later rows, but tile i of either may lead)
+    int nr_o[2], nt_o[2];
+    tile_info(pair + (rank ? 1 : -1), nr_o, nt_o);
+    n_t[0] = max(n_t[0], nt_o[0]);
+    n_t[1] = max(n_t[1], nt_o[1]);
   }
   // key tiles [t0, t0 + n_tiles) of this CTA; n_t[i] and every loop below count tiles from t0
   int t0 = 0;
-  if (p.kv_splits > 1) {
+  if (!kPair && p.kv_splits > 1) {
     const int all = max(n_t[0], n_t[1]);
     const int per = (all + p.kv_splits - 1) / p.kv_splits;
     t0 = split * per;
@@ -156,23 +180,30 @@ attn_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_constant__ CU
     tma_prefetch_desc(&tm_k);
     if (kWithPV) tma_prefetch_desc(&tm_v);
     mbar_init(&bars->q_full, 1);
-    for (int i = 0; i < kKvStages; ++i) {
+    for (int i = 0; i < kStages; ++i) {
       mbar_init(&bars->kv_full[i], 1);
       mbar_init(&bars->kv_empty[i], 1);
     }
+    // kPair: the softmax threads of BOTH CTAs arrive on rank 0's p_half / s_free
     for (int i = 0; i < 2; ++i) {
       for (int b = 0; b < 2; ++b) {
         mbar_init(&bars->s_full[i][b], 1);
-        mbar_init(&bars->s_free[i][b], 128);
+        mbar_init(&bars->s_free[i][b], kPair ? 8 : 128);
       }
       mbar_init(&bars->o_full[i], 1);
-      mbar_init(&bars->p_half[i], 128);
+      mbar_init(&bars->p_half[i], kPair ? 8 : 128);
     }
+    mbar_init(&bars->v_landed, 1);
     fence_mbar_init();
   }
   if (warp == kWarpMma) {
-    tmem_alloc(&bars->tmem_base, 512);
-    tmem_relinquish();
+    if (kPair) {
+      tmem_alloc_pair(&bars->tmem_base, 512);
+      tmem_relinquish_pair();
+    } else {
+      tmem_alloc(&bars->tmem_base, 512);
+      tmem_relinquish();
+    }
   }
   // rows of the query tiles that the TMA box never writes (128 - rpt*g of them when g does not divide 128)
   if (rpt * g < kTile && warp < 8) {
@@ -185,7 +216,7 @@ attn_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_constant__ CU
     fence_proxy_async_smem();
   }
   tc_fence_before();
-  __syncthreads();
+  if (kPair) cluster_sync(); else __syncthreads();
   tc_fence_after();
   const uint32_t tmem = bars->tmem_base;
 
@@ -196,35 +227,60 @@ attn_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_constant__ CU
       // warp 0 loads Q and the even ring items, warp 2 the odd ones (PV variant: K tiles / V tiles);
       // the block-table entries of a warp's next item are fetched before it waits for the free slot.
       if (warp == kWarpProd0 && lane == 0) {
-        const int nq = nrows[1] > 0 ? 2 : 1;
-        mbar_expect_tx(&bars->q_full, (uint32_t)(nq * 2 * rpt * g * 128));
-        for (int i = 0; i < nq; ++i) {
-          tma_load_3d(smem + Cfg::kOffQ + i * kTileBytes, &tm_q, &bars->q_full, 0, kvh * g, row_base + i * rpt);
-          tma_load_3d(smem + Cfg::kOffQ + i * kTileBytes + kHalfBytes, &tm_q, &bars->q_full, 64, kvh * g,
-                      row_base + i * rpt);
+        if (kPair) {
+          // both CTAs always load both query tiles (rows past the batch read as zeros; rows of another request
+          // are never stored), so rank 0's barrier expects a fixed byte count
+          const uint32_t qbar = mapa_u32(smem_u32(&bars->q_full), 0);
+          if (rank == 0) mbar_expect_tx(&bars->q_full, (uint32_t)(2 * 2 * 2 * rpt * g * 128));
+          for (int i = 0; i < 2; ++i) {
+            tma_load_3d_pair(smem + Cfg::kOffQ + i * kTileBytes, &tm_q, qbar, 0, kvh * g, row_base + i * rpt);
+            tma_load_3d_pair(smem + Cfg::kOffQ + i * kTileBytes + kHalfBytes, &tm_q, qbar, 64, kvh * g,
+                             row_base + i * rpt);
+          }
+        } else {
+          const int nq = nrows[1] > 0 ? 2 : 1;
+          mbar_expect_tx(&bars->q_full, (uint32_t)(nq * 2 * rpt * g * 128));
+          for (int i = 0; i < nq; ++i) {
+            tma_load_3d(smem + Cfg::kOffQ + i * kTileBytes, &tm_q, &bars->q_full, 0, kvh * g, row_base + i * rpt);
+            tma_load_3d(smem + Cfg::kOffQ + i * kTileBytes + kHalfBytes, &tm_q, &bars->q_full, 64, kvh * g,
+                        row_base + i * rpt);
+          }
         }
       }
-      const int pg_in_tile = lane >> 1, half = lane & 1;
+      // single CTA: lane = (page of the tile, 64-column half), 16 boxes per item.
+      // kPair: 8 boxes per item: K item = this CTA's 64 keys (4 pages) x both halves -> [half][64 keys][128 B];
+      //        V item = all 8 pages x the CTA's own 64-column half -> [128 keys][128 B].
       const int n_items = kWithPV ? 2 * n_tiles : n_tiles;
+      const int pg_k = kPair ? 4 * rank + (lane >> 1) : (lane >> 1), half_k = lane & 1;
+      const int pg_v = kPair ? lane : (lane >> 1), half_v = kPair ? rank : (lane & 1);
+      const int n_boxes = kPair ? 8 : 16;
       auto table_entry = [&](int it) -> int {
         const int t = t0 + (kWithPV ? (it >> 1) : it);
         const bool is_v = kWithPV && (it & 1);
-        int lp = t * 8 + pg_in_tile;
+        int lp = t * 8 + (is_v ? pg_v : pg_k);
         if (lp > n_pages - 1) lp = n_pages - 1;  // pages past the sequence: any valid page (keys are masked)
         return (is_v ? p.v_table : p.k_table)[(size_t)req * p.max_pages + lp];
       };
+      const uint32_t full0 = kPair ? mapa_u32(smem_u32(&bars->kv_full[0]), 0) : 0;
       int it = (warp == kWarpProd1) ? 1 : 0;
-      int blk = it < n_items ? table_entry(it) : 0;
+      int blk = (it < n_items && lane < n_boxes) ? table_entry(it) : 0;
       for (; it < n_items; it += 2) {
-        const int blk_next = (it + 2 < n_items) ? table_entry(it + 2) : 0;
+        const int blk_next = (it + 2 < n_items && lane < n_boxes) ? table_entry(it + 2) : 0;
         const bool is_v = kWithPV && (it & 1);
-        const int s = it % kKvStages, u = it / kKvStages;
+        const int s = it % kStages, u = it / kStages;
         mbar_wait(&bars->kv_empty[s], (u & 1) ^ 1);
-        if (lane == 0) mbar_expect_tx(&bars->kv_full[s], kTileBytes);
+        if (lane == 0 && rank == 0) mbar_expect_tx(&bars->kv_full[s], kTileBytes);  // both CTAs' bytes
         __syncwarp();
-        if (lane < 16) {
-          tma_load_2d(smem + Cfg::kOffKV + s * kTileBytes + half * kHalfBytes + pg_in_tile * 2048,
-                      is_v ? &tm_v : &tm_k, &bars->kv_full[s], half * 64, (blk * p.num_kv_heads + kvh) * kPage);
+        if (lane < n_boxes) {
+          const int row0 = (blk * p.num_kv_heads + kvh) * kPage;
+          if (kPair) {
+            uint8_t *dst = smem + Cfg::kOffKV + s * kStageBytes +
+                           (is_v ? pg_v * 2048 : half_k * (kHalfBytes / 2) + (lane >> 1) * 2048);
+            tma_load_2d_pair(dst, is_v ? &tm_v : &tm_k, full0 + s * 8, (is_v ? half_v : half_k) * 64, row0);
+          } else {
+            tma_load_2d(smem + Cfg::kOffKV + s * kTileBytes + half_k * kHalfBytes + pg_k * 2048,
+                        is_v ? &tm_v : &tm_k, &bars->kv_full[s], half_k * 64, row0);
+          }
         }
         blk = blk_next;
       }
@@ -232,26 +288,35 @@ attn_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_constant__ CU
       // ================================================================ MMA issuer
       // One thread runs the whole issue loop (waits included): no per-instruction election, and the
       // descriptors are a base value plus small constants (the address field is (addr >> 4)).
-      if (elect_one()) {
-        constexpr uint32_t idesc_qk = umma_idesc_bf16(128, 128, 0, 0);
-        constexpr uint32_t idesc_pv = umma_idesc_bf16(128, 128, 0, 1);
-        constexpr uint32_t kSlotStep = kTileBytes >> 4;
+      if (rank == 0 && elect_one()) {
+        constexpr uint32_t idesc_qk = umma_idesc_bf16(kPair ? 256 : 128, 128, 0, 0);
+        constexpr uint32_t idesc_pv = umma_idesc_bf16(kPair ? 256 : 128, 128, 0, 1);
+        constexpr uint32_t kSlotStep = kStageBytes >> 4;
+        constexpr int kKHalf = kPair ? kHalfBytes / 2 : kHalfBytes;  // bytes between the two 64-column halves of K
         const uint64_t q_desc = umma_smem_desc(smem_u32(smem + Cfg::kOffQ), 16, 1024);
         const uint64_t k_desc = umma_smem_desc(smem_u32(smem + Cfg::kOffKV), 16, 1024);
         const uint64_t v_desc = umma_smem_desc(smem_u32(smem + Cfg::kOffKV), kHalfBytes, 1024);
         const uint32_t q_lo = (uint32_t)q_desc, k_lo = (uint32_t)k_desc, v_lo = (uint32_t)v_desc;
         const uint32_t qk_hi = (uint32_t)(k_desc >> 32), v_hi = (uint32_t)(v_desc >> 32);
+        auto commit = [&](uint64_t *bar) {
+          if (kPair) umma_commit_pair(bar); else umma_commit(bar);
+        };
+        auto wait_softmax = [&](uint64_t *bar, uint32_t parity) {  // kPair: arrivals come from both CTAs
+          if (kPair) mbar_wait_cluster(bar, parity); else mbar_wait(bar, parity);
+        };
         mbar_wait(&bars->q_full, 0);
         // S_i[buffer b] = Q_i K(slot)^T
         auto issue_qk = [&](int i, int b, int slot) {
-          const uint32_t qd = q_lo + (uint32_t)i * kSlotStep, kd = k_lo + (uint32_t)slot * kSlotStep;
+          const uint32_t qd = q_lo + (uint32_t)i * (kTileBytes >> 4), kd = k_lo + (uint32_t)slot * kSlotStep;
           const uint32_t d = tmem + (kWithPV ? i * 128 : (i * 2 + b) * 128);
 #pragma unroll
           for (int kk = 0; kk < 8; ++kk) {
-            const uint32_t o = ((kk >> 2) * kHalfBytes + (kk & 3) * 32) >> 4;
-            umma_ss2(d, qd + o, qk_hi, kd + o, qk_hi, idesc_qk, kk > 0);
+            const uint32_t oq = ((kk >> 2) * kHalfBytes + (kk & 3) * 32) >> 4;
+            const uint32_t ok = ((kk >> 2) * kKHalf + (kk & 3) * 32) >> 4;
+            if (kPair) umma_ss2_pair(d, qd + oq, qk_hi, kd + ok, qk_hi, idesc_qk, kk > 0);
+            else umma_ss2(d, qd + oq, qk_hi, kd + ok, qk_hi, idesc_qk, kk > 0);
           }
-          umma_commit(&bars->s_full[i][b]);
+          commit(&bars->s_full[i][b]);
         };
         if (kWithPV) {
           // ring item 2t+1 = V(t), 2t+2 = K(t+1): (slot, phase) advanced incrementally
@@ -261,36 +326,46 @@ attn_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_constant__ CU
             tc_fence_after();
             if (n_t[0] > 0) issue_qk(0, 0, 0);
             if (n_t[1] > 0) issue_qk(1, 0, 0);
-            umma_commit(&bars->kv_empty[0]);
+            commit(&bars->kv_empty[0]);
           }
           for (int t = 0; t < n_tiles; ++t) {
             const bool more = t + 1 < n_tiles;
             mbar_wait(&bars->kv_full[sv], phv);            // V(t)
+            if (kPair && (t0 + t + 1) * kTile > T) {
+              // the tile with keys >= T: the softmax threads of both CTAs zero those V rows before they arrive
+              mbar_arrive(&bars->v_landed);
+              mbar_arrive_cluster(mapa_u32(smem_u32(&bars->v_landed), 1));
+            }
             if (more) mbar_wait(&bars->kv_full[sk], phk);  // K(t+1)
             const uint32_t vd = v_lo + (uint32_t)sv * kSlotStep;
 #pragma unroll
             for (int i = 0; i < 2; ++i) {
               if (t < n_t[i]) {
                 const uint32_t d_o = tmem + 256 + i * 128, a_p = tmem + i * 128;
-                mbar_wait(&bars->p_half[i], t & 1);  // keys [0, 64) of P_i(t) are in TMEM
+                wait_softmax(&bars->p_half[i], t & 1);  // keys [0, 64) of P_i(t) are in TMEM
                 tc_fence_after();
 #pragma unroll
-                for (int kk = 0; kk < 4; ++kk)  // 16 keys per MMA: 8 TMEM columns of packed bf16 P
-                  umma_ts2(d_o, a_p + kk * 8, vd + kk * 128, v_hi, idesc_pv, (t > 0 || kk > 0));
-                mbar_wait(&bars->s_free[i][0], t & 1);  // all of P_i(t)
+                for (int kk = 0; kk < 4; ++kk) {  // 16 keys per MMA: 8 TMEM columns of packed bf16 P
+                  if (kPair) umma_ts2_pair(d_o, a_p + kk * 8, vd + kk * 128, v_hi, idesc_pv, (t > 0 || kk > 0));
+                  else umma_ts2(d_o, a_p + kk * 8, vd + kk * 128, v_hi, idesc_pv, (t > 0 || kk > 0));
+                }
+                wait_softmax(&bars->s_free[i][0], t & 1);  // all of P_i(t)
                 tc_fence_after();
 #pragma unroll
-                for (int kk = 4; kk < 8; ++kk) umma_ts2(d_o, a_p + kk * 8, vd + kk * 128, v_hi, idesc_pv, 1);
-                if (t == n_t[i] - 1) umma_commit(&bars->o_full[i]);
+                for (int kk = 4; kk < 8; ++kk) {
+                  if (kPair) umma_ts2_pair(d_o, a_p + kk * 8, vd + kk * 128, v_hi, idesc_pv, 1);
+                  else umma_ts2(d_o, a_p + kk * 8, vd + kk * 128, v_hi, idesc_pv, 1);
+                }
+                if (t == n_t[i] - 1) commit(&bars->o_full[i]);
                 if (t + 1 < n_t[i]) issue_qk(i, 0, sk);
               }
             }
-            umma_commit(&bars->kv_empty[sv]);
-            if (more) umma_commit(&bars->kv_empty[sk]);
+            commit(&bars->kv_empty[sv]);
+            if (more) commit(&bars->kv_empty[sk]);
             sv += 2;
-            if (sv >= kKvStages) { sv -= kKvStages; phv ^= 1; }
+            if (sv >= kStages) { sv -= kStages; phv ^= 1; }
             sk += 2;
-            if (sk >= kKvStages) { sk -= kKvStages; phk ^= 1; }
+            if (sk >= kStages) { sk -= kStages; phk ^= 1; }
           }
         } else {
           int slot = 0, ph = 0;
@@ -305,8 +380,8 @@ attn_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_constant__ CU
                 issue_qk(i, b, slot);
               }
             }
-            umma_commit(&bars->kv_empty[slot]);
-            if (++slot == kKvStages) { slot = 0; ph ^= 1; }
+            commit(&bars->kv_empty[slot]);
+            if (++slot == kStages) { slot = 0; ph ^= 1; }
           }
         }
       }
@@ -325,6 +400,9 @@ attn_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_constant__ CU
     const uint32_t tmem_s = tmem + lane_addr + (kWithPV ? qt * 128 : qt * 256);
     const uint32_t tmem_o = tmem + lane_addr + 256 + qt * 128;
     const int my_tiles = qt ? n_t[1] : n_t[0];
+    // kPair: P-ready arrivals go to rank 0's barriers (the issuer lives there)
+    const uint32_t p_half_r0 = kPair ? mapa_u32(smem_u32(&bars->p_half[qt]), 0) : 0;
+    const uint32_t s_free_r0 = kPair ? mapa_u32(smem_u32(&bars->s_free[qt][0]), 0) : 0;
     float m_used = -INFINITY, l = 0.f;
 
     for (int t = 0; t < my_tiles; ++t) {
@@ -389,15 +467,18 @@ attn_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_constant__ CU
 
       if (kWithPV && (t0 + t + 1) * kTile > T) {
         // V rows of keys beyond the sequence may hold anything (even NaN patterns): zero them
+        // (kPair: this CTA's V half completes on rank 0's barrier; rank 0's issuer passes the news on. Only the
+        // last tile of the sequence qualifies, so v_landed is used once.)
         const int it = 2 * t + 1;
-        mbar_wait(&bars->kv_full[it % kKvStages], (it / kKvStages) & 1);
+        if (kPair) mbar_wait_cluster(&bars->v_landed, 0);
+        else mbar_wait(&bars->kv_full[it % kStages], (it / kStages) & 1);
         if ((t0 + t) * kTile + row >= T) {
           const uint4 z = make_uint4(0, 0, 0, 0);
-          uint8_t *v0 = smem + Cfg::kOffKV + (it % kKvStages) * kTileBytes + row * 128;
+          uint8_t *v0 = smem + Cfg::kOffKV + (it % kStages) * kStageBytes + row * 128;
 #pragma unroll
           for (int i = 0; i < 8; ++i) {
             *reinterpret_cast<uint4 *>(v0 + i * 16) = z;
-            *reinterpret_cast<uint4 *>(v0 + kHalfBytes + i * 16) = z;
+            if (!kPair) *reinterpret_cast<uint4 *>(v0 + kHalfBytes + i * 16) = z;
           }
         }
         fence_proxy_async_smem();
@@ -430,7 +511,12 @@ attn_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_constant__ CU
           tmem_st32(tmem_s + h * 32, *reinterpret_cast<uint32_t(*)[32]>(&pk[0]));
           tmem_wait_st();
           tc_fence_before();
-          mbar_arrive(h == 0 ? &bars->p_half[qt] : &bars->s_free[qt][0]);
+          if (kPair) {  // one arrival per warp: 8 (4 of them remote) instead of 256 per hand-off
+            __syncwarp();
+            if (lane == 0) mbar_arrive_cluster(h == 0 ? p_half_r0 : s_free_r0);
+          } else {
+            mbar_arrive(h == 0 ? &bars->p_half[qt] : &bars->s_free[qt][0]);
+          }
         }
       }
       l = l * alpha + (rsum2.x + rsum2.y);
@@ -491,8 +577,13 @@ attn_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_constant__ CU
   }
 
   tc_fence_before();
-  __syncthreads();
-  if (warp == kWarpMma) tmem_dealloc(tmem, 512);
+  if (kPair) {
+    cluster_sync();  // the peer may still read this CTA's shared memory / arrive on its barriers before this
+    if (warp == kWarpMma) tmem_dealloc_pair(tmem, 512);
+  } else {
+    __syncthreads();
+    if (warp == kWarpMma) tmem_dealloc(tmem, 512);
+  }
 }
 
 // Combine the key splits of attn_kernel<true>: out = sum_s exp(lse_s - lse) O_s, in the fixed order 0..splits-1.
@@ -564,7 +655,7 @@ int attn_lse_splits(const sx_pool *pool, const sx_batch *b, int32_t total_rows) 
 
 sx_status launch_attn(const sx_pool *pool, const sx_batch *b, bool with_pv, const void *q, const int32_t *rows,
                       const int32_t *rows_off, int32_t total_rows, void *out, float *lse, int kv_splits,
-                      float *part, cudaStream_t st) {
+                      float *part, bool cta_pair, cudaStream_t st) {
   const int g = pool->num_q_heads / pool->num_kv_heads;
   const int rpt = kTile / g;
   CUtensorMap tm_q, tm_k, tm_v;
@@ -596,10 +687,31 @@ sx_status launch_attn(const sx_pool *pool, const sx_batch *b, bool with_pv, cons
   p.scale_log2 = (float)(kLog2e / sqrt((double)kHeadDim));
   const int grid = (total_rows / (2 * rpt) + b->num_reqs) * pool->num_kv_heads;  // >= sum_r ceil(n_r / 2rpt) * Hkv
   cudaError_t e;
-  if (with_pv) {
-    e = cudaFuncSetAttribute(attn_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, AttnCfg::kSmemBytes);
+  if (with_pv && p.kv_splits == 1 && cta_pair) {
+    // CTA pairs: clusters of two CTAs over adjacent row pairs; sum_r ceil(pairs_r / 2) clusters per KV head
+    e = cudaFuncSetAttribute(attn_kernel<true, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, AttnCfg::kSmemBytes);
     if (e != cudaSuccess) return set_error(SX_ERR_CUDA, "attn smem attr: %s", cudaGetErrorString(e));
-    attn_kernel<true><<<grid * p.kv_splits, kAttnThreads, AttnCfg::kSmemBytes, st>>>(tm_q, tm_k, tm_v, p);
+    const int clusters = (total_rows / (4 * rpt) + b->num_reqs) * pool->num_kv_heads;
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = dim3(2 * clusters);
+    cfg.blockDim = dim3(kAttnThreads);
+    cfg.dynamicSmemBytes = AttnCfg::kSmemBytes;
+    cfg.stream = st;
+    cudaLaunchAttribute attr[1];
+    attr[0].id = cudaLaunchAttributeClusterDimension;
+    attr[0].val.clusterDim.x = 2;
+    attr[0].val.clusterDim.y = 1;
+    attr[0].val.clusterDim.z = 1;
+    cfg.attrs = attr;
+    cfg.numAttrs = 1;
+    e = cudaLaunchKernelEx(&cfg, attn_kernel<true, true>, tm_q, tm_k, tm_v, p);
+    if (e != cudaSuccess) return set_error(SX_ERR_CUDA, "attn pair launch: %s", cudaGetErrorString(e));
+    return check_launch("attn_kernel<pv,pair>");
+  }
+  if (with_pv) {
+    e = cudaFuncSetAttribute(attn_kernel<true, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, AttnCfg::kSmemBytes);
+    if (e != cudaSuccess) return set_error(SX_ERR_CUDA, "attn smem attr: %s", cudaGetErrorString(e));
+    attn_kernel<true, false><<<grid * p.kv_splits, kAttnThreads, AttnCfg::kSmemBytes, st>>>(tm_q, tm_k, tm_v, p);
     if (p.kv_splits > 1) {
       sx_status ms = check_launch("attn_kernel<pv>");
       if (ms != SX_OK) return ms;
@@ -609,9 +721,10 @@ sx_status launch_attn(const sx_pool *pool, const sx_batch *b, bool with_pv, cons
       return check_launch("attn_merge_kernel");
     }
   } else {
-    e = cudaFuncSetAttribute(attn_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, AttnCfg::kSmemBytes);
+    e = cudaFuncSetAttribute(attn_kernel<false, false>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                             AttnCfg::kSmemBytes);
     if (e != cudaSuccess) return set_error(SX_ERR_CUDA, "lse smem attr: %s", cudaGetErrorString(e));
-    attn_kernel<false><<<grid * p.kv_splits, kAttnThreads, AttnCfg::kSmemBytes, st>>>(tm_q, tm_k, tm_v, p);
+    attn_kernel<false, false><<<grid * p.kv_splits, kAttnThreads, AttnCfg::kSmemBytes, st>>>(tm_q, tm_k, tm_v, p);
   }
   return check_launch(with_pv ? "attn_kernel<pv>" : "attn_kernel<lse>");
 }

@@ -47,7 +47,7 @@ size_t select_scratch_bytes(const sx_batch *b);
 // tcgen05 kernels. q_rows: bf16 [total_rows][Hq][128]; rows == nullptr => row n is position n - off[req].
 sx_status launch_attn(const sx_pool *pool, const sx_batch *b, bool with_pv, const void *q, const int32_t *rows,
                       const int32_t *rows_off, int32_t total_rows, void *out, float *lse, int kv_splits,
-                      float *part, cudaStream_t st);
+                      float *part, bool cta_pair, cudaStream_t st);
 int attn_pv_splits(const sx_pool *pool, const sx_batch *b, int32_t total_rows);
 size_t attn_part_bytes();
 int attn_lse_splits(const sx_pool *pool, const sx_batch *b, int32_t total_rows);

@@ -30,6 +30,7 @@ class GpuLayer:
     def __init__(self, lay, lt, device="cuda", batch: Optional[sx.DeviceBatch] = None):
         self.lay = lay
         self.dev = torch.device(device)
+        self.cta_pair = False   # SX_ATTN_CTA_PAIR for every attention call of this layer
         self.batch = batch if batch is not None else sx.DeviceBatch(lay, self.dev)
         # lt: workloads.LayerTensors (numpy bit patterns) or any object whose pool_k / pool_v / q_full /
         # k_fresh / v_fresh are already 2-byte device tensors
@@ -127,7 +128,7 @@ class GpuLayer:
         self.out = torch.empty((n, hq, 128), dtype=torch.int16, device=self.dev)
         self.lse = torch.empty((n, hq), dtype=torch.float32, device=self.dev) if want_lse else None
         sx.sparse_attn(self.pool, self.batch, self.q_R, self.out, rows_R=self.rows_R, rows_off=self.rows_off,
-                       total_rows=n, lse=self.lse, cuda_core=cuda_core)
+                       total_rows=n, lse=self.lse, cuda_core=cuda_core, cta_pair=self.cta_pair)
 
     # ---- whole layers
     def step_sparse(self, rows_given=None, do_realign: bool = True, want_scores: bool = True):
@@ -154,5 +155,6 @@ class GpuLayer:
         sx.scatter_kv(self.pool, self.batch, self.k_fresh, self.v_fresh, all_rows, self.batch.tok_off, max_rows=t)
         self.out = torch.empty((t, lay.num_q_heads, 128), dtype=torch.int16, device=self.dev)
         self.lse = torch.empty((t, lay.num_q_heads), dtype=torch.float32, device=self.dev) if want_lse else None
-        sx.sparse_attn(self.pool, self.batch, self.q_full, self.out, total_rows=t, lse=self.lse, full=True)
+        sx.sparse_attn(self.pool, self.batch, self.q_full, self.out, total_rows=t, lse=self.lse, full=True,
+                       cta_pair=self.cta_pair)
         self.rows_R = all_rows

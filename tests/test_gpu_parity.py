@@ -127,12 +127,15 @@ def test_scatter_stage(name):
     assert np.array_equal(g.batch.v_block_table.cpu().numpy(), vt)
 
 
+@pytest.mark.parametrize("pair", [False, True], ids=["1cta", "cta-pair"])
 @pytest.mark.parametrize("name", list(CASES))
-def test_sparse_layer_chained(name):
-    """Whole sparse layer on the GPU (its own outputs feed the next stage) vs the oracle layer driver."""
+def test_sparse_layer_chained(name, pair):
+    """Whole sparse layer on the GPU (its own outputs feed the next stage) vs the oracle layer driver.
+    cta-pair: stage (c) with SX_ATTN_CTA_PAIR (2-CTA clusters, odd pair counts and ragged tails included)."""
     GpuLayer, dev_to_bits = _gpu()
     lay, lt, res, pk, pv, kt, vt = prepared(name)
     g = GpuLayer(lay, lt)
+    g.cta_pair = pair
     g.step_sparse()
     torch.cuda.synchronize()
     sc = g.scores.cpu().numpy().astype(np.float64)
@@ -171,13 +174,15 @@ def test_sparse_layer_chained(name):
         assert np.all(np.abs(a - b) <= 2.0 ** -7 * np.abs(b) + 1e-5)
 
 
+@pytest.mark.parametrize("pair", [False, True], ids=["1cta", "cta-pair"])
 @pytest.mark.parametrize("name", ["tiny", "tiny-ragged", "tiny-g7", "C1", "C3-eighth"])
-def test_full_layer(name):
+def test_full_layer(name, pair):
     """Full-attention layer (layers below the threshold, Alg. 1 l.507-511): R = all positions."""
     GpuLayer, dev_to_bits = _gpu()
     lay, lt = prepared(name)[:2]
     res, pk, pv, kt, vt = oracle_layer(lay, lt, mode="full")
     g = GpuLayer(lay, lt)
+    g.cta_pair = pair
     g.step_full()
     torch.cuda.synchronize()
     out = orc.bf16_to_f64(dev_to_bits(g.out))
