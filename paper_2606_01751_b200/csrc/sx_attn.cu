@@ -67,7 +67,8 @@ struct AttnBars {
   uint64_t q_full;
   uint64_t kv_full[kKvStagesPair], kv_empty[kKvStagesPair];
   uint64_t s_full[2][2];  // [query tile][buffer]: S = Q K^T landed in TMEM   (buffer 1: LSE-only variant)
-  uint64_t s_free[2][2];  // softmax -> MMA: P written (PV variant) / S consumed (LSE-only); 128 arrivals
+  uint64_t s_free[2][2];  // softmax -> MMA. PV variant: [0] all of P written, [1] S is in registers;
+                          // LSE-only: S of buffer b consumed. 128 arrivals
   uint64_t p_half[2];     // softmax -> MMA: keys [0, 64) of P written (PV variant); 128 arrivals
   uint64_t o_full[2];     // last PV of the query tile completed
   uint64_t v_landed;      // CTA-pair variant: the V tile that holds keys >= T is in shared memory (both CTAs)
@@ -248,10 +249,12 @@ attn_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_constant__ CU
         }
       }
       // single CTA: lane = (page of the tile, 64-column half), 16 boxes per item.
-      // kPair: 8 boxes per item: K item = this CTA's 64 keys (4 pages) x both halves -> [half][64 keys][128 B];
+      // kPair: 8 boxes per item: K item = this CTA's 64 keys (4 pages) x both halves -> [half][64 keys][128 B],
+      //        the keys being 32 of each 64-key half of the tile: pages {2r, 2r+1, 4+2r, 5+2r} for rank r;
       //        V item = all 8 pages x the CTA's own 64-column half -> [128 keys][128 B].
       const int n_items = kWithPV ? 2 * n_tiles : n_tiles;
-      const int pg_k = kPair ? 4 * rank + (lane >> 1) : (lane >> 1), half_k = lane & 1;
+      const int pgi = lane >> 1;
+      const int pg_k = kPair ? 2 * rank + (pgi & 1) + 4 * (pgi >> 1) : pgi, half_k = lane & 1;
       const int pg_v = kPair ? lane : (lane >> 1), half_v = kPair ? rank : (lane & 1);
       const int n_boxes = kPair ? 8 : 16;
       auto table_entry = [&](int it) -> int {
@@ -289,10 +292,12 @@ attn_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_constant__ CU
       // One thread runs the whole issue loop (waits included): no per-instruction election, and the
       // descriptors are a base value plus small constants (the address field is (addr >> 4)).
       if (rank == 0 && elect_one()) {
-        constexpr uint32_t idesc_qk = umma_idesc_bf16(kPair ? 256 : 128, 128, 0, 0);
+        // PV variant: S = Q K^T is issued as two 64-key halves (N = 64), see issue_qk_half
+        constexpr uint32_t idesc_qk = umma_idesc_bf16(kPair ? 256 : 128, kWithPV ? 64 : 128, 0, 0);
         constexpr uint32_t idesc_pv = umma_idesc_bf16(kPair ? 256 : 128, 128, 0, 1);
         constexpr uint32_t kSlotStep = kStageBytes >> 4;
         constexpr int kKHalf = kPair ? kHalfBytes / 2 : kHalfBytes;  // bytes between the two 64-column halves of K
+        constexpr uint32_t kKSub = ((kPair ? 32 : 64) * 128) >> 4;   // this CTA's K rows of a 64-key half (16-B units)
         const uint64_t q_desc = umma_smem_desc(smem_u32(smem + Cfg::kOffQ), 16, 1024);
         const uint64_t k_desc = umma_smem_desc(smem_u32(smem + Cfg::kOffKV), 16, 1024);
         const uint64_t v_desc = umma_smem_desc(smem_u32(smem + Cfg::kOffKV), kHalfBytes, 1024);
@@ -318,14 +323,33 @@ attn_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_constant__ CU
           }
           commit(&bars->s_full[i][b]);
         };
+        // PV variant: keys [64h, 64h + 64) of the tile in `slot` -> columns [64h, 64h + 64) of S_i, no commit
+        auto issue_qk_half = [&](int i, int slot, int h) {
+          const uint32_t qd = q_lo + (uint32_t)i * (kTileBytes >> 4);
+          const uint32_t kd = k_lo + (uint32_t)slot * kSlotStep + (uint32_t)h * kKSub;
+          const uint32_t d = tmem + i * 128 + h * 64;
+#pragma unroll
+          for (int kk = 0; kk < 8; ++kk) {
+            const uint32_t oq = ((kk >> 2) * kHalfBytes + (kk & 3) * 32) >> 4;
+            const uint32_t ok = ((kk >> 2) * kKHalf + (kk & 3) * 32) >> 4;
+            if (kPair) umma_ss2_pair(d, qd + oq, qk_hi, kd + ok, qk_hi, idesc_qk, kk > 0);
+            else umma_ss2(d, qd + oq, qk_hi, kd + ok, qk_hi, idesc_qk, kk > 0);
+          }
+        };
         if (kWithPV) {
           // ring item 2t+1 = V(t), 2t+2 = K(t+1): (slot, phase) advanced incrementally
           int sv = 1, sk = 2, phv = 0, phk = 0;
           if (n_tiles > 0) {  // (a key split may hold no tile of this CTA's rows)
             mbar_wait(&bars->kv_full[0], 0);
             tc_fence_after();
-            if (n_t[0] > 0) issue_qk(0, 0, 0);
-            if (n_t[1] > 0) issue_qk(1, 0, 0);
+#pragma unroll
+            for (int i = 0; i < 2; ++i) {
+              if (n_t[i] > 0) {
+                issue_qk_half(i, 0, 0);
+                issue_qk_half(i, 0, 1);
+                commit(&bars->s_full[i][0]);
+              }
+            }
             commit(&bars->kv_empty[0]);
           }
           for (int t = 0; t < n_tiles; ++t) {
@@ -342,6 +366,13 @@ attn_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_constant__ CU
             for (int i = 0; i < 2; ++i) {
               if (t < n_t[i]) {
                 const uint32_t d_o = tmem + 256 + i * 128, a_p = tmem + i * 128;
+                if (t + 1 < n_t[i]) {
+                  // S_i(t) is in the softmax threads' registers and P_i(t) will only use columns [0, 64): the
+                  // upper half of S_i(t + 1) is computed now, off the P -> PV -> QK -> softmax chain
+                  wait_softmax(&bars->s_free[i][1], t & 1);
+                  tc_fence_after();
+                  issue_qk_half(i, sk, 1);
+                }
                 wait_softmax(&bars->p_half[i], t & 1);  // keys [0, 64) of P_i(t) are in TMEM
                 tc_fence_after();
 #pragma unroll
@@ -357,7 +388,10 @@ attn_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_constant__ CU
                   else umma_ts2(d_o, a_p + kk * 8, vd + kk * 128, v_hi, idesc_pv, 1);
                 }
                 if (t == n_t[i] - 1) commit(&bars->o_full[i]);
-                if (t + 1 < n_t[i]) issue_qk(i, 0, sk);
+                if (t + 1 < n_t[i]) {
+                  issue_qk_half(i, sk, 0);
+                  commit(&bars->s_full[i][0]);
+                }
               }
             }
             commit(&bars->kv_empty[sv]);
@@ -403,6 +437,7 @@ attn_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_constant__ CU
     // kPair: P-ready arrivals go to rank 0's barriers (the issuer lives there)
     const uint32_t p_half_r0 = kPair ? mapa_u32(smem_u32(&bars->p_half[qt]), 0) : 0;
     const uint32_t s_free_r0 = kPair ? mapa_u32(smem_u32(&bars->s_free[qt][0]), 0) : 0;
+    const uint32_t s_loaded_r0 = kPair ? mapa_u32(smem_u32(&bars->s_free[qt][1]), 0) : 0;
     float m_used = -INFINITY, l = 0.f;
 
     for (int t = 0; t < my_tiles; ++t) {
@@ -424,9 +459,14 @@ attn_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_constant__ CU
       for (int c = 0; c < 4; ++c) {
         if (c == 2) {
           tmem_wait_ld();
+          tc_fence_before();
           if (!kWithPV) {
-            tc_fence_before();
             mbar_arrive(&bars->s_free[qt][b]);
+          } else if (kPair) {  // S is in registers: columns [64, 128) may take the next tile's S
+            __syncwarp();
+            if (lane == 0) mbar_arrive_cluster(s_loaded_r0);
+          } else {
+            mbar_arrive(&bars->s_free[qt][1]);
           }
         }
         if (nvalid < kTile) {
