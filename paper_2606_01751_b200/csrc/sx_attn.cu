@@ -14,7 +14,9 @@
 //     K(1), V(1), ...). K is the K-major B operand of S = Q K^T, V the MN-major B operand of O += P V.
 //   * TMEM (512 columns): S_0, S_1 (128 fp32 columns each), O_0, O_1 (128 each). P (bf16) is written
 //     by the softmax threads back into the first 64 columns of its S and is the TMEM A operand of
-//     the PV MMA, so P never touches shared memory.
+//     the PV MMA, so P never touches shared memory. S = Q K^T is issued as two N = 64 MMAs: the upper
+//     one (keys 64-127 -> columns 64-127, which P never uses) as soon as the softmax threads hold the
+//     previous S in registers, the lower one after the PV MMAs that read P.
 //   * warps 8 and 10 = TMA producers (K tiles / V tiles), warp 9 = MMA issuer (one elected lane);
 //     warps 0-3 / 4-7 = softmax warpgroups of query tile 0 / 1: thread = one row of S (tcgen05.ld), fp32 online softmax in the
 //     exp2 domain with lazy rescale (O is rescaled only when the row maximum grew by more than 2^8),
