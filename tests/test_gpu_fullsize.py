@@ -58,13 +58,15 @@ def _check_keys(name, lay, lt, gk, pk, kt, kref):
     assert np.array_equal(gk[untouched], lt.pool_k[untouched]), name
 
 
-@pytest.mark.parametrize("name", ["C2", "C4", "C4-cow", "C5"])
+@pytest.mark.parametrize("name", ["C2", "C2-pair", "C4", "C4-cow", "C5"])
 def test_fullsize_sparse_layer(name):
     """One sparse-mode layer with its own two-sweep selection (what bench.py --config <name> times).
     C4-cow: the copy-on-write variant of C4 (V pages alias the shared source pages until a row is written,
-    reading A14); keys, scores and index sets are those of C4, so the same carve log applies."""
+    reading A14); keys, scores and index sets are those of C4, so the same carve log applies.
+    C2-pair: stage (c) with SX_ATTN_CTA_PAIR (the 2-CTA cluster kernel; 47 row pairs per request = an odd count)."""
     GpuLayer, dev_to_bits = _gpu()
-    lay = wl.config_c4(cow=True) if name == "C4-cow" else wl.CONFIGS[name]()
+    cta_pair = name.endswith("-pair")
+    lay = wl.config_c4(cow=True) if name == "C4-cow" else wl.CONFIGS[name.split("-")[0]]()
     name = name.split("-")[0]
     lt = wl.build_layer(lay, 0)
     apply_carve(lt, load_carve(os.path.join(GOLD, "carve_%s.txt" % name)))
@@ -72,6 +74,7 @@ def test_fullsize_sparse_layer(name):
 
     # ---- GPU: whole layer, chained
     g = GpuLayer(lay, lt)
+    g.cta_pair = cta_pair
     g.realign()
     torch.cuda.synchronize()
     gk_re, gv_re = dev_to_bits(g.pool_k).copy(), dev_to_bits(g.pool_v).copy()
