@@ -173,6 +173,11 @@ sx_status sx_score_select_ex(const sx_pool *pool, const sx_batch *batch, const v
                              float *scores, int32_t *sel_idx, int32_t *rows_R, int32_t *rows_off_out, void *ws,
                              size_t ws_bytes, sx_stream stream);
 
+/* Token classes (Alg. 1 l.500-501). A position of a request is NEW if it is listed in new_idx (I_nr), REUSED if a
+ * segment covers it (I_reuse: re-aligned by sx_rope_realign, the candidates of the top-k, the only members of
+ * S_ov / S_tail), otherwise a PREFIX-CACHE HIT: its K/V are already in the request's pages at the right position
+ * ("excluded from the current prefill computation"): visible as a key everywhere, never a candidate, never a query
+ * row. With prefix hits, full-attention layers are run in mode 0 with the non-prefix positions as rows_R. */
 #define SX_ATTN_CUDA_CORE 2 /* flag for sx_sparse_attn's mode: CUDA-core kernels for small row sets */
 #define SX_ATTN_CTA_PAIR 4  /* flag for sx_sparse_attn's mode: 2-CTA clusters with tcgen05.mma.cta_group::2 */
 

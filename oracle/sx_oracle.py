@@ -217,11 +217,15 @@ def scores(pool_k: np.ndarray, k_table_row: np.ndarray, seq_len: int, q_new: np.
     return (s, lse) if want_lse else s
 
 
-def select_topk(s: np.ndarray, is_new: np.ndarray, k: int) -> Tuple[np.ndarray, np.ndarray]:
+def select_topk(s: np.ndarray, is_new: np.ndarray, k: int, cand_mask=None) -> Tuple[np.ndarray, np.ndarray]:
     """Eq. (3) over cached positions only (reading A7); order by (score desc, position asc) (A8).
-    Returns (S_key sorted by position, R = I_nr U S_key sorted)."""
+    Returns (S_key sorted by position, R = I_nr U S_key sorted).
+    cand_mask: I_reuse as a boolean mask (default: every position that is not new). Positions that are neither
+    new nor candidates are prefix-cache hits (Alg. 1 l.501: excluded from the current prefill computation)."""
     s = np.asarray(s, dtype=np.float64)
-    cand = np.nonzero(~np.asarray(is_new, dtype=bool))[0]
+    if cand_mask is None:
+        cand_mask = ~np.asarray(is_new, dtype=bool)
+    cand = np.nonzero(np.asarray(cand_mask, dtype=bool))[0]
     k = max(0, min(int(k), len(cand)))
     order = np.lexsort((cand, -s[cand]))          # primary: -score ascending, secondary: position
     sel = np.sort(cand[order[:k]]).astype(np.int32)
@@ -230,14 +234,16 @@ def select_topk(s: np.ndarray, is_new: np.ndarray, k: int) -> Tuple[np.ndarray, 
 
 
 def recompute_set(is_new: np.ndarray, sel: np.ndarray, seg_ranges, overflow_blocks: int = 1,
-                  tail_tokens: int = 64, block: int = 16) -> np.ndarray:
+                  tail_tokens: int = 64, block: int = 16, cand_mask=None) -> np.ndarray:
     """Alg. 1 l.535-539, one request: R = I_nr U S_key U S_ov U S_tail, sorted.
     S_ov: every maximal contiguous interval [a, b] of I_nr expanded by `overflow_blocks` blocks of `block`
     positions on both sides (clipped to the request). S_tail: if the last position is a reused token, the
     last `tail_tokens` positions of the reused segment that contains it. seg_ranges: [(start, end)) of the
-    reused segments of this request in current positions."""
+    reused segments of this request in current positions. cand_mask: I_reuse (default: not new); S_ov and
+    S_tail hold reused positions only (prefix-cache hits are never recomputed)."""
     is_new = np.asarray(is_new, dtype=bool)
     t = len(is_new)
+    cand_mask = ~is_new if cand_mask is None else np.asarray(cand_mask, dtype=bool)
     r = set(int(i) for i in np.nonzero(is_new)[0]) | set(int(i) for i in sel)
     a = None
     for i in range(t + 1):                       # walk the maximal intervals of I_nr
@@ -246,10 +252,10 @@ def recompute_set(is_new: np.ndarray, sel: np.ndarray, seg_ranges, overflow_bloc
             a = i
         if not inside and a is not None:
             b = i - 1
-            r.update(range(max(0, a - overflow_blocks * block), a))
-            r.update(range(b + 1, min(t, b + 1 + overflow_blocks * block)))
+            r.update(q for q in range(max(0, a - overflow_blocks * block), a) if cand_mask[q])
+            r.update(q for q in range(b + 1, min(t, b + 1 + overflow_blocks * block)) if cand_mask[q])
             a = None
-    if tail_tokens > 0 and not is_new[t - 1]:
+    if tail_tokens > 0 and cand_mask[t - 1]:
         start = 0
         for (s0, s1) in seg_ranges:
             if s0 <= t - 1 < s1:
@@ -330,7 +336,11 @@ def layer_step(pool_k, pool_v, k_table, v_table, cow_private, segments, src_bloc
                 s, l = scores(pool_k, k_table[r], t, q_full[o + nidx], nidx, num_q_heads, want_lse=True)
                 is_new = np.zeros(t, dtype=bool)
                 is_new[nidx] = True
-                sel, rows = select_topk(s, is_new, int(k_per_req[r]))
+                cand = np.zeros(t, dtype=bool)       # I_reuse: the positions covered by the request's segments
+                for (sr, slen, _old, snew, _off) in np.asarray(segments).reshape(-1, 5):
+                    if int(sr) == r:
+                        cand[int(snew):int(snew) + int(slen)] = True
+                sel, rows = select_topk(s, is_new, int(k_per_req[r]), cand)
                 res.scores.append(s)
                 res.lse_new.append(l)
             else:

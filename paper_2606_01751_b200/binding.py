@@ -262,7 +262,9 @@ def sparse_attn(pool: DevicePool, batch: DeviceBatch, q: torch.Tensor, out: torc
 def selection_offsets(lay) -> tuple:
     """Host CSR offsets (sel_off, rows_off) for k_per_req clamped to the cached-token count."""
     n_new = np.diff(np.asarray(lay.new_off)).astype(np.int64)
-    n_cached = np.asarray(lay.seq_len, dtype=np.int64) - n_new
+    n_cached = np.zeros(len(n_new), dtype=np.int64)      # |I_reuse| = tokens covered by segments
+    for seg in np.asarray(lay.segments).reshape(-1, 5):
+        n_cached[int(seg[0])] += int(seg[1])
     k = np.minimum(np.asarray(lay.k_per_req, dtype=np.int64), n_cached)
     sel_off = np.concatenate([[0], np.cumsum(k)]).astype(np.int32)
     rows_off = np.concatenate([[0], np.cumsum(k + n_new)]).astype(np.int32)

@@ -76,7 +76,7 @@ select_kernel(int num_kv_heads, int total_tokens, const int32_t *__restrict__ se
   const int ns = gridDim.y, sl = blockIdx.y;
   int *ghist = scratch + (size_t)blockIdx.x * (4 * 256 + 4 * 64);  // [4 passes][256] then [4 counters][64 slices]
   int *gcnt = ghist + 4 * 256;
-  extern __shared__ uint32_t is_new[];  // bitmap over positions; a second bitmap (forced rows) follows it
+  extern __shared__ uint32_t is_new[];  // bitmaps over positions: I_nr, forced rows (S_ov U S_tail), candidates
   __shared__ int hist[256];
   __shared__ int warp_tot[3][kSelWarps];
   __shared__ int tot[3];
@@ -92,16 +92,30 @@ select_kernel(int num_kv_heads, int total_tokens, const int32_t *__restrict__ se
   const int n0 = new_off[req], nn = new_off[req + 1] - n0;
   const int words = (T + 31) >> 5;
   int k = sel_off[req + 1] - sel_off[req];
-  const int n_cached = T - nn;
+  // Candidates of Eq. (3) = I_reuse = the positions covered by this request's segments. Positions that are neither
+  // new nor in a segment are prefix-cache hits (Alg. 1 l.501: "excluded from the current prefill computation"):
+  // visible as keys, never candidates, never in S_ov / S_tail, never query rows.
+  int n_cached = 0;
+  for (int m = 0; m < num_segments; ++m)
+    if (segs[m].req == req) n_cached += segs[m].len;
   if (k > n_cached) k = n_cached;
   if (k < 0) k = 0;
 
   uint32_t *forced = is_new + words;  // S_ov U S_tail (Alg. 1 l.535-536), cached positions only
-  for (int i = threadIdx.x; i < 2 * words; i += kSelThreads) is_new[i] = 0u;
+  uint32_t *cand = forced + words;    // I_reuse
+  for (int i = threadIdx.x; i < 3 * words; i += kSelThreads) is_new[i] = 0u;
   __syncthreads();
   for (int i = threadIdx.x; i < nn; i += kSelThreads) {
     int p = new_idx[n0 + i];
     atomicOr(&is_new[p >> 5], 1u << (p & 31));
+  }
+  for (int m = 0; m < num_segments; ++m) {  // segment bounds are multiples of 16: half a bitmap word per page
+    if (segs[m].req != req) continue;
+    const int p0 = segs[m].new_pos;
+    for (int c = threadIdx.x; c < segs[m].len / kPage; c += kSelThreads) {
+      const int q = p0 + c * kPage;
+      if (q < T) atomicOr(&cand[q >> 5], 0xFFFFu << (q & 31));
+    }
   }
   if (ov_tokens > 0 || tail_tokens > 0) {
     __syncthreads();
@@ -111,14 +125,14 @@ select_kernel(int num_kv_heads, int total_tokens, const int32_t *__restrict__ se
       const int p = new_idx[n0 + i];
       if (i == 0 || new_idx[n0 + i - 1] != p - 1)
         for (int q = max(0, p - ov_tokens); q < p; ++q)
-          if (!((is_new[q >> 5] >> (q & 31)) & 1u)) atomicOr(&forced[q >> 5], 1u << (q & 31));
+          if ((cand[q >> 5] >> (q & 31)) & 1u) atomicOr(&forced[q >> 5], 1u << (q & 31));
       if (i == nn - 1 || new_idx[n0 + i + 1] != p + 1)
         for (int q = p + 1; q <= min(T - 1, p + ov_tokens); ++q)
-          if (!((is_new[q >> 5] >> (q & 31)) & 1u)) atomicOr(&forced[q >> 5], 1u << (q & 31));
+          if ((cand[q >> 5] >> (q & 31)) & 1u) atomicOr(&forced[q >> 5], 1u << (q & 31));
     }
     // tail fallback (Alg. 1 l.536): the prompt ends inside a reused segment -> its last
     // tail_tokens positions are recomputed
-    if (tail_tokens > 0 && !((is_new[(T - 1) >> 5] >> ((T - 1) & 31)) & 1u)) {
+    if (tail_tokens > 0 && ((cand[(T - 1) >> 5] >> ((T - 1) & 31)) & 1u)) {
       int seg_start = 0;  // start of the reused segment that contains position T - 1
       for (int m = 0; m < num_segments; ++m)
         if (segs[m].req == req && segs[m].new_pos <= T - 1 && T - 1 < segs[m].new_pos + segs[m].len)
@@ -152,7 +166,7 @@ select_kernel(int num_kv_heads, int total_tokens, const int32_t *__restrict__ se
         for (int q = 0; q < 8; ++q) {
           const int j = j0 + q * kSelThreads + threadIdx.x;
           int bin = -1;
-          if (j < je && !((is_new[j >> 5] >> (j & 31)) & 1u) && (u[q] & mask) == prefix)
+          if (j < je && ((cand[j >> 5] >> (j & 31)) & 1u) && (u[q] & mask) == prefix)
             bin = (int)((u[q] >> shift) & 255u);
           const unsigned peers = __match_any_sync(0xffffffffu, bin);
           if (bin >= 0 && (threadIdx.x & 31) == __ffs(peers) - 1) atomicAdd(&hist[bin], __popc(peers));
@@ -249,7 +263,7 @@ select_kernel(int num_kv_heads, int total_tokens, const int32_t *__restrict__ se
     if (j < j_hi) {
       isn = (is_new[j >> 5] >> (j & 31)) & 1u;
       frc = (forced[j >> 5] >> (j & 31)) & 1u;
-      if (!isn && k > 0) {
+      if (k > 0 && ((cand[j >> 5] >> (j & 31)) & 1u)) {
         gt = u > thr;
         eq = u == thr;
       }
@@ -353,7 +367,7 @@ sx_status launch_select(const sx_pool *pool, const sx_batch *b, const float *par
                         const int32_t *rows_off, float *scores, int32_t *sel_idx, int32_t *rows_R, int ov_blocks,
                         int tail_tokens, int32_t *rows_tmp, int32_t *rows_cnt, int32_t *rows_off_out, int *scratch,
                         cudaStream_t st) {
-  size_t smem = 2 * sizeof(uint32_t) * (size_t)((b->max_seq_len + 31) / 32);
+  size_t smem = 3 * sizeof(uint32_t) * (size_t)((b->max_seq_len + 31) / 32);
   if (smem > 200 * 1024) return set_error(SX_ERR_UNSUPPORTED, "max_seq_len %d too large for the select bitmaps", b->max_seq_len);
   if (smem > 40 * 1024) {
     cudaError_t e = cudaFuncSetAttribute(select_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);

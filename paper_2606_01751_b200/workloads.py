@@ -124,6 +124,19 @@ class Layout:
     def total_seg_pages(self) -> int:
         return int(self.segments[:, 1].sum() // PAGE) if self.num_segments else 0
 
+    def cached_mask(self, req: int) -> np.ndarray:
+        """bool [T_req]: position is covered by a reused segment (I_reuse, the top-k candidates)."""
+        m = np.zeros(int(self.seq_len[req]), dtype=bool)
+        for s in range(self.num_segments):
+            r, ln, _, new_pos, _ = (int(v) for v in self.segments[s])
+            if r == req:
+                m[new_pos:new_pos + ln] = True
+        return m
+
+    def prefix_mask(self, req: int) -> np.ndarray:
+        """bool [T_req]: prefix-cache hit (neither new nor in a segment)."""
+        return ~(self.cached_mask(req) | self.is_new_mask(req))
+
     def is_new_mask(self, req: int) -> np.ndarray:
         m = np.zeros(int(self.seq_len[req]), dtype=bool)
         m[self.new_idx[self.new_off[req]:self.new_off[req + 1]]] = True
@@ -150,7 +163,9 @@ class LayerTensors:
     v_fresh: np.ndarray  # [sum T][Hkv][128]
 
 
-ReqSpec = Sequence[Tuple[str, int]]   # ("new", length) | ("seg", pool_segment_id)
+# ("new", length) | ("seg", pool_segment_id) | ("prefix", length): positions whose K/V the request's own pages
+# already hold at the right positions (prefix-cache hits, Alg. 1 l.501): keys only, no queries, never candidates
+ReqSpec = Sequence[Tuple[str, int]]
 
 
 def build_layout(name: str, cfg_id: int, num_q_heads: int, num_kv_heads: int, rope_theta: float,
@@ -165,7 +180,7 @@ def build_layout(name: str, cfg_id: int, num_q_heads: int, num_kv_heads: int, ro
     for r, spec in enumerate(requests):
         t = 0
         for kind, val in spec:
-            t += val if kind == "new" else pool_segments[val].length
+            t += val if kind in ("new", "prefix") else pool_segments[val].length
         seq_len[r] = t
     pages_per_req = (seq_len + PAGE - 1) // PAGE
     max_pages = int(pages_per_req.max())
@@ -193,6 +208,9 @@ def build_layout(name: str, cfg_id: int, num_q_heads: int, num_kv_heads: int, ro
                 assert val % PAGE == 0 or pos + val == seq_len[r]
                 new_idx.append(np.arange(pos, pos + val, dtype=np.int32))
                 pos += val
+            elif kind == "prefix":
+                assert pos % PAGE == 0 and val % PAGE == 0
+                pos += val
             else:
                 ps = pool_segments[val]
                 assert pos % PAGE == 0
@@ -208,7 +226,9 @@ def build_layout(name: str, cfg_id: int, num_q_heads: int, num_kv_heads: int, ro
         new_off.append(sum(len(a) for a in new_idx))
     tok_off = np.concatenate([[0], np.cumsum(seq_len)]).astype(np.int32)
     n_new = np.diff(np.asarray(new_off))
-    n_cached = seq_len - n_new
+    n_cached = np.zeros(num_reqs, dtype=np.int64)       # |I_reuse|: segment tokens (prefix hits are not candidates)
+    for (r, ln, _old, _new, _off) in segs:
+        n_cached[r] += ln
     if k_override is not None:
         k_per_req = np.asarray(k_override, dtype=np.int32)
     else:
@@ -273,6 +293,12 @@ def build_layer(lay: Layout, layer: int = 0, threads: int = 8, need_q: bool = Tr
     with ThreadPoolExecutor(max_workers=max(1, threads)) as ex:
         list(ex.map(do_pool_seg, range(len(lay.pool_segments))))
         list(ex.map(do_tok_chunk, chunks))
+    # prefix-cache hits: the request's own pages already hold their K/V (here: the fresh rows of those positions)
+    for r in range(lay.num_reqs):
+        o = int(lay.tok_off[r])
+        for pos in np.nonzero(lay.prefix_mask(r))[0]:
+            pool_k[lay.k_block_table[r, pos // PAGE], :, pos % PAGE, :] = k_fresh[o + pos]
+            pool_v[lay.v_block_table[r, pos // PAGE], :, pos % PAGE, :] = v_fresh[o + pos]
     return LayerTensors(layer=layer, pool_k=pool_k, pool_v=pool_v, q_full=q_full,
                         k_fresh=k_fresh, v_fresh=v_fresh)
 
@@ -383,7 +409,7 @@ def config_c5(scale: float = 1.0, ratio: float = 0.05) -> Layout:
 CONFIGS = {"C1": config_c1, "C2": config_c2, "C3": config_c3, "C4": config_c4, "C5": config_c5}
 
 
-def config_tail(seed_id: int = 15) -> Layout:
+def config_tail(seed_id: int = 15, prefix: int = 0) -> Layout:
     """Requests that END inside a reused segment (tail fallback) and whose new-token intervals
     touch reused segments on both sides (overflow): request 0 ends with a 96-token segment
     (tail = its last 64 tokens), request 1 with a 32-token one (tail = all of it), request 2 ends with new
@@ -392,16 +418,22 @@ def config_tail(seed_id: int = 15) -> Layout:
     reqs = [[("new", 16), ("seg", 0), ("new", 16), ("seg", 1), ("seg", 3)],
             [("seg", 2), ("new", 32), ("seg", 0)],
             [("new", 32), ("seg", 1), ("new", 16), ("seg", 2), ("new", 16)]]
+    if prefix:  # prefix-cache hits in front of every request: the first new interval of requests 0 and 2 then has a
+        # prefix-hit block before it, which the overflow must NOT pull in
+        reqs = [[("prefix", prefix)] + spec for spec in reqs]
     # budgets below the number of cached tokens that some new query can see (the tokens behind the last new
     # token score exactly 0 and would turn the cut into a pure position tie)
     return build_layout("tail", seed_id, 4, 2, 10000.0, pool, reqs, [0.2, 0.25, 0.3], 0.1, k_override=[8, 4, 19])
 
 
 def config_tiny(seed_id: int = 9, num_q_heads: int = 4, num_kv_heads: int = 2, tail: int = 0,
-                rope_style: int = 0, cow: bool = False) -> Layout:
-    """Two small requests with uneven segments, negative and zero deltas; optional ragged tail (T % 16 != 0)."""
+                rope_style: int = 0, cow: bool = False, prefix: int = 0) -> Layout:
+    """Two small requests with uneven segments, negative and zero deltas; optional ragged tail (T % 16 != 0);
+    prefix > 0: both requests start with prefix-cache hits (2 * prefix and prefix tokens, multiples of 16)."""
     pool = [PoolSegment(32, 64), PoolSegment(48, 0), PoolSegment(16, 160)]
     reqs = [[("new", 16), ("seg", 0), ("new", 32), ("seg", 1), ("new", 16 + tail)],
             [("seg", 2), ("new", 16), ("seg", 0), ("new", 16)]]
+    if prefix:
+        reqs = [[("prefix", 2 * prefix)] + reqs[0], [("prefix", prefix)] + reqs[1]]
     return build_layout("tiny", seed_id, num_q_heads, num_kv_heads, 10000.0, pool, reqs, [0.25, 0.5], 0.1,
                         cow=cow, rope_style=rope_style)

@@ -72,7 +72,7 @@ def carve_margins(lay: wl.Layout, lt: wl.LayerTensors, tau: float = 1e-3, max_it
         for r in range(lay.num_reqs):
             k = int(lay.k_per_req[r])
             is_new = lay.is_new_mask(r)
-            cand = np.nonzero(~is_new)[0]
+            cand = np.nonzero(lay.cached_mask(r))[0]    # I_reuse (prefix-cache hits are not candidates)
             if k <= 0 or k >= len(cand):
                 continue
             s = sc[r][cand]

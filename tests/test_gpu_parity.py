@@ -33,6 +33,7 @@ CASES = {
     "tiny-g7": lambda: wl.config_tiny(seed_id=12, num_q_heads=7, num_kv_heads=1, tail=3),
     "tiny-g1": lambda: wl.config_tiny(seed_id=13, num_q_heads=2, num_kv_heads=2),
     "tiny-cow": lambda: wl.config_tiny(seed_id=14, cow=True),
+    "tiny-prefix": lambda: wl.config_tiny(seed_id=15, prefix=16, tail=7),   # prefix-cache hits: keys only
     "C1": lambda: wl.config_c1(),
     "C2-quarter": lambda: wl.config_c2(scale=0.25),
     "C3-eighth": lambda: wl.config_c3(scale=0.125),
@@ -339,12 +340,13 @@ def test_realign_all_layers_in_one_launch():
         assert np.array_equal(dev_to_bits(g.pool_v), v)
 
 
-@pytest.mark.parametrize("ov,tail", [(1, 64), (1, 0), (0, 64), (2, 16)])
-def test_overflow_and_tail_fallback(ov, tail):
+@pytest.mark.parametrize("ov,tail,prefix", [(1, 64, 0), (1, 0, 0), (0, 64, 0), (2, 16, 0), (1, 64, 32), (2, 16, 16)])
+def test_overflow_and_tail_fallback(ov, tail, prefix):
     """sx_score_select_ex: R = I_nr U S_key U S_ov U S_tail (Alg. 1 l.535-539) bit-exact against the oracle,
-    then scatter + attention on that (data-dependent) row list."""
+    then scatter + attention on that (data-dependent) row list. prefix > 0: every request starts with prefix-cache
+    hits (visible keys that are never candidates and never pulled in by the overflow)."""
     GpuLayer, dev_to_bits = _gpu()
-    lay = wl.config_tail()
+    lay = wl.config_tail(prefix=prefix)
     lt = wl.build_layer(lay, 0)
     carve_margins(lay, lt)
     g = GpuLayer(lay, lt)
@@ -370,9 +372,10 @@ def test_overflow_and_tail_fallback(ov, tail):
         orc.scatter_kv(pk, pv, kt, vt, None, r, nidx, lt.k_fresh[o + nidx], lt.v_fresh[o + nidx])
         s = orc.scores(pk, kt[r], t, lt.q_full[o + nidx], nidx, lay.num_q_heads)
         is_new = lay.is_new_mask(r)
-        sel, _ = orc.select_topk(s, is_new, int(lay.k_per_req[r]))
+        cand = lay.cached_mask(r)
+        sel, _ = orc.select_topk(s, is_new, int(lay.k_per_req[r]), cand)
         segr = [(int(n), int(n + ln)) for (rq, ln, _, n, _) in lay.segments.tolist() if rq == r]
-        rows = orc.recompute_set(is_new, sel, segr, ov, tail)
+        rows = orc.recompute_set(is_new, sel, segr, ov, tail, cand_mask=cand)
         r0, r1 = int(g.rows_off_h[r]), int(g.rows_off_h[r + 1])
         assert np.array_equal(sel_g[g.sel_off_h[r]:g.sel_off_h[r + 1]], sel), (r, ov, tail)
         assert np.array_equal(rows_g[r0:r1], rows), (r, ov, tail)

@@ -388,3 +388,32 @@ def test_recompute_set_hand_cases():
     assert rows.tolist() == list(range(16, 32)) + list(range(48, 64)) + [70]
     _, plain = orc.select_topk(np.arange(80, dtype=np.float64), is_new, 0)
     assert np.array_equal(orc.recompute_set(is_new, np.asarray([], dtype=np.int32), [], 0, 0), plain)
+
+
+def test_prefix_hits_are_never_candidates_nor_recomputed():
+    """Alg. 1 l.501: "Prefix-cache hits, if present, are excluded from the current prefill computation."
+    Hand case, T = 64: prefix hits [0,16), new [16,32), reused segment [32,64). The prefix positions carry
+    the LARGEST scores and must still not be selected; overflow stops at the prefix (expected lists typed by hand)."""
+    is_new = np.zeros(64, dtype=bool)
+    is_new[16:32] = True
+    cand = np.zeros(64, dtype=bool)
+    cand[32:64] = True
+    s = np.zeros(64)
+    s[0:16] = 100.0                       # prefix hits: high scores, not candidates
+    s[40], s[50], s[33] = 3.0, 2.0, 1.0
+    sel, rows = orc.select_topk(s, is_new, 2, cand)
+    assert sel.tolist() == [40, 50]
+    assert rows.tolist() == list(range(16, 32)) + [40, 50]
+    sel, _ = orc.select_topk(s, is_new, 1000, cand)      # the budget is clamped to |I_reuse| = 32
+    assert sel.tolist() == list(range(32, 64))
+    # default (no mask) = every position that is not new, as before
+    sel, _ = orc.select_topk(s, is_new, 2)
+    assert sel.tolist() == [0, 1]
+    # overflow: one block after the interval (reused), none before it (prefix hit); tail: last position is reused
+    rows = orc.recompute_set(is_new, np.asarray([40]), [(32, 64)], overflow_blocks=1, tail_tokens=8, cand_mask=cand)
+    assert rows.tolist() == list(range(16, 48)) + list(range(56, 64))
+    # a prompt that ENDS in prefix-hit tokens has no tail fallback
+    cand2 = np.zeros(64, dtype=bool)
+    cand2[0:16] = True                    # reused [0,16), new [16,32), prefix-like [32,64) (not candidates)
+    rows = orc.recompute_set(is_new, np.asarray([], dtype=np.int32), [(0, 16)], 1, 8, cand_mask=cand2)
+    assert rows.tolist() == list(range(0, 32))

@@ -101,3 +101,20 @@ def test_tail_layout_and_row_capacity():
             for sel in (cand[:k], cand[-k:] if k else cand[:0]):
                 rows = orc.recompute_set(is_new, sel, segr, ov, tail)
                 assert len(rows) <= cap[r + 1] - cap[r]
+
+
+def test_prefix_layout_classes_partition_the_request():
+    """tiny layout with prefix-cache hits: every position is exactly one of new / reused / prefix hit, the prefix
+    rows of the request's own pages hold the fresh K/V of those positions, budgets count reused tokens only."""
+    lay = wl.config_tiny(seed_id=15, prefix=16, tail=7)
+    lt = wl.build_layer(lay, 0)
+    for r in range(lay.num_reqs):
+        new, reused, pre = lay.is_new_mask(r), lay.cached_mask(r), lay.prefix_mask(r)
+        assert np.all(new.astype(int) + reused.astype(int) + pre.astype(int) == 1)
+        assert pre[:16 * (2 - r)].all() and pre.sum() == 16 * (2 - r)
+        assert int(lay.k_per_req[r]) <= int(reused.sum())
+        o = int(lay.tok_off[r])
+        for pos in np.nonzero(pre)[0]:
+            page, row = lay.k_block_table[r, pos // 16], pos % 16
+            assert np.array_equal(lt.pool_k[page, :, row, :], lt.k_fresh[o + pos])
+            assert np.array_equal(lt.pool_v[page, :, row, :], lt.v_fresh[o + pos])
