@@ -146,7 +146,8 @@ sx_status sx_scatter_kv(const sx_pool *pool, const sx_batch *batch, const void *
  *   scores    device fp32 [total_tokens] or NULL: s_j of every position (token (r,j) at tok_off[r]+j).
  *   sel_idx   device int32 [sel_off[num_reqs]]: S_key per request, ascending positions.
  *   rows_R    device int32 [rows_off[num_reqs]]: R = I_nr U S_key per request, ascending.
- * Candidates are the cached positions only; order = (score descending, position ascending).
+ * Candidates are the REUSED positions only (those covered by a segment of the request; see "Token classes" below);
+ * order = (score descending, position ascending); k is clamped to their number.
  * Scores are fp32 sums in a fixed order (deterministic). Uses ws. */
 sx_status sx_score_select(const sx_pool *pool, const sx_batch *batch, const void *q_new,
                           const float *lse_new, int32_t lse_by_token, const int32_t *sel_off,
