@@ -102,7 +102,7 @@ class ClockSampler:
 
 
 def make_layout(cfg: str, rank: int, world: int):
-    lay = wl.CONFIGS[cfg]()
+    lay = wl.CONFIGS["C3" if cfg == "C3-layer" else cfg]()   # C3-layer: one sparse C3 layer with its own selection
     return lay
 
 
@@ -459,6 +459,14 @@ def run_ours(args):
                          "stage_ms": {k: round(v, 4) for k, v in o["stage_ms"].items()},
                          "attn_tflops": o["roofline"]["achieved"], "attn_frac": o["roofline"]["frac"],
                          "attn_peak": o["roofline"]["peak_src"], "hbm_stage": o["hbm"]}
+        if cfg == "C3":
+            # reading A11, secondary mode: a sparse C3 layer that runs its OWN two-sweep selection (what a stack
+            # costs when every sparse layer selects: 4 full layers + 28 x this)
+            o = measure("C3-layer", 30, 5, ctx, want_e2e=False, want_clocks=False)
+            others["C3_select_every_layer"] = {
+                "ms_per_sparse_layer": round(o["ms_per_step"], 4),
+                "stage_ms": {k: round(v, 4) for k, v in o["stage_ms"].items()},
+                "note": "one sparse C3 layer: realign, scatter(I_nr), two-sweep selection, scatter(S_key), attention"}
         others["S6"] = measure_s6(ctx)
     if rank != 0:
         return
