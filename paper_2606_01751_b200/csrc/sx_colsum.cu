@@ -40,7 +40,7 @@ struct ColsumParams {
   int lse_by_token;
   int lse_splits;     // > 1: lse holds that many partial normalisers [split][total_new][Hq] (key splits)
   size_t lse_stride;  // total_new * Hq
-  float2 *col_tab;   // [query tiles of the batch][Hkv][128]: (lse * log2 e, position as int bits)
+  float2 *col_tab;   // [query tiles of the batch][Hkv] rows of 1 KB: float lse * log2 e [128], then int position [128]
   float *partial;    // [Hkv][total_tokens]
   int num_reqs, max_pages, num_q_heads, num_kv_heads, group, rows_per_tile, total_tokens;
   float scale_log2;
@@ -57,6 +57,8 @@ struct CsBars {
 // Column table of sweep 2: for every GQA-packed query tile (rows_per_tile queries x g heads = up to 128
 // columns) the log2-domain normaliser and the position of each column; pad columns get (+inf, -1) so that
 // their exp2 is 0. One 1-KB row per (query tile, KV head): the colsum producer fetches it with one bulk copy.
+// Normalisers and positions are stored one after the other (128 floats, then 128 ints): tiles that need no
+// causal mask (the majority) read the normalisers only, four columns per 16-byte shared-memory load.
 __global__ void __launch_bounds__(128)
 coltab_kernel(const ColsumParams p) {
   const int g = p.group, rpt = p.rows_per_tile;
@@ -86,7 +88,9 @@ coltab_kernel(const ColsumParams p) {
     }
     lse2 = l * (float)kLog2e;
   }
-  p.col_tab[((size_t)blockIdx.x * p.num_kv_heads + kvh) * 128 + ct] = make_float2(lse2, __int_as_float(qpos));
+  float *row = reinterpret_cast<float *>(p.col_tab + ((size_t)blockIdx.x * p.num_kv_heads + kvh) * 128);
+  row[ct] = lse2;
+  row[128 + ct] = __int_as_float(qpos);
 }
 
 // exp2 of two values on the FMA pipe: x = n + f, n = rint(x), |f| <= 1/2; cubic for 2^f (relative error
@@ -247,9 +251,9 @@ colsum_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_constant__ 
     for (int it = 0; it < n_it; ++it) {
       const int b = it & 1, cs = it & (kCsColStages - 1);
       mbar_wait(&bars->c_full[cs], (it / kCsColStages) & 1);
-      const uint32_t col = smem_u32(col_sm + cs * 128 + hf * 64);
+      const uint32_t col = smem_u32(col_sm + cs * 128) + hf * 256;   // lse of this thread's 64 columns; +512: positions
       // queries are sorted by position: only tiles whose first query is below the tile's last key need a mask
-      const bool need_mask = __float_as_int(lds_f1(smem_u32(col_sm + cs * 128) + 4)) < j0 + kTile - 1;
+      const bool need_mask = __float_as_int(lds_f1(smem_u32(col_sm + cs * 128) + 512)) < j0 + kTile - 1;
       mbar_wait(&bars->d_full[b], (it >> 1) & 1);
       tc_fence_after();
       uint32_t d[2][32];
@@ -261,22 +265,29 @@ colsum_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_constant__ 
 #pragma unroll
       for (int c = 0; c < 2; ++c)
 #pragma unroll
-        for (int i = 0; i < 32; i += 2) {
-          const float4 cc = lds_f4(col + (c * 32 + i) * 8);  // (lse, pos) of two columns
-          float2 x = __ffma2_rn(make_float2(__uint_as_float(d[c][i]), __uint_as_float(d[c][i + 1])), sc2,
-                                make_float2(-cc.x, -cc.z));
-          float2 e;
-          if ((i & 15) < 2 * SX_COLSUM_POLY) {
-            e = cs_ex2_poly2(x);
-          } else {
-            e.x = ex2_approx(x.x);
-            e.y = ex2_approx(x.y);
+        for (int i = 0; i < 32; i += 4) {
+          const float4 l4 = lds_f4(col + (c * 32 + i) * 4);  // lse of four columns
+          float4 p4 = make_float4(0.f, 0.f, 0.f, 0.f);
+          if (need_mask) p4 = lds_f4(col + 512 + (c * 32 + i) * 4);  // their positions (int bits)
+#pragma unroll
+          for (int h2 = 0; h2 < 2; ++h2) {
+            const int ii = i + 2 * h2;
+            const float la = h2 ? l4.z : l4.x, lb = h2 ? l4.w : l4.y;
+            float2 x = __ffma2_rn(make_float2(__uint_as_float(d[c][ii]), __uint_as_float(d[c][ii + 1])), sc2,
+                                  make_float2(-la, -lb));
+            float2 e;
+            if ((ii & 15) < 2 * SX_COLSUM_POLY) {
+              e = cs_ex2_poly2(x);
+            } else {
+              e.x = ex2_approx(x.x);
+              e.y = ex2_approx(x.y);
+            }
+            if (need_mask) {
+              e.x = (__float_as_int(h2 ? p4.z : p4.x) >= j) ? e.x : 0.f;
+              e.y = (__float_as_int(h2 ? p4.w : p4.y) >= j) ? e.y : 0.f;
+            }
+            acc2 = __fadd2_rn(acc2, e);
           }
-          if (need_mask) {
-            e.x = (__float_as_int(cc.y) >= j) ? e.x : 0.f;
-            e.y = (__float_as_int(cc.w) >= j) ? e.y : 0.f;
-          }
-          acc2 = __fadd2_rn(acc2, e);
         }
     }
     // the two halves of a key add up in a fixed order
