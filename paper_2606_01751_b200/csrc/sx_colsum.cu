@@ -111,6 +111,40 @@ __device__ __forceinline__ float2 cs_ex2_poly2(float2 x) {
   return r;
 }
 
+// One consumer thread, one D tile: sum of exp2(s * c - lse_col) over its 64 columns (d[2][32] = raw scores of its key
+// against the 64 (query, head) columns; `col` = shared-memory address of their normalisers, positions 512 B further).
+template <bool kMask>
+__device__ __forceinline__ float2 cs_consume(const uint32_t (&d)[2][32], uint32_t col, float2 sc2, int j, float2 acc2) {
+#pragma unroll
+  for (int c = 0; c < 2; ++c)
+#pragma unroll
+    for (int i = 0; i < 32; i += 4) {
+      const float4 l4 = lds_f4(col + (c * 32 + i) * 4);  // lse of four columns
+      float4 p4 = make_float4(0.f, 0.f, 0.f, 0.f);
+      if (kMask) p4 = lds_f4(col + 512 + (c * 32 + i) * 4);  // their positions (int bits)
+#pragma unroll
+      for (int h2 = 0; h2 < 2; ++h2) {
+        const int ii = i + 2 * h2;
+        const float la = h2 ? l4.z : l4.x, lb = h2 ? l4.w : l4.y;
+        float2 x = __ffma2_rn(make_float2(__uint_as_float(d[c][ii]), __uint_as_float(d[c][ii + 1])), sc2,
+                              make_float2(-la, -lb));
+        float2 e;
+        if ((ii & 15) < 2 * SX_COLSUM_POLY) {
+          e = cs_ex2_poly2(x);
+        } else {
+          e.x = ex2_approx(x.x);
+          e.y = ex2_approx(x.y);
+        }
+        if (kMask) {  // a query sees key j iff its position is >= j
+          e.x = (__float_as_int(h2 ? p4.z : p4.x) >= j) ? e.x : 0.f;
+          e.y = (__float_as_int(h2 ? p4.w : p4.y) >= j) ? e.y : 0.f;
+        }
+        acc2 = __fadd2_rn(acc2, e);
+      }
+    }
+  return acc2;
+}
+
 __global__ void __launch_bounds__(kCsThreads, 2)
 colsum_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_constant__ CUtensorMap tm_k,
               const ColsumParams p) {
@@ -262,33 +296,10 @@ colsum_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_constant__ 
       tmem_wait_ld();
       tc_fence_before();
       mbar_arrive(&bars->d_empty[b]);  // D[b] is in registers: the next-but-one tile may overwrite it
-#pragma unroll
-      for (int c = 0; c < 2; ++c)
-#pragma unroll
-        for (int i = 0; i < 32; i += 4) {
-          const float4 l4 = lds_f4(col + (c * 32 + i) * 4);  // lse of four columns
-          float4 p4 = make_float4(0.f, 0.f, 0.f, 0.f);
-          if (need_mask) p4 = lds_f4(col + 512 + (c * 32 + i) * 4);  // their positions (int bits)
-#pragma unroll
-          for (int h2 = 0; h2 < 2; ++h2) {
-            const int ii = i + 2 * h2;
-            const float la = h2 ? l4.z : l4.x, lb = h2 ? l4.w : l4.y;
-            float2 x = __ffma2_rn(make_float2(__uint_as_float(d[c][ii]), __uint_as_float(d[c][ii + 1])), sc2,
-                                  make_float2(-la, -lb));
-            float2 e;
-            if ((ii & 15) < 2 * SX_COLSUM_POLY) {
-              e = cs_ex2_poly2(x);
-            } else {
-              e.x = ex2_approx(x.x);
-              e.y = ex2_approx(x.y);
-            }
-            if (need_mask) {
-              e.x = (__float_as_int(h2 ? p4.z : p4.x) >= j) ? e.x : 0.f;
-              e.y = (__float_as_int(h2 ? p4.w : p4.y) >= j) ? e.y : 0.f;
-            }
-            acc2 = __fadd2_rn(acc2, e);
-          }
-        }
+      // (two copies of the loop: a per-element `if (need_mask)` would be predicated compares and selects that
+      // take issue slots on every tile, and only the few tiles on the causal diagonal need them)
+      if (need_mask) acc2 = cs_consume<true>(d, col, sc2, j, acc2);
+      else acc2 = cs_consume<false>(d, col, sc2, j, acc2);
     }
     // the two halves of a key add up in a fixed order
     float *xch = reinterpret_cast<float *>(col_sm);  // every column row has been consumed
