@@ -30,8 +30,8 @@ constexpr int kCsOffCol = kCsOffQ + kCsStages * kCsTileBytes;  // float2 [kCsCol
 constexpr int kCsOffBar = kCsOffCol + kCsColStages * 1024;
 constexpr int kCsSmemBytes = kCsOffBar + 256 + 1024;  // 2 CTAs per SM
 #ifndef SX_COLSUM_POLY
-#define SX_COLSUM_POLY 1  // of every 8 pairs of exponentials, this many pairs go to the FMA pipe (0..8);
-                          // measured on C2 / C5: 1 is 2-2.5 % faster than 0, 2 equal, 3 slower
+#define SX_COLSUM_POLY 2  // of every 8 pairs of exponentials, this many pairs go to the FMA pipe (0..8);
+                          // measured on C2 / C4 / C5 (MUFU pipe 77 % busy at 1): 2 and 3 are 1-2 % faster than 1, 4 slower
 #endif
 
 struct ColsumParams {
