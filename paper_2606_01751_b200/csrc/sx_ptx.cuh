@@ -38,12 +38,26 @@ __device__ __forceinline__ bool mbar_try_wait(uint64_t *bar, uint32_t parity) {
       : "memory");
   return ok != 0;
 }
-// Spin with a watchdog: a protocol bug traps (launch error) instead of hanging the GPU.
+// try_wait with a suspend-time hint: the thread may sleep up to `ns` before the instruction returns false (it is
+// woken as soon as the phase completes), so a waiting warp re-issues far fewer instructions
+__device__ __forceinline__ bool mbar_try_wait_hint(uint64_t *bar, uint32_t parity, uint32_t ns) {
+  uint32_t ok;
+  asm volatile(
+      "{\n\t.reg .pred p;\n\t"
+      "mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2, %3;\n\t"
+      "selp.b32 %0, 1, 0, p;\n\t}"
+      : "=r"(ok)
+      : "r"(smem_u32(bar)), "r"(parity), "r"(ns)
+      : "memory");
+  return ok != 0;
+}
+// Spin with a watchdog: a protocol bug traps (launch error) instead of hanging the GPU. The watchdog counts
+// polls (one add and compare per poll; a clock64 comparison had been a third of the waiting warps' instructions).
 __device__ __forceinline__ void mbar_wait(uint64_t *bar, uint32_t parity) {
   if (mbar_try_wait(bar, parity)) return;
-  const long long t0 = clock64();
-  while (!mbar_try_wait(bar, parity)) {
-    if (clock64() - t0 > 4000000000LL) __trap();  // ~2 s
+  uint32_t polls = 0;
+  while (!mbar_try_wait_hint(bar, parity, 2000u)) {
+    if (++polls > (1u << 26)) __trap();  // seconds, whatever the hint is worth
   }
 }
 
@@ -263,9 +277,9 @@ __device__ __forceinline__ bool mbar_try_wait_cluster(uint64_t *bar, uint32_t pa
 // local barrier whose arrivals (also) come from the peer CTA: acquire at cluster scope
 __device__ __forceinline__ void mbar_wait_cluster(uint64_t *bar, uint32_t parity) {
   if (mbar_try_wait_cluster(bar, parity)) return;
-  const long long t0 = clock64();
+  uint32_t polls = 0;
   while (!mbar_try_wait_cluster(bar, parity)) {
-    if (clock64() - t0 > 4000000000LL) __trap();
+    if (++polls > (1u << 26)) __trap();
   }
 }
 // TMA loads whose completion goes to a barrier given by its shared::cluster address (rank 0's barrier)
