@@ -273,7 +273,7 @@ attn_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_constant__ CU
         const int blk_next = (it + 2 < n_items && lane < n_boxes) ? table_entry(it + 2) : 0;
         const bool is_v = kWithPV && (it & 1);
         const int s = it % kStages, u = it / kStages;
-        mbar_wait(&bars->kv_empty[s], (u & 1) ^ 1);
+        mbar_wait_relaxed(&bars->kv_empty[s], (u & 1) ^ 1);   // the ring is several tiles deep: no hurry
         if (lane == 0 && rank == 0) mbar_expect_tx(&bars->kv_full[s], kTileBytes);  // both CTAs' bytes
         __syncwarp();
         if (lane < n_boxes) {

@@ -60,6 +60,16 @@ __device__ __forceinline__ void mbar_wait(uint64_t *bar, uint32_t parity) {
     if (++polls > (1u << 26)) __trap();  // seconds, whatever the hint is worth
   }
 }
+// Wait of a warp that is NOT on the critical path (a TMA producer waiting for a free ring slot several tiles
+// ahead of the consumers): sleep between polls, so that the wait issues a few instructions per microsecond
+// instead of one poll every ~60 cycles (issued instructions of waiting warps cost power on a capped GPU).
+__device__ __forceinline__ void mbar_wait_relaxed(uint64_t *bar, uint32_t parity) {
+  uint32_t polls = 0;
+  while (!mbar_try_wait(bar, parity)) {
+    __nanosleep(200);
+    if (++polls > (1u << 24)) __trap();
+  }
+}
 
 // generic-proxy writes (st.shared) -> visible to the async proxy (TMA / tcgen05.mma operand reads)
 __device__ __forceinline__ void fence_proxy_async_smem() {
