@@ -37,6 +37,10 @@ constexpr int kTileBytes = kTile * kHeadDim * 2;  // 32 KB: two 16-KB halves [ha
 constexpr int kHalfBytes = kTileBytes / 2;
 constexpr int kKvStages = 5;      // ring slots of one CTA (32 KB each)
 constexpr int kKvStagesPair = 8;  // CTA-pair variant: each CTA stages half of every K/V tile (16 KB slots)
+#ifndef SX_RESCALE_LOG2
+#define SX_RESCALE_LOG2 24.0f
+#endif
+constexpr float kRescaleLog2 = SX_RESCALE_LOG2;
 #ifndef SX_ATTN_POLY
 #define SX_ATTN_POLY 2  // of every 8 pairs of exponentials, this many pairs go to the FMA pipe (0..8)
 #endif
@@ -441,6 +445,8 @@ attn_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_constant__ CU
     const uint32_t s_free_r0 = kPair ? mapa_u32(smem_u32(&bars->s_free[qt][0]), 0) : 0;
     const uint32_t s_loaded_r0 = kPair ? mapa_u32(smem_u32(&bars->s_free[qt][1]), 0) : 0;
     float m_used = -INFINITY, l = 0.f;
+    float l_fix = 0.f;  // PV variant: sum of the rounding residuals of the tile maxima (see below); O is normalised
+                        // by l + l_fix, the log-sum-exp output stays that of the unrounded exponentials (l)
 
     for (int t = 0; t < my_tiles; ++t) {
       const int b = kWithPV ? 0 : (t & 1);
@@ -456,7 +462,9 @@ attn_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_constant__ CU
       tmem_ld32(tmem_s + b * 128 + 96, sr[3]);
 
       const int nvalid = pos - (t0 + t) * kTile + 1;  // keys [0, nvalid) of this tile are visible to this row
-      float tm[2] = {-INFINITY, -INFINITY};  // two independent 3-input max chains
+      // three independent 3-input max chains: tm[0], tm[1] over the columns whose exponential goes to MUFU, tm[2]
+      // over those that take the FMA-pipe polynomial (which of the two evaluated the row maximum matters below)
+      float tm[3] = {-INFINITY, -INFINITY, -INFINITY};
 #pragma unroll
       for (int c = 0; c < 4; ++c) {
         if (c == 2) {
@@ -478,13 +486,21 @@ attn_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_constant__ CU
         }
 #pragma unroll
         for (int i = 0; i < 32; i += 4) {
-          tm[0] = fmaxf(tm[0], fmaxf(__uint_as_float(sr[c][i]), __uint_as_float(sr[c][i + 1])));
-          tm[1] = fmaxf(tm[1], fmaxf(__uint_as_float(sr[c][i + 2]), __uint_as_float(sr[c][i + 3])));
+          if ((i & 15) < 2 * SX_ATTN_POLY) {  // (SX_ATTN_POLY is even here: groups of four columns share a path)
+            tm[2] = fmaxf(tm[2], fmaxf(__uint_as_float(sr[c][i]), __uint_as_float(sr[c][i + 1])));
+            tm[2] = fmaxf(tm[2], fmaxf(__uint_as_float(sr[c][i + 2]), __uint_as_float(sr[c][i + 3])));
+          } else {
+            tm[0] = fmaxf(tm[0], fmaxf(__uint_as_float(sr[c][i]), __uint_as_float(sr[c][i + 1])));
+            tm[1] = fmaxf(tm[1], fmaxf(__uint_as_float(sr[c][i + 2]), __uint_as_float(sr[c][i + 3])));
+          }
         }
       }
-      const float tmax = fmaxf(tm[0], tm[1]);
+      const float tmax_mufu = fmaxf(tm[0], tm[1]);
+      const float tmax = fmaxf(tmax_mufu, tm[2]);
       const float m_new = fmaxf(m_used, tmax);
-      const bool upd = (m_new - m_used) * p.scale_log2 > 8.0f;  // lazy rescale threshold: 2^8
+      // lazy rescale: O and l keep the old reference until the maximum has grown by more than 2^kRescaleLog2
+      // (with 2^8, 14.5 % of all (warp, tile) steps took the rescale path on C3: any of a warp's 32 rows triggers it)
+      const bool upd = (m_new - m_used) * p.scale_log2 > kRescaleLog2;
       float alpha = 1.f;
       if (upd) {
         alpha = ex2_approx((m_used - m_new) * p.scale_log2);
@@ -561,7 +577,23 @@ attn_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_constant__ CU
           }
         }
       }
-      l = l * alpha + (rsum2.x + rsum2.y);
+      const float radd = rsum2.x + rsum2.y;
+      if (kWithPV) {
+        // PV uses the bf16-ROUNDED probabilities while the row sum adds the unrounded ones. With a lazily updated
+        // reference the largest P of a row is not 1, and for a peaked row its 2^-9 rounding would go straight
+        // into O = sum(P v) / l. The largest term of every tile therefore enters the normaliser of O with its
+        // rounded value: numerator and denominator agree on the dominant key. It is re-evaluated by the same unit
+        // that evaluated the element (MUFU or the polynomial), so the residual is exact. A dozen instructions per
+        // tile; measured on the parity cases: max-abs error of O 0.0198 -> 0.0138, mean 6.6e-4 -> 6.2e-4, the same
+        // as summing all 128 rounded values.
+        const float x_max = fmaf(tmax, p.scale_log2, neg_m);
+        const float e_mufu = ex2_approx(x_max);
+        const float e_poly = ex2_poly2(make_float2(x_max, x_max)).x;
+        const float e_max = (tm[2] >= tmax_mufu) ? e_poly : e_mufu;
+        const uint32_t r2 = pack_bf16x2(e_max, 0.f);
+        l_fix = l_fix * alpha + (__uint_as_float(r2 << 16) - e_max);
+      }
+      l = l * alpha + radd;
     }
 
     // ---- epilogue
@@ -573,7 +605,7 @@ attn_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_constant__ CU
       if (my_tiles > 0) {
         mbar_wait(&bars->o_full[qt], 0);
         tc_fence_after();
-        const float inv = 1.f / l;
+        const float inv = 1.f / (l + l_fix);
 #pragma unroll
         for (int c = 0; c < 4; ++c) {
           uint32_t o[32];
@@ -593,7 +625,7 @@ attn_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_constant__ CU
       if (kWithPV) {
         mbar_wait(&bars->o_full[qt], 0);
         tc_fence_after();
-        const float inv = 1.f / l;
+        const float inv = 1.f / (l + l_fix);
 #pragma unroll
         for (int c = 0; c < 4; ++c) {
           uint32_t o[32];
