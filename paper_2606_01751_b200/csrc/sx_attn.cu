@@ -19,7 +19,8 @@
 //     previous S in registers, the lower one after the PV MMAs that read P.
 //   * warps 8 and 10 = TMA producers (K tiles / V tiles), warp 9 = MMA issuer (one elected lane);
 //     warps 0-3 / 4-7 = softmax warpgroups of query tile 0 / 1: thread = one row of S (tcgen05.ld), fp32 online softmax in the
-//     exp2 domain with lazy rescale (O is rescaled only when the row maximum grew by more than 2^8),
+//     exp2 domain with lazy rescale (O is rescaled only when the row maximum grew by more than 2^24; the
+//     largest term of every tile enters O's normaliser with its bf16-rounded value, see the softmax loop),
 //     a fixed fraction of the exponentials evaluated on the FMA pipe (Cody-Waite + cubic) because
 //     MUFU.EX2 (16/clk/SM) would otherwise co-limit the tensor pipe. The two tiles ping-pong:
 //     while one tile's softmax runs, the tensor pipe executes the other tile's PV and next QK^T.
