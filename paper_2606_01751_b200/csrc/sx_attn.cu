@@ -45,6 +45,7 @@ constexpr float kRescaleLog2 = SX_RESCALE_LOG2;
 #ifndef SX_ATTN_POLY
 #define SX_ATTN_POLY 2  // of every 8 pairs of exponentials, this many pairs go to the FMA pipe (0..8)
 #endif
+static_assert(SX_ATTN_POLY % 2 == 0, "groups of four S columns must share one exponential path (row-maximum tracking)");
 
 struct AttnParams {
   const int32_t *rows;      // [total_rows] positions, or nullptr (row n of request r = position n - rows_off[r])
