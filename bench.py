@@ -37,7 +37,7 @@ from paper_2606_01751_b200 import workloads as wl  # noqa: E402
 
 METRIC = "sparse_recompute_context_tokens_per_s"
 UNIT = "tokens/s"
-CTA_PAIR = False  # --cta-pair: stage (c) runs with the SX_ATTN_CTA_PAIR flag
+CTA_PAIR = None   # None: library rule; --cta-pair / --single-cta force SX_ATTN_CTA_PAIR / SX_ATTN_SINGLE_CTA
 L_STACK, THRESHOLD = 32, 4
 
 
@@ -308,7 +308,8 @@ def measure(cfg, steps, warmup, ctx, want_e2e=True, want_clocks=True):
     # a kernel timed alone between L2 flushes (single-layer configs) is held against the burst peak, the
     # attention launches inside the long C3 step against the sustained one (B200_PROFILING.md)
     tf_peak, tf_src = (peaks["tf_sustained"], "sustained") if stack else (peaks["tf_burst"], "burst")
-    roofline = {"bound": "tensor", "kernel": "attn_kernel<true%s> (sx_sparse_attn)" % (", cta pair" if CTA_PAIR else ""), "achieved": round(achieved, 1),
+    roofline = {"bound": "tensor", "kernel": "attn_kernel<true%s> (sx_sparse_attn)" % (
+                    ", cta pair" if (CTA_PAIR or (CTA_PAIR is None and lay.num_reqs == 1)) else ""), "achieved": round(achieved, 1),
                 "peak": tf_peak, "unit": "TFLOP/s", "frac": round(achieved / tf_peak, 4),
                 "peak_src": "%s bf16 %s" % (peaks["src"], tf_src),
                 # dram__bytes_read + dram__bytes_write per attention launch, averaged over the 32 launches of a C3 step
@@ -703,10 +704,12 @@ def main():
     ap.add_argument("--no-cpu", action="store_true")
     ap.add_argument("--no-others", action="store_true", help="skip the short runs of the other BASELINE configs")
     ap.add_argument("--cta-pair", action="store_true",
-                    help="stage (c) with SX_ATTN_CTA_PAIR (2-CTA clusters, tcgen05.mma.cta_group::2)")
+                    help="force stage (c) onto 2-CTA clusters (SX_ATTN_CTA_PAIR, tcgen05.mma.cta_group::2)")
+    ap.add_argument("--single-cta", action="store_true",
+                    help="force stage (c) onto the single-CTA kernel (SX_ATTN_SINGLE_CTA); default: library rule")
     args = ap.parse_args()
     global CTA_PAIR
-    CTA_PAIR = args.cta_pair
+    CTA_PAIR = True if args.cta_pair else (False if args.single_cta else None)
     if args.impl == "reference":
         run_reference(args)
     else:

@@ -180,7 +180,8 @@ sx_status sx_score_select_ex(const sx_pool *pool, const sx_batch *batch, const v
  * ("excluded from the current prefill computation"): visible as a key everywhere, never a candidate, never a query
  * row. With prefix hits, full-attention layers are run in mode 0 with the non-prefix positions as rows_R. */
 #define SX_ATTN_CUDA_CORE 2 /* flag for sx_sparse_attn's mode: CUDA-core kernels for small row sets */
-#define SX_ATTN_CTA_PAIR 4  /* flag for sx_sparse_attn's mode: 2-CTA clusters with tcgen05.mma.cta_group::2 */
+#define SX_ATTN_CTA_PAIR 4  /* flag for sx_sparse_attn's mode: force 2-CTA clusters (tcgen05.mma.cta_group::2) */
+#define SX_ATTN_SINGLE_CTA 8 /* flag for sx_sparse_attn's mode: force the single-CTA tensor-core kernel */
 
 /* (c) Alg. 1 l.546-548 (sparse) / l.507-511 (full). mode 0: query rows are rows_R (as produced by
  * sx_score_select); mode 1: rows_R and rows_off are ignored, every position of every request is
@@ -197,11 +198,12 @@ sx_status sx_score_select_ex(const sx_pool *pool, const sx_batch *batch, const v
  *   - mode | SX_ATTN_CUDA_CORE: row sets with total_rows * g < 64 * num_reqs (fewer than 64 query rows per
  *     KV head on average; g = Hq/Hkv <= 32) take CUDA-core split-KV kernels, fp32 FMA throughout (the rule of
  *     BASELINE.json north_star; measured slower than the padded tensor-core tile on B200). Uses ws.
- *   - mode | SX_ATTN_CTA_PAIR: when the tensor-core path runs without key splits, clusters of two CTAs work on
- *     adjacent pairs of query tiles with M = 256 MMAs (tcgen05.mma.cta_group::2): every K/V tile is fetched once
- *     per cluster, half into each CTA. Same arithmetic per row, hence the same results as the default; measured
- *     0.3-0.5 % faster on the power-capped 32-layer stack and 1-7 % slower on single layers (S10), so
- *     it is opt-in. Ignored where key splits or the CUDA-core kernels apply.
+ *   - CTA pairs: when the tensor-core path runs without key splits it exists in two forms with the same arithmetic
+ *     per row (hence the same results): one CTA per pair of query tiles, or clusters of two CTAs on adjacent pairs
+ *     with M = 256 MMAs (tcgen05.mma.cta_group::2), where every K/V tile is fetched once per cluster, half into
+ *     each CTA. Measured (S10): clusters are 1-2 % faster for a batch of ONE request (long uniform
+ *     launches) and 5-6 % slower for batches of several requests, so that is the default rule;
+ *     mode | SX_ATTN_CTA_PAIR / mode | SX_ATTN_SINGLE_CTA force one or the other.
  * All are deterministic and meet the same tolerance against fp64. */
 sx_status sx_sparse_attn(const sx_pool *pool, const sx_batch *batch, int32_t mode, const void *q,
                          const int32_t *rows_R, const int32_t *rows_off, int32_t total_rows,

@@ -241,9 +241,9 @@ def rows_capacity(lay, overflow_blocks: int, tail_tokens: int) -> np.ndarray:
 def sparse_attn(pool: DevicePool, batch: DeviceBatch, q: torch.Tensor, out: torch.Tensor,
                 rows_R: Optional[torch.Tensor] = None, rows_off: Optional[torch.Tensor] = None,
                 total_rows: Optional[int] = None, lse: Optional[torch.Tensor] = None, full: bool = False,
-                cuda_core: bool = False, cta_pair: bool = False, stream=None):
-    """Stage (c), Alg. 1 l.546-548 (sparse rows) / l.507-511 (full=True). cuda_core / cta_pair = the
-    SX_ATTN_CUDA_CORE / SX_ATTN_CTA_PAIR mode flags of include/sparsex.h."""
+                cuda_core: bool = False, cta_pair: Optional[bool] = None, stream=None):
+    """Stage (c), Alg. 1 l.546-548 (sparse rows) / l.507-511 (full=True). cuda_core = SX_ATTN_CUDA_CORE;
+    cta_pair: None = the library's rule, True / False = SX_ATTN_CTA_PAIR / SX_ATTN_SINGLE_CTA (include/sparsex.h)."""
     global LAUNCHES
     ws = batch.workspace(pool)
     n = int(q.shape[0]) if total_rows is None else int(total_rows)
@@ -254,7 +254,7 @@ def sparse_attn(pool: DevicePool, batch: DeviceBatch, q: torch.Tensor, out: torc
         small = grid < 148 and min(148 // grid, ((batch.c.max_seq_len + 127) // 128) // 2) > 1
     LAUNCHES += (2 if small else 1) if n else 0
     assert q.is_contiguous() and out.is_contiguous()
-    _check(load().sx_sparse_attn(ctypes.byref(pool.c), ctypes.byref(batch.c), (1 if full else 0) | (2 if cuda_core else 0) | (4 if cta_pair else 0), _ptr(q),
+    _check(load().sx_sparse_attn(ctypes.byref(pool.c), ctypes.byref(batch.c), (1 if full else 0) | (2 if cuda_core else 0) | (0 if cta_pair is None else (4 if cta_pair else 8)), _ptr(q),
                                  _ptr(rows_R), _ptr(rows_off), n, _ptr(out), _ptr(lse), _ptr(ws), ws.numel(),
                                  _stream(stream)), "sx_sparse_attn")
 

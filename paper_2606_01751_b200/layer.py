@@ -30,7 +30,7 @@ class GpuLayer:
     def __init__(self, lay, lt, device="cuda", batch: Optional[sx.DeviceBatch] = None):
         self.lay = lay
         self.dev = torch.device(device)
-        self.cta_pair = False   # SX_ATTN_CTA_PAIR for every attention call of this layer
+        self.cta_pair = None    # None: library rule; True / False: SX_ATTN_CTA_PAIR / SX_ATTN_SINGLE_CTA
         self.batch = batch if batch is not None else sx.DeviceBatch(lay, self.dev)
         # lt: workloads.LayerTensors (numpy bit patterns) or any object whose pool_k / pool_v / q_full /
         # k_fresh / v_fresh are already 2-byte device tensors
