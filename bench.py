@@ -313,8 +313,8 @@ def measure(cfg, steps, warmup, ctx, want_e2e=True, want_clocks=True):
                 "peak": tf_peak, "unit": "TFLOP/s", "frac": round(achieved / tf_peak, 4),
                 "peak_src": "%s bf16 %s" % (peaks["src"], tf_src),
                 # dram__bytes_read + dram__bytes_write per attention launch, averaged over the 32 launches of a C3 step
-                # (28 sparse x 377.7 MB + 4 full x 2163.4 MB; ncu --set full, profiles/r1_v3_kernels_ncu_full.md)
-                "traffic": 600.9e6 if stack else None, "traffic_unit": "B per launch (ncu capture)",
+                # (28 sparse x 420.4 MB + 4 full x 2108.1 MB; ncu --set full, profiles/r1_v3e_launches_c3.md)
+                "traffic": 631.3e6 if stack else None, "traffic_unit": "B per launch (ncu capture)",
                 "algorithmic_bytes_per_launch": round(float(sum(
                     4.0 * int(n) * hkv * 128 for n in lay.seq_len) * n_layers +
                     4.0 * (n_rows_total * n_sparse + T * n_full) * hq * 128) / n_layers, 1),
