@@ -4,9 +4,12 @@ seeded workloads C2..C5, layer 0, so that the full-size GPU parity tests replay 
 the fp64 oracle (minutes per config). Calls only oracle/ (through tests/helpers.py) and the seeded input
 generator; nothing here touches the CUDA path.
 
-    python tests/golden/make_carve.py [C2 C3 C4 C5]
+    python tests/golden/make_carve.py [C2 C3 C4 C5 C3_L3]
 
 Each line: physical block, row in block, scale applied to that key row (all KV heads), in application order.
+C3_L3: the margin of the BOUNDARY-layer selection of C3 in paper mode (layer index 3, readings A11/A16): that
+selection reads a pool whose keys are all fresh, so the carve rescales rows of K_fresh of layer 3; each line is
+batch token index, scale (helpers.carve_margins_fresh / apply_carve_fresh).
 """
 import os
 import sys
@@ -16,13 +19,26 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 sys.path.insert(0, os.path.dirname(HERE))
 sys.path.insert(0, os.path.dirname(os.path.dirname(HERE)))
 
-from helpers import carve_margins  # noqa: E402
+from helpers import carve_margins, carve_margins_fresh  # noqa: E402
 from paper_2606_01751_b200 import workloads as wl  # noqa: E402
 
 
 def main():
-    for name in (sys.argv[1:] or ["C2", "C3", "C4", "C5"]):
+    for name in (sys.argv[1:] or ["C2", "C3", "C4", "C5", "C3_L3"]):
         t0 = time.time()
+        if name == "C3_L3":
+            lay = wl.CONFIGS["C3"]()
+            lt = wl.build_layer(lay, 3)
+            log = []
+            hist = carve_margins_fresh(lay, lt, log=log)
+            with open(os.path.join(HERE, "carve_C3_L3.txt"), "w") as f:
+                f.write("# margin carve of the boundary-layer selection: workloads.CONFIGS['C3'](), layer 3, K_fresh rows, "
+                        "tau = 1e-3; band sizes per iteration %r\n" % (hist,))
+                f.write("# written by tests/golden/make_carve.py (fp64 oracle only); columns: batch token index, scale\n")
+                for tok, scale in log:
+                    f.write("%d %.2f\n" % (tok, scale))
+            print(name, hist, len(log), "ops, %.0f s" % (time.time() - t0), flush=True)
+            continue
         lay = wl.CONFIGS[name]()
         lt = wl.build_layer(lay, 0)
         log = []

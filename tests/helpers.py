@@ -108,6 +108,105 @@ def carve_margins(lay: wl.Layout, lt: wl.LayerTensors, tau: float = 1e-3, max_it
     raise RuntimeError("margin carving did not converge: %r" % hist)
 
 
+def oracle_scores_full_layer(lay: wl.Layout, lt: wl.LayerTensors):
+    """fp64 scores of every request on the pool state the BOUNDARY-layer selection sees (Alg. 1 l.507-531,
+    readings A11/A16): the layer ran in full mode, so every position holds its fresh key."""
+    pk, pv = lt.pool_k.copy(), lt.pool_v.copy()
+    kt, vt = lay.k_block_table.copy(), lay.v_block_table.copy()
+    orc.realign(pk, pv, kt, vt, lay.segments, lay.src_blocks, lay.rope_theta, lay.rope_style)
+    out = []
+    for r in range(lay.num_reqs):
+        t, o = int(lay.seq_len[r]), int(lay.tok_off[r])
+        orc.scatter_kv(pk, pv, kt, vt, None, r, np.arange(t, dtype=np.int32), lt.k_fresh[o:o + t], lt.v_fresh[o:o + t])
+        nidx = lay.new_idx[lay.new_off[r]:lay.new_off[r + 1]]
+        out.append(orc.scores(pk, kt[r], t, lt.q_full[o + nidx], nidx, lay.num_q_heads))
+    return out
+
+
+def carve_margins_fresh(lay: wl.Layout, lt: wl.LayerTensors, tau: float = 1e-3, max_iter: int = 20, log=None,
+                        widen_later: float = 1.5):
+    """carve_margins for the boundary-layer selection of paper mode (readings A10/A11/A16): that selection
+    reads a pool in which every key is FRESH (the layer ran full attention), so the margin at the rank-k cut is
+    carved into lt.k_fresh: the fresh key row of every cached position whose fp64 score lies within tau of the
+    cut is rescaled (x1.25 above, x0.8 below) and re-rounded to bf16, until the band is empty and the gap is
+    >= 2 tau. `log` receives (batch token index, scale) in application order (replay: apply_carve_fresh)."""
+    hist = []
+    for it in range(max_iter):
+        widen = 3.0 if it == 0 else widen_later
+        sc = oracle_scores_full_layer(lay, lt)
+        band_total = 0
+        for r in range(lay.num_reqs):
+            k = int(lay.k_per_req[r])
+            cand = np.nonzero(lay.cached_mask(r))[0]
+            if k <= 0 or k >= len(cand):
+                continue
+            s = sc[r][cand]
+            order = np.lexsort((cand, -s))
+            c = 0.5 * (s[order[k - 1]] + s[order[k]])
+            gap_ok = (s[order[k - 1]] - s[order[k]]) >= 2 * tau * c
+            if gap_ok and not np.any(np.abs(s - c) <= tau * c):
+                continue
+            band = np.nonzero(np.abs(s - c) <= widen * tau * c)[0]
+            if len(band) == 0:
+                band = np.asarray([order[k - 1], order[k]])
+            band_total += len(band)
+            o = int(lay.tok_off[r])
+            for bi in band.tolist():
+                tok = o + int(cand[bi])
+                scale = 1.25 if s[bi] > c else 0.8
+                lt.k_fresh[tok] = orc.f64_to_bf16(orc.bf16_to_f64(lt.k_fresh[tok]) * scale)
+                if log is not None:
+                    log.append((tok, scale))
+        hist.append(band_total)
+        if band_total == 0:
+            return hist
+    raise RuntimeError("margin carving (fresh keys) did not converge: %r" % hist)
+
+
+def apply_carve_fresh(lt: wl.LayerTensors, ops):
+    """Replay a fresh-key carve log: k_fresh[token] (every KV head) times scale, re-rounded to bf16, in order."""
+    for tok, scale in ops:
+        lt.k_fresh[tok] = orc.f64_to_bf16(orc.bf16_to_f64(lt.k_fresh[tok]) * scale)
+
+
+def load_carve_fresh(path):
+    ops = []
+    with open(path) as f:
+        for ln in f:
+            if ln.startswith("#") or not ln.strip():
+                continue
+            a, b = ln.split()
+            ops.append((int(a), float(b)))
+    return ops
+
+
+def edge_rows(rows: np.ndarray, n_spread: int, rows_per_pair: int, every: int = 7) -> np.ndarray:
+    """Indices into the sorted row list `rows` (one request) chosen to hit the launch geometry of stage (c) at
+    full size: a spread of n_spread rows, plus -- for every `every`-th CTA (rows_per_pair rows of R per CTA; an odd
+    stride, so that both CTAs of a 2-CTA cluster and both parities of 64-row CTAs against 128-key tiles occur) and
+    for the last two CTAs (the last cluster, whose odd pair may be empty) -- the CTA's first row, the last row
+    of its first query tile, the first row of its second tile and its last row, plus every listed row whose
+    POSITION is 128k-1, 128k or 128k+1 for the key-tile edges k of that CTA's last row."""
+    n = len(rows)
+    if n == 0:
+        return np.zeros(0, np.int64)
+    pick = set(np.unique(np.linspace(0, n - 1, min(n, n_spread)).astype(np.int64)).tolist())
+    n_cta = (n + rows_per_pair - 1) // rows_per_pair
+    ctas = sorted(set(list(range(0, n_cta, every)) + [max(0, n_cta - 2), n_cta - 1]))
+    half = rows_per_pair // 2
+    for c in ctas:
+        lo, hi = c * rows_per_pair, min(n, (c + 1) * rows_per_pair)
+        for i in (lo, lo + half - 1, lo + half, hi - 1):
+            if lo <= i < hi:
+                pick.add(int(i))
+        # rows of this CTA sitting on a 128-key tile edge
+        pos = rows[lo:hi].astype(np.int64)
+        m = ((pos % 128) == 127) | ((pos % 128) == 0) | ((pos % 128) == 1)
+        for i in np.nonzero(m)[0][:6].tolist() + np.nonzero(m)[0][-3:].tolist():
+            pick.add(int(lo + i))
+    return np.asarray(sorted(pick), dtype=np.int64)
+
+
 def apply_carve(lt: wl.LayerTensors, ops):
     """Replay a carve log: key row (block, row) of every KV head times scale, re-rounded to bf16, in order."""
     for blk, row, scale in ops:
