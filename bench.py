@@ -272,7 +272,7 @@ def measure(cfg, steps, warmup, ctx, want_e2e=True, want_clocks=True):
     for _ in range(max(warmup, 3)):
         step()
     barrier()
-    launches0 = sx.LAUNCHES
+    launches0 = sx.launch_count()
     ev["on"] = True
     sampler = ClockSampler(local)
     if rank == 0 and want_clocks:
@@ -290,7 +290,7 @@ def measure(cfg, steps, warmup, ctx, want_e2e=True, want_clocks=True):
         step_ms.append(a.elapsed_time(b))
     clocks = sampler.stop() if (rank == 0 and want_clocks) else None
     ev["on"] = False
-    launches = sx.LAUNCHES - launches0
+    launches = sx.launch_count() - launches0     # kernels launched in the timed region, counted inside libsparsex.so
     t_ms = du.max_over_ranks(float(np.sum(step_ms)), dev)
     ms_per_step = t_ms / steps
     stage_ms = {k: float(sum(x.elapsed_time(y) for x, y in v)) / steps for k, v in ev.items() if k != "on"}

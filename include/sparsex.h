@@ -13,8 +13,12 @@
  *
  * Conventions
  *   - "device" pointers are CUDA device memory owned by the caller; "host" values are plain integers
- *     in the structs below. The library allocates nothing, frees nothing and keeps no state.
- *   - Every call is asynchronous on `stream` and never synchronises the device. A non-zero status
+ *     in the structs below. The library allocates nothing and frees nothing. The only process-wide state it
+ *     keeps is (i) a bounded cache of encoded TMA tensor maps keyed by (base pointer, shape) -- a pure function
+ *     of its key, so it cannot go stale -- (ii) the kernel-launch counter of sx_launch_count() and (iii) the
+ *     thread-local text of sx_last_error(). All entry points may be called from several threads.
+ *   - Every stage call is asynchronous on `stream` and never synchronises the device (the two validation calls
+ *     sx_check_batch / sx_check_rows do: they are for descriptor construction time). A non-zero status
  *     means nothing was launched (argument errors) or a launch failed (SX_ERR_CUDA);
  *     sx_last_error() then returns a thread-local description.
  *   - The workspace `ws` is scratch that calls write: calls that may run concurrently (different streams)
@@ -118,7 +122,10 @@ sx_status sx_rope_realign(const sx_pool *pool, const sx_batch *batch, void *ws, 
  * num_blocks / num_kv_heads), all addressed through the same batch descriptor (block tables and segment map
  * are per request, not per layer). The re-alignment reads only cached source pages, never an output of the
  * current step, so it can be completed for every layer of the scheduling batch before the first layer runs
- * ("completes RoPE alignment for all requests in a scheduling batch", 331). */
+ * ("completes RoPE alignment for all requests in a scheduling batch", 331).
+ * Not available with copy-on-write (batch->cow_private != NULL and num_layers > 1 -> SX_ERR_UNSUPPORTED): the
+ * COW state is the v_block_table, which then belongs to ONE layer (page contents are per layer, so every layer
+ * needs its own table and its own sx_batch; see sx_scatter_kv). */
 sx_status sx_rope_realign_layers(const sx_pool *pools, int32_t num_layers, const sx_batch *batch, void *ws,
                                  size_t ws_bytes, sx_stream stream);
 
@@ -128,7 +135,8 @@ sx_status sx_rope_realign_layers(const sx_pool *pools, int32_t num_layers, const
  *   K[k_block_table[r][p/16]][:][p%16][:] = k_fresh[n],  V likewise through v_block_table.
  * Copy-on-write (batch->cow_private != NULL): before any row is written, a touched page whose
  * table entry differs from its reserved private page (>= 0) is copied there and the entry is
- * flipped (K and V tables independently). Rows not listed are untouched.
+ * flipped (K and V tables independently). Rows not listed are untouched. The flipped table describes THIS
+ * layer's pool only: under COW every layer of a stack has its own block tables (its own sx_batch).
  * max_rows (host) >= rows_off[num_reqs] sizes the grid. */
 sx_status sx_scatter_kv(const sx_pool *pool, const sx_batch *batch, const void *k_fresh,
                         const void *v_fresh, const int32_t *rows, const int32_t *rows_off,
@@ -208,6 +216,24 @@ sx_status sx_score_select_ex(const sx_pool *pool, const sx_batch *batch, const v
 sx_status sx_sparse_attn(const sx_pool *pool, const sx_batch *batch, int32_t mode, const void *q,
                          const int32_t *rows_R, const int32_t *rows_off, int32_t total_rows,
                          void *out, float *lse, void *ws, size_t ws_bytes, sx_stream stream);
+
+/* Validation of the DEVICE-resident descriptor arrays, which the stage calls cannot see from the host mirrors:
+ * seq_len / tok_off / new_off consistent with the host counts; new_idx strictly ascending inside its request;
+ * every segment's len / old_pos / new_pos a positive multiple of block_size, src_off the running
+ * sum of len / block_size, segments sorted by (req, new_pos) and non-overlapping, inside the request's pages;
+ * src_blocks, the block-table entries of used pages and cow_private inside the pool. One small kernel, one error
+ * word copied back: this call SYNCHRONISES `stream`. Returns SX_OK or SX_ERR_INVALID_ARG with the failing check
+ * and its index in sx_last_error(). A descriptor that fails here would corrupt pages in the stage calls. Uses ws. */
+sx_status sx_check_batch(const sx_pool *pool, const sx_batch *batch, void *ws, size_t ws_bytes, sx_stream stream);
+
+/* Same for a row list handed to sx_scatter_kv / sx_sparse_attn: rows_off ascending from 0 with
+ * rows_off[num_reqs] <= max_rows; rows strictly ascending inside [0, seq_len) of their request.
+ * SYNCHRONISES `stream`. Uses ws. */
+sx_status sx_check_rows(const sx_pool *pool, const sx_batch *batch, const int32_t *rows, const int32_t *rows_off,
+                        int32_t max_rows, void *ws, size_t ws_bytes, sx_stream stream);
+
+/* Number of kernels this library has launched in the process so far (diagnostic; monotone, thread safe). */
+uint64_t sx_launch_count(void);
 
 /* Thread-local text of the last error returned on this thread ("" if none). Static storage. */
 const char *sx_last_error(void);

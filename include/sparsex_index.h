@@ -71,8 +71,11 @@ int32_t sx_index_release(sx_index *ix, const int32_t *src_blocks, int32_t n);
 
 /* Utilisation-triggered eviction ("when KV Cache block utilization exceeds 90 % ... delete the
  * least-referenced blocks from the frozen-block pool"): while used_blocks / total_blocks > threshold, remove
- * unreferenced frozen entries in order (hit count ascending, insertion order ascending); each removal frees
- * one physical block. evicted_out (capacity max_out) receives the physical ids. Returns how many were evicted. */
+ * physical blocks whose virtual blocks are ALL frozen and unreferenced (several namespaces / token views may sit
+ * on one physical block; one referenced or non-frozen view keeps the block), in order (hit count summed over the
+ * block's views ascending, then its oldest insertion first). All views of an evicted block leave the index and
+ * the block is reported once: evicted_out (capacity max_out) receives the distinct physical ids. Returns how
+ * many blocks were freed. */
 int32_t sx_index_evict(sx_index *ix, int32_t used_blocks, int32_t total_blocks, double threshold,
                        int32_t *evicted_out, int32_t max_out);
 

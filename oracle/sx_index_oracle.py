@@ -6,8 +6,9 @@ the definition "reusable only when both token IDs and the extra key match" (PAPE
 
   virtual block: physical block id + position of the block's first token when cached.
   frozen block: survives reference count 0; leaves through erase or eviction only.
-  eviction: above the utilisation threshold remove the least-referenced unreferenced
-                  frozen entries first (ties: older first); one physical block freed per removal.
+  eviction: above the utilisation threshold free the least-referenced physical blocks whose
+                  views are ALL frozen and unreferenced (ties: older first); every view of a freed block leaves,
+                  the block is reported once (a block that another namespace still references is never freed).
 """
 from __future__ import annotations
 
@@ -78,10 +79,19 @@ class IndexOracle:
         return removed
 
     def evict(self, used, total, threshold=0.9, max_out=1 << 16):
-        cand = sorted(((e["hits"], e["serial"], k) for k, e in self.d.items() if e["frozen"] and e["refs"] == 0))
+        by_block = {}
+        for k, e in self.d.items():
+            by_block.setdefault(e["block"], []).append(k)
+        cand = []
+        for b, keys in by_block.items():
+            ents = [self.d[k] for k in keys]
+            if all(e["frozen"] and e["refs"] == 0 for e in ents):
+                cand.append((sum(e["hits"] for e in ents), min(e["serial"] for e in ents), b))
         out = []
-        for _, _, k in cand:
+        for _, _, b in sorted(cand):
             if len(out) >= max_out or (used - len(out)) / total <= threshold:
                 break
-            out.append(self.d.pop(k)["block"])
+            for k in by_block[b]:
+                del self.d[k]
+            out.append(b)
         return out

@@ -23,9 +23,9 @@ _LIB_PATH = os.path.join(_HERE, "libsparsex.so")
 _lib = None
 
 SX_OK = 0
-LAUNCHES = 0   # kernels launched through this binding (each stage call adds its known kernel count)
 EXPORTS = ["sx_workspace_size", "sx_rope_realign", "sx_rope_realign_layers", "sx_scatter_kv", "sx_score_select",
-           "sx_score_select_ex", "sx_sparse_attn", "sx_last_error", "sx_version"]
+           "sx_score_select_ex", "sx_sparse_attn", "sx_check_batch", "sx_check_rows", "sx_launch_count",
+           "sx_last_error", "sx_version"]
 
 
 class SxPool(ctypes.Structure):
@@ -78,6 +78,12 @@ def load():
         lib.sx_score_select_ex.argtypes = [PP, PB, vp, vp, i32, vp, vp, i32, i32, vp, vp, vp, vp, vp, sz, vp]
         lib.sx_sparse_attn.restype = ctypes.c_int
         lib.sx_sparse_attn.argtypes = [PP, PB, i32, vp, vp, vp, i32, vp, vp, vp, sz, vp]
+        lib.sx_check_batch.restype = ctypes.c_int
+        lib.sx_check_batch.argtypes = [PP, PB, vp, sz, vp]
+        lib.sx_check_rows.restype = ctypes.c_int
+        lib.sx_check_rows.argtypes = [PP, PB, vp, vp, i32, vp, sz, vp]
+        lib.sx_launch_count.restype = ctypes.c_uint64
+        lib.sx_launch_count.argtypes = []
         lib.sx_last_error.restype = ctypes.c_char_p
         lib.sx_version.restype = ctypes.c_char_p
         _lib = lib
@@ -86,6 +92,11 @@ def load():
 
 def version() -> str:
     return load().sx_version().decode()
+
+
+def launch_count() -> int:
+    """Kernels the library has launched in this process so far (counted inside libsparsex.so)."""
+    return int(load().sx_launch_count())
 
 
 def _check(rc: int, what: str):
@@ -157,6 +168,22 @@ class DeviceBatch:
         return self._ws
 
 
+def check_batch(pool: DevicePool, batch: DeviceBatch, stream=None):
+    """Validate the device-resident descriptor arrays (sx_check_batch; synchronises). Raises SparseXError."""
+    ws = batch.workspace(pool)
+    _check(load().sx_check_batch(ctypes.byref(pool.c), ctypes.byref(batch.c), _ptr(ws), ws.numel(), _stream(stream)),
+           "sx_check_batch")
+
+
+def check_rows(pool: DevicePool, batch: DeviceBatch, rows: torch.Tensor, rows_off: torch.Tensor,
+               max_rows: Optional[int] = None, stream=None):
+    """Validate a row list for sx_scatter_kv / sx_sparse_attn (sx_check_rows; synchronises)."""
+    ws = batch.workspace(pool)
+    n = int(rows.numel()) if max_rows is None else int(max_rows)
+    _check(load().sx_check_rows(ctypes.byref(pool.c), ctypes.byref(batch.c), _ptr(rows), _ptr(rows_off), n, _ptr(ws),
+                                ws.numel(), _stream(stream)), "sx_check_rows")
+
+
 def workspace_size(pool: DevicePool, batch: DeviceBatch) -> int:
     n = ctypes.c_size_t(0)
     _check(load().sx_workspace_size(ctypes.byref(pool.c), ctypes.byref(batch.c), ctypes.byref(n)),
@@ -166,8 +193,6 @@ def workspace_size(pool: DevicePool, batch: DeviceBatch) -> int:
 
 def rope_realign(pool: DevicePool, batch: DeviceBatch, stream=None):
     """Stage (a): K pages rotated by R_delta into the request's pages, V copied."""
-    global LAUNCHES
-    LAUNCHES += 2 if batch.c.num_segments else 0          # rope_table_kernel + realign_kernel
     ws = batch.workspace(pool)
     _check(load().sx_rope_realign(ctypes.byref(pool.c), ctypes.byref(batch.c), _ptr(ws), ws.numel(),
                                   _stream(stream)), "sx_rope_realign")
@@ -175,9 +200,7 @@ def rope_realign(pool: DevicePool, batch: DeviceBatch, stream=None):
 
 def rope_realign_layers(pools, batch: DeviceBatch, stream=None):
     """Stage (a) for a stack of layers in one launch (same batch descriptor for all layers)."""
-    global LAUNCHES
     n = len(pools)
-    LAUNCHES += (1 + (n + 63) // 64) if batch.c.num_segments else 0
     ws = batch.workspace(pools[0])
     arr = (SxPool * n)(*[p.c for p in pools])
     _check(load().sx_rope_realign_layers(arr, n, ctypes.byref(batch.c), _ptr(ws), ws.numel(), _stream(stream)),
@@ -187,9 +210,7 @@ def rope_realign_layers(pools, batch: DeviceBatch, stream=None):
 def scatter_kv(pool: DevicePool, batch: DeviceBatch, k_fresh: torch.Tensor, v_fresh: torch.Tensor,
                rows: torch.Tensor, rows_off: torch.Tensor, max_rows: Optional[int] = None, stream=None):
     """Stage (d), Alg. 1 l.509-510/544-545: fresh K,V rows into their paged slots (COW aware)."""
-    global LAUNCHES
     n = int(rows.numel()) if max_rows is None else int(max_rows)
-    LAUNCHES += (1 + (1 if batch.cow_private is not None else 0)) if n else 0
     assert k_fresh.is_contiguous() and v_fresh.is_contiguous() and rows.dtype == torch.int32
     _check(load().sx_scatter_kv(ctypes.byref(pool.c), ctypes.byref(batch.c), _ptr(k_fresh), _ptr(v_fresh),
                                 _ptr(rows), _ptr(rows_off), n, _stream(stream)), "sx_scatter_kv")
@@ -200,8 +221,6 @@ def score_select(pool: DevicePool, batch: DeviceBatch, q_new: torch.Tensor, sel_
                  scores: Optional[torch.Tensor] = None, lse_new: Optional[torch.Tensor] = None,
                  lse_by_token: bool = False, stream=None):
     """Stage (b), Eq. (1)-(3): Sparse-Q scores, head/query aggregation, top-k, R = I_nr U S_key."""
-    global LAUNCHES
-    LAUNCHES += 2 + ((3 if lse_new is None else 2) if batch.c.total_new else 0)   # [lse sweep] coltab colsum score_sum select
     ws = batch.workspace(pool)
     _check(load().sx_score_select(ctypes.byref(pool.c), ctypes.byref(batch.c), _ptr(q_new), _ptr(lse_new),
                                   1 if lse_by_token else 0, _ptr(sel_off), _ptr(rows_off), _ptr(scores), _ptr(sel_idx), _ptr(rows_R),
@@ -215,8 +234,6 @@ def score_select_ex(pool: DevicePool, batch: DeviceBatch, q_new: torch.Tensor, s
                     lse_by_token: bool = False, stream=None):
     """Stage (b) with overflow and tail fallback (Alg. 1 l.535-539): R = I_nr U S_key U S_ov U S_tail; the
     actual CSR offsets of the packed rows_R come back in rows_off_out (device)."""
-    global LAUNCHES
-    LAUNCHES += 3 + ((3 if lse_new is None else 2) if batch.c.total_new else 0)
     ws = batch.workspace(pool)
     _check(load().sx_score_select_ex(ctypes.byref(pool.c), ctypes.byref(batch.c), _ptr(q_new), _ptr(lse_new),
                                      1 if lse_by_token else 0, _ptr(sel_off), _ptr(rows_cap_off),
@@ -244,15 +261,8 @@ def sparse_attn(pool: DevicePool, batch: DeviceBatch, q: torch.Tensor, out: torc
                 cuda_core: bool = False, cta_pair: Optional[bool] = None, stream=None):
     """Stage (c), Alg. 1 l.546-548 (sparse rows) / l.507-511 (full=True). cuda_core = SX_ATTN_CUDA_CORE;
     cta_pair: None = the library's rule, True / False = SX_ATTN_CTA_PAIR / SX_ATTN_SINGLE_CTA (include/sparsex.h)."""
-    global LAUNCHES
     ws = batch.workspace(pool)
     n = int(q.shape[0]) if total_rows is None else int(total_rows)
-    g = pool.c.num_q_heads // pool.c.num_kv_heads
-    small = cuda_core and g <= 32 and n * g < 64 * batch.c.num_reqs   # CUDA-core path: split kernel + merge kernel
-    if not small and n:          # few CTAs against a long context: key splits + merge kernel (attn_pv_splits)
-        grid = (n // (2 * (128 // g)) + batch.c.num_reqs) * pool.c.num_kv_heads
-        small = grid < 148 and min(148 // grid, ((batch.c.max_seq_len + 127) // 128) // 2) > 1
-    LAUNCHES += (2 if small else 1) if n else 0
     assert q.is_contiguous() and out.is_contiguous()
     _check(load().sx_sparse_attn(ctypes.byref(pool.c), ctypes.byref(batch.c), (1 if full else 0) | (2 if cuda_core else 0) | (0 if cta_pair is None else (4 if cta_pair else 8)), _ptr(q),
                                  _ptr(rows_R), _ptr(rows_off), n, _ptr(out), _ptr(lse), _ptr(ws), ws.numel(),

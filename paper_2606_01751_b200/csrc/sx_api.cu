@@ -4,6 +4,9 @@
 #include <stdio.h>
 #include <string.h>
 
+#include <atomic>
+#include <mutex>
+
 #include "sx_internal.h"
 
 namespace sx {
@@ -18,9 +21,12 @@ sx_status set_error(sx_status st, const char *fmt, ...) {
   return st;
 }
 
+static std::atomic<uint64_t> g_launches{0};  // diagnostic only (sx_launch_count)
+
 sx_status check_launch(const char *what) {
   cudaError_t e = cudaGetLastError();
   if (e != cudaSuccess) return set_error(SX_ERR_CUDA, "%s: %s", what, cudaGetErrorString(e));
+  g_launches.fetch_add(1, std::memory_order_relaxed);
   return SX_OK;
 }
 
@@ -100,24 +106,58 @@ typedef CUresult (*EncodeTiledFn)(CUtensorMap *, CUtensorMapDataType, cuuint32_t
                                   CUtensorMapFloatOOBfill);
 
 static sx_status get_encode(EncodeTiledFn *fn) {
+  static std::once_flag once;
   static EncodeTiledFn cached = nullptr;
-  if (!cached) {
+  static cudaError_t err = cudaSuccess;
+  std::call_once(once, [] {
     void *p = nullptr;
     cudaDriverEntryPointQueryResult q;
-    cudaError_t e = cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &p, cudaEnableDefault, &q);
-    if (e != cudaSuccess || q != cudaDriverEntryPointSuccess || !p) {
-      cudaGetLastError();
-      return set_error(SX_ERR_CUDA, "cuTensorMapEncodeTiled unavailable: %s", cudaGetErrorString(e));
-    }
-    cached = reinterpret_cast<EncodeTiledFn>(p);
+    err = cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &p, cudaEnableDefault, &q);
+    if (err == cudaSuccess && q == cudaDriverEntryPointSuccess) cached = reinterpret_cast<EncodeTiledFn>(p);
+  });
+  if (!cached) {
+    cudaGetLastError();
+    return set_error(SX_ERR_CUDA, "cuTensorMapEncodeTiled unavailable: %s", cudaGetErrorString(err));
   }
   *fn = cached;
   return SX_OK;
 }
 
+// Encoded tensor maps are a pure function of (base pointer, shape): a small process-wide cache keyed by exactly
+// those values saves the three driver encodes per stage call (visible on launch-bound configs such as C1). The
+// only state the library keeps besides the last-error text and the launch counter; nothing in it can go stale.
+struct TmapKey {
+  const void *base;
+  int a, b, c, d;  // pool: (num_blocks, Hkv, -1, -1); q: (total_rows, Hq, group, rows_per_tile)
+  bool operator==(const TmapKey &o) const { return base == o.base && a == o.a && b == o.b && c == o.c && d == o.d; }
+};
+constexpr int kTmapCache = 256;
+static std::mutex g_tmap_mu;
+static TmapKey g_tmap_key[kTmapCache];
+static CUtensorMap g_tmap_val[kTmapCache];
+static int g_tmap_n = 0, g_tmap_next = 0;
+
+static bool tmap_lookup(const TmapKey &k, CUtensorMap *out) {
+  std::lock_guard<std::mutex> lk(g_tmap_mu);
+  for (int i = 0; i < g_tmap_n; ++i)
+    if (g_tmap_key[i] == k) {
+      *out = g_tmap_val[i];
+      return true;
+    }
+  return false;
+}
+static void tmap_store(const TmapKey &k, const CUtensorMap &v) {
+  std::lock_guard<std::mutex> lk(g_tmap_mu);
+  const int i = g_tmap_n < kTmapCache ? g_tmap_n++ : (g_tmap_next++ % kTmapCache);
+  g_tmap_key[i] = k;
+  g_tmap_val[i] = v;
+}
+
 // Pool viewed as a 2-D bf16 matrix [num_blocks*Hkv*16 rows][128]; box = 64 columns x 16 rows (one
 // half of one (page, head) tile), 128-B swizzle: lands as two 8-row x 128-B swizzle atoms.
 sx_status make_tmap_pool(CUtensorMap *out, const void *base, int num_blocks, int num_kv_heads) {
+  const TmapKey key{base, num_blocks, num_kv_heads, -1, -1};
+  if (tmap_lookup(key, out)) return SX_OK;
   EncodeTiledFn enc;
   sx_status st = get_encode(&enc);
   if (st != SX_OK) return st;
@@ -129,6 +169,7 @@ sx_status make_tmap_pool(CUtensorMap *out, const void *base, int num_blocks, int
                    CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
                    CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
   if (r != CUDA_SUCCESS) return set_error(SX_ERR_CUDA, "cuTensorMapEncodeTiled(pool) failed: %d", (int)r);
+  tmap_store(key, *out);
   return SX_OK;
 }
 
@@ -138,6 +179,8 @@ sx_status make_tmap_pool(CUtensorMap *out, const void *base, int num_blocks, int
 // zero-filled by the TMA unit.
 sx_status make_tmap_q(CUtensorMap *out, const void *base, int total_rows, int num_q_heads, int group,
                       int rows_per_tile) {
+  const TmapKey key{base, total_rows, num_q_heads, group, rows_per_tile};
+  if (tmap_lookup(key, out)) return SX_OK;
   EncodeTiledFn enc;
   sx_status st = get_encode(&enc);
   if (st != SX_OK) return st;
@@ -149,6 +192,7 @@ sx_status make_tmap_q(CUtensorMap *out, const void *base, int total_rows, int nu
                    CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
                    CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
   if (r != CUDA_SUCCESS) return set_error(SX_ERR_CUDA, "cuTensorMapEncodeTiled(q) failed: %d", (int)r);
+  tmap_store(key, *out);
   return SX_OK;
 }
 
@@ -160,7 +204,27 @@ extern "C" {
 
 const char *sx_last_error(void) { return g_err; }
 
-const char *sx_version(void) { return "sparsex-b200 0.1 (sm_100a; tcgen05/TMEM/TMA)"; }
+const char *sx_version(void) { return "sparsex-b200 0.2 (sm_100a; tcgen05/TMEM/TMA)"; }
+
+uint64_t sx_launch_count(void) { return g_launches.load(std::memory_order_relaxed); }
+
+sx_status sx_check_batch(const sx_pool *pool, const sx_batch *batch, void *ws, size_t ws_bytes, sx_stream stream) {
+  sx_status st = validate(pool, batch);
+  if (st != SX_OK) return st;
+  st = validate_ws(pool, batch, ws, ws_bytes);
+  if (st != SX_OK) return st;
+  return run_check_batch(pool, batch, ws, reinterpret_cast<cudaStream_t>(stream));
+}
+
+sx_status sx_check_rows(const sx_pool *pool, const sx_batch *batch, const int32_t *rows, const int32_t *rows_off,
+                        int32_t max_rows, void *ws, size_t ws_bytes, sx_stream stream) {
+  sx_status st = validate(pool, batch);
+  if (st != SX_OK) return st;
+  st = validate_ws(pool, batch, ws, ws_bytes);
+  if (st != SX_OK) return st;
+  if (!rows_off || max_rows < 0 || (max_rows > 0 && !rows)) return set_error(SX_ERR_INVALID_ARG, "check_rows: NULL array");
+  return run_check_rows(batch, rows, rows_off, max_rows, ws, reinterpret_cast<cudaStream_t>(stream));
+}
 
 sx_status sx_workspace_size(const sx_pool *pool, const sx_batch *batch, size_t *bytes) {
   if (!bytes) return set_error(SX_ERR_INVALID_ARG, "bytes is NULL");
@@ -175,6 +239,12 @@ sx_status sx_workspace_size(const sx_pool *pool, const sx_batch *batch, size_t *
 sx_status sx_rope_realign_layers(const sx_pool *pools, int32_t num_layers, const sx_batch *batch, void *ws,
                                  size_t ws_bytes, sx_stream stream) {
   if (!pools || num_layers <= 0) return set_error(SX_ERR_INVALID_ARG, "pools is NULL or num_layers <= 0");
+  // Copy-on-write state lives in the batch's v_block_table, page CONTENTS are per layer: after layer 0's scatter has
+  // flipped an entry to the private page, the other layers' private pages would never be filled. A descriptor with
+  // cow_private therefore describes the tables of ONE layer (one sx_batch per layer under COW).
+  if (batch && batch->cow_private && num_layers > 1)
+    return set_error(SX_ERR_UNSUPPORTED,
+                     "copy-on-write tables are per layer: call sx_rope_realign with one sx_batch per layer");
   for (int l = 0; l < num_layers; ++l) {
     sx_status st = validate(&pools[l], batch);
     if (st != SX_OK) return st;

@@ -204,18 +204,38 @@ int32_t sx_index_evict(sx_index *ix, int32_t used_blocks, int32_t total_blocks, 
                        int32_t *evicted_out, int32_t max_out) {
   if (!ix || total_blocks <= 0 || used_blocks < 0 || max_out < 0 || (max_out > 0 && !evicted_out))
     return SX_ERR_INVALID_ARG;
-  std::vector<sx_index::It> cand;
-  for (auto it = ix->map.begin(); it != ix->map.end(); ++it)
-    if (it->second.frozen && it->second.refs == 0) cand.push_back(it);
-  std::sort(cand.begin(), cand.end(), [](const sx_index::It &a, const sx_index::It &b) {
-    if (a->second.hits != b->second.hits) return a->second.hits < b->second.hits;
-    return a->second.serial < b->second.serial;
+  // Eviction frees PHYSICAL blocks, and several virtual blocks (other namespaces, other token views) may sit on
+  // one physical block: a block is evictable only if EVERY view of it is frozen and unreferenced; it is ranked by
+  // the hand-outs of all its views (sum of hits, then its oldest view), all its views leave the index together and
+  // the block is reported once.
+  struct Blk {
+    int32_t block;
+    int64_t hits, serial;
+    std::vector<sx_index::It> views;
+  };
+  std::unordered_map<int32_t, Blk> blocks;
+  std::unordered_map<int32_t, bool> pinned;  // some view of the block is referenced or not frozen
+  for (auto it = ix->map.begin(); it != ix->map.end(); ++it) {
+    const Entry &e = it->second;
+    if (!e.frozen || e.refs > 0) pinned[e.block] = true;
+    auto ins = blocks.emplace(e.block, Blk{e.block, 0, e.serial, {}});
+    Blk &b = ins.first->second;
+    b.hits += e.hits;
+    b.serial = std::min(b.serial, e.serial);
+    b.views.push_back(it);
+  }
+  std::vector<Blk *> cand;
+  for (auto &kv : blocks)
+    if (!pinned.count(kv.first)) cand.push_back(&kv.second);
+  std::sort(cand.begin(), cand.end(), [](const Blk *a, const Blk *b) {
+    if (a->hits != b->hits) return a->hits < b->hits;
+    return a->serial < b->serial;
   });
   int n = 0;
-  for (auto &it : cand) {
+  for (Blk *b : cand) {
     if (n >= max_out || (double)(used_blocks - n) / (double)total_blocks <= threshold) break;
-    evicted_out[n++] = it->second.block;
-    ix->erase(it);
+    evicted_out[n++] = b->block;
+    for (auto &it : b->views) ix->erase(it);
   }
   return n;
 }

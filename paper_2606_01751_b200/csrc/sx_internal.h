@@ -60,6 +60,11 @@ sx_status launch_colsum(const sx_pool *pool, const sx_batch *b, const void *q_ne
                         int lse_by_token, int lse_splits, float *partial, float2 *col_tab, cudaStream_t st);
 size_t colsum_tab_bytes(const sx_pool *pool, const sx_batch *b);
 
+// descriptor validation (sx_check.cu): one kernel + one error word copied back; synchronises the stream
+sx_status run_check_batch(const sx_pool *pool, const sx_batch *b, void *ws, cudaStream_t st);
+sx_status run_check_rows(const sx_batch *b, const int32_t *rows, const int32_t *rows_off, int32_t max_rows, void *ws,
+                         cudaStream_t st);
+
 // TMA descriptor construction (driver entry point fetched through the runtime; no libcuda link)
 sx_status make_tmap_pool(CUtensorMap *out, const void *base, int num_blocks, int num_kv_heads);
 sx_status make_tmap_q(CUtensorMap *out, const void *base, int total_rows, int num_q_heads, int group,

@@ -82,6 +82,7 @@ select_kernel(int num_kv_heads, int total_tokens, const int32_t *__restrict__ se
   __shared__ int tot[3];
   __shared__ uint32_t sh_prefix;
   __shared__ int sh_remaining;
+  __shared__ int sh_ncand;
 
   const int req = blockIdx.x;
   const int T = seq_len[req];
@@ -95,15 +96,14 @@ select_kernel(int num_kv_heads, int total_tokens, const int32_t *__restrict__ se
   // Candidates of Eq. (3) = I_reuse = the positions covered by this request's segments. Positions that are neither
   // new nor in a segment are prefix-cache hits (Alg. 1 l.501: "excluded from the current prefill computation"):
   // visible as keys, never candidates, never in S_ov / S_tail, never query rows.
-  int n_cached = 0;
-  for (int m = 0; m < num_segments; ++m)
-    if (segs[m].req == req) n_cached += segs[m].len;
-  if (k > n_cached) k = n_cached;
-  if (k < 0) k = 0;
-
   uint32_t *forced = is_new + words;  // S_ov U S_tail (Alg. 1 l.535-536), cached positions only
   uint32_t *cand = forced + words;    // I_reuse
   for (int i = threadIdx.x; i < 3 * words; i += kSelThreads) is_new[i] = 0u;
+  if (threadIdx.x == 0) {
+    sh_ncand = 0;
+    sh_prefix = 0u;
+    sh_remaining = 0;
+  }
   __syncthreads();
   for (int i = threadIdx.x; i < nn; i += kSelThreads) {
     int p = new_idx[n0 + i];
@@ -117,6 +117,23 @@ select_kernel(int num_kv_heads, int total_tokens, const int32_t *__restrict__ se
       if (q < T) atomicOr(&cand[q >> 5], 0xFFFFu << (q & 31));
     }
   }
+  // k is clamped to the number of candidates that really exist: bits of the candidate bitmap below T (a segment
+  // whose last page straddles seq_len, or overlapping segments, make sum(len) an overestimate)
+  __syncthreads();
+  {
+    int c = 0;
+    for (int i = threadIdx.x; i < words; i += kSelThreads) {
+      uint32_t wv = cand[i];
+      if (i == words - 1 && (T & 31)) wv &= (1u << (T & 31)) - 1u;
+      c += __popc(wv);
+    }
+#pragma unroll
+    for (int d = 16; d > 0; d >>= 1) c += __shfl_xor_sync(0xffffffffu, c, d);
+    if ((threadIdx.x & 31) == 0 && c) atomicAdd(&sh_ncand, c);
+  }
+  __syncthreads();
+  if (k > sh_ncand) k = sh_ncand;
+  if (k < 0) k = 0;
   if (ov_tokens > 0 || tail_tokens > 0) {
     __syncthreads();
     // overflow (Alg. 1 l.535): every maximal interval [a, b] of I_nr grows by one block
@@ -227,7 +244,10 @@ select_kernel(int num_kv_heads, int total_tokens, const int32_t *__restrict__ se
   //   A: equals of the threshold per warp -> which of them are taken (lowest positions first, reading A8)
   //   B: |S_key| and |R| per warp          C: write S_key and R in ascending position order
   // (three cheap passes over L2-resident scores instead of a block-wide scan per 1024 positions)
-  const int so = sel_off[req], ro = rows_off[req], cap_r = rows_off[req + 1] - ro;
+  // (extended selection: rows_R is the workspace array rows_tmp [total_tokens], where request r owns the T_r
+  // slots behind tok_off[r] -- always enough, whatever capacities the caller passed)
+  const int so = sel_off[req], ro = rows_cnt ? off : rows_off[req];
+  const int cap_r = min(rows_off[req + 1] - rows_off[req], T);
   const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
   const unsigned lt = (1u << lane) - 1u;
   const int seg = ((((je - jb) + kSelWarps - 1) / kSelWarps) + 127) & ~127;  // positions per warp, multiple of 32 * kB
@@ -346,14 +366,14 @@ select_kernel(int num_kv_heads, int total_tokens, const int32_t *__restrict__ se
   if (rows_cnt && threadIdx.x == 0 && sl == 0) rows_cnt[req] = min(total_r, cap_r);
 }
 
-// Extended selection only: per-request row lists sit in capacity-sized slots of `tmp`; pack them into one
+// Extended selection only: per-request row lists sit in the T_r-sized slots of `tmp` (at tok_off[r]); pack them into one
 // CSR (rows_R, rows_off_out) so that the scatter and attention stages take them unchanged.
 __global__ void __launch_bounds__(kSelThreads)
-compact_rows_kernel(int num_reqs, const int32_t *__restrict__ cap_off, const int32_t *__restrict__ cnt,
+compact_rows_kernel(int num_reqs, const int32_t *__restrict__ tok_off, const int32_t *__restrict__ cnt,
                     const int32_t *__restrict__ tmp, int32_t *__restrict__ rows_R, int32_t *__restrict__ rows_off_out) {
   int out = 0;
   for (int r = 0; r < num_reqs; ++r) {
-    const int n = cnt[r], src = cap_off[r];
+    const int n = cnt[r], src = tok_off[r];
     for (int i = threadIdx.x; i < n; i += kSelThreads) rows_R[out + i] = tmp[src + i];
     if (threadIdx.x == 0) rows_off_out[r] = out;
     out += n;
@@ -406,7 +426,7 @@ sx_status launch_select(const sx_pool *pool, const sx_batch *b, const float *par
                                                                   rows_dst, ov_tokens, tail_tokens, segs, nseg, cnt, scratch);
   sx_status s = check_launch("select_kernel");
   if (s != SX_OK || !ex) return s;
-  compact_rows_kernel<<<1, kSelThreads, 0, st>>>(b->num_reqs, rows_off, rows_cnt, rows_tmp, rows_R, rows_off_out);
+  compact_rows_kernel<<<1, kSelThreads, 0, st>>>(b->num_reqs, b->tok_off, rows_cnt, rows_tmp, rows_R, rows_off_out);
   return check_launch("compact_rows_kernel");
 }
 

@@ -148,7 +148,8 @@ class Layout:
         for s in range(self.num_segments):
             r, ln, _, new_pos, _ = (int(v) for v in self.segments[s])
             if r == req:
-                m[new_pos:new_pos + ln] = self.pool_salient[int(self.seg_pool_id[s])]
+                n = len(m[new_pos:new_pos + ln])     # a trimmed request ends inside its last segment
+                m[new_pos:new_pos + ln] = self.pool_salient[int(self.seg_pool_id[s])][:n]
         return m
 
 
@@ -171,7 +172,10 @@ ReqSpec = Sequence[Tuple[str, int]]
 def build_layout(name: str, cfg_id: int, num_q_heads: int, num_kv_heads: int, rope_theta: float,
                  pool_segments: Sequence[PoolSegment], requests: Sequence[ReqSpec],
                  ratios: Sequence[float], salient_frac: float, cow: bool = False,
-                 rope_style: int = 0, k_override: Optional[Sequence[int]] = None) -> Layout:
+                 rope_style: int = 0, k_override: Optional[Sequence[int]] = None,
+                 trim: Optional[Sequence[int]] = None) -> Layout:
+    """trim[r] (< 16): tokens cut from the END of request r, whose last item must then be a segment: the
+    segment's last page straddles seq_len (ragged tail inside a reused segment, reading A19)."""
     pool_segments = list(pool_segments)
     for ps in pool_segments:
         assert ps.length % PAGE == 0 and ps.old_pos % PAGE == 0 and ps.length > 0
@@ -182,6 +186,10 @@ def build_layout(name: str, cfg_id: int, num_q_heads: int, num_kv_heads: int, ro
         for kind, val in spec:
             t += val if kind in ("new", "prefix") else pool_segments[val].length
         seq_len[r] = t
+    if trim is not None:
+        for r, cut in enumerate(trim):
+            assert 0 <= cut < PAGE and (cut == 0 or requests[r][-1][0] == "seg")
+            seq_len[r] -= cut
     pages_per_req = (seq_len + PAGE - 1) // PAGE
     max_pages = int(pages_per_req.max())
     n_src = sum(ps.length // PAGE for ps in pool_segments)
@@ -409,7 +417,8 @@ def config_c5(scale: float = 1.0, ratio: float = 0.05) -> Layout:
 CONFIGS = {"C1": config_c1, "C2": config_c2, "C3": config_c3, "C4": config_c4, "C5": config_c5}
 
 
-def config_tail(seed_id: int = 15, prefix: int = 0) -> Layout:
+def config_tail(seed_id: int = 15, prefix: int = 0, trim: Optional[Sequence[int]] = None,
+                k_override: Sequence[int] = (8, 4, 19)) -> Layout:
     """Requests that END inside a reused segment (tail fallback) and whose new-token intervals
     touch reused segments on both sides (overflow): request 0 ends with a 96-token segment
     (tail = its last 64 tokens), request 1 with a 32-token one (tail = all of it), request 2 ends with new
@@ -423,7 +432,8 @@ def config_tail(seed_id: int = 15, prefix: int = 0) -> Layout:
         reqs = [[("prefix", prefix)] + spec for spec in reqs]
     # budgets below the number of cached tokens that some new query can see (the tokens behind the last new
     # token score exactly 0 and would turn the cut into a pure position tie)
-    return build_layout("tail", seed_id, 4, 2, 10000.0, pool, reqs, [0.2, 0.25, 0.3], 0.1, k_override=[8, 4, 19])
+    return build_layout("tail", seed_id, 4, 2, 10000.0, pool, reqs, [0.2, 0.25, 0.3], 0.1, k_override=list(k_override),
+                        trim=trim)
 
 
 def config_tiny(seed_id: int = 9, num_q_heads: int = 4, num_kv_heads: int = 2, tail: int = 0,

@@ -94,3 +94,25 @@ def test_selection_offsets():
     n_new = np.diff(lay.new_off)
     assert np.array_equal(np.diff(sel_off), lay.k_per_req)
     assert np.array_equal(np.diff(rows_off), lay.k_per_req + n_new)
+
+
+def test_cow_tables_are_per_layer(lib):
+    """Copy-on-write state (v_block_table) belongs to one layer: the all-layer realign refuses a COW descriptor
+    with more than one layer (include/sparsex.h) instead of leaving the other layers' private pages unfilled."""
+    lay = wl.config_tiny(cow=True)
+    pool, b = _host_structs(lay)
+    b.cow_private = 0x100
+    pools = (sx.SxPool * 2)(pool, pool)
+    ws = ctypes.c_void_p(0x10000)
+    assert lib.sx_rope_realign_layers(pools, 2, ctypes.byref(b), ws, 1 << 30, None) == -2
+    assert b"per layer" in lib.sx_last_error()
+
+
+def test_check_calls_validate_host_arguments_first(lib):
+    lay = wl.config_tiny()
+    pool, b = _host_structs(lay)
+    ws = ctypes.c_void_p(0x10000)
+    assert lib.sx_check_batch(None, ctypes.byref(b), ws, 1 << 30, None) == -1
+    assert lib.sx_check_batch(ctypes.byref(pool), ctypes.byref(b), ws, 16, None) == -3
+    assert lib.sx_check_rows(ctypes.byref(pool), ctypes.byref(b), ws, None, 4, ws, 1 << 30, None) == -1
+    assert lib.sx_launch_count() >= 0

@@ -439,3 +439,124 @@ def test_paper_mode_boundary_selection_uncarved_band():
     assert len(np.setdiff1d(sel, ref_sel)) <= band
     own_sel, own_rows = orc.select_topk(g3.scores.cpu().numpy().astype(np.float64), lay.is_new_mask(0), k)
     assert np.array_equal(sel, own_sel) and np.array_equal(g3.rows_R.cpu().numpy(), own_rows)
+
+
+def test_check_batch_and_rows_reject_bad_device_descriptors():
+    """sx_check_batch / sx_check_rows (include/sparsex.h): the device-resident arrays that the stage calls cannot
+    see from the host mirrors. A misaligned segment must give SX_ERR_INVALID_ARG, not corrupt pages."""
+    GpuLayer, dev_to_bits = _gpu()
+    from paper_2606_01751_b200 import binding as sx
+    import copy
+    lay = wl.config_tiny()
+    lt = wl.build_layer(lay, 0)
+    g = GpuLayer(lay, lt)
+    sx.check_batch(g.pool, g.batch)                                   # a good descriptor passes
+
+    def broken(mutate, needle):
+        bad = copy.deepcopy(lay)
+        mutate(bad)
+        gb = GpuLayer(bad, lt)
+        with pytest.raises(sx.SparseXError) as ei:
+            sx.check_batch(gb.pool, gb.batch)
+        assert "(-1)" in str(ei.value) and needle in str(ei.value), str(ei.value)
+
+    def seg_set(m, col, val):
+        def f(bad):
+            bad.segments = bad.segments.copy()
+            bad.segments[m, col] = val
+        return f
+    broken(seg_set(1, 3, int(lay.segments[1, 3]) + 8), "multiple of block_size")      # new_pos misaligned
+    broken(seg_set(0, 2, int(lay.segments[0, 2]) + 4), "multiple of block_size")      # old_pos misaligned
+    broken(seg_set(2, 4, int(lay.segments[2, 4]) + 1), "running sum")                 # src_off
+    broken(seg_set(1, 3, int(lay.segments[0, 3])), "sorted")                          # overlaps segment 0
+
+    def bad_new_idx(bad):
+        bad.new_idx = bad.new_idx.copy()
+        bad.new_idx[3], bad.new_idx[4] = bad.new_idx[4], bad.new_idx[3]
+    broken(bad_new_idx, "new_idx")
+
+    def bad_page(bad):
+        bad.src_blocks = bad.src_blocks.copy()
+        bad.src_blocks[1] = bad.num_blocks + 7
+    broken(bad_page, "src_blocks")
+
+    def bad_table(bad):
+        bad.k_block_table = bad.k_block_table.copy()
+        bad.k_block_table[1, 0] = -3
+    broken(bad_table, "k_block_table")
+
+    # row lists
+    rows = torch.tensor([0, 5, 9, 2, 3], dtype=torch.int32, device=g.dev)
+    off = torch.tensor([0, 3, 5], dtype=torch.int32, device=g.dev)
+    sx.check_rows(g.pool, g.batch, rows, off)
+    with pytest.raises(sx.SparseXError):
+        sx.check_rows(g.pool, g.batch, torch.tensor([0, 9, 5, 2, 3], dtype=torch.int32, device=g.dev), off)
+    with pytest.raises(sx.SparseXError):
+        sx.check_rows(g.pool, g.batch, torch.tensor([0, 5, 9, 2, 4000], dtype=torch.int32, device=g.dev), off)
+    with pytest.raises(sx.SparseXError):
+        sx.check_rows(g.pool, g.batch, rows, torch.tensor([0, 4, 3], dtype=torch.int32, device=g.dev))
+
+
+@pytest.mark.parametrize("extended", [False, True], ids=["select", "select_ex"])
+def test_budget_clamped_to_real_candidates_and_unclipped_capacities(extended):
+    """Two requests END inside a reused segment whose last page straddles seq_len (reading A19), and ask for more
+    cached tokens than exist: k must be clamped to the candidates below seq_len (sum of segment lengths
+    overestimates them). The extended call additionally gets capacities far above T_r, as a C caller might pass."""
+    GpuLayer, dev_to_bits = _gpu()
+    from paper_2606_01751_b200 import binding as sx
+    lay = wl.config_tail(trim=[5, 3, 0], k_override=[200, 200, 19])
+    lt = wl.build_layer(lay, 0)
+    carve_margins(lay, lt)
+    res, pk, pv, kt, vt = oracle_layer(lay, lt, mode="sparse")
+    g = GpuLayer(lay, lt)
+    g.realign()
+    g.scatter_new()
+    if not extended:
+        g.select()
+        sel, rows = g.sel_idx.cpu().numpy(), g.rows_R.cpu().numpy()
+        for r in range(lay.num_reqs):
+            n_sel, n_rows = len(res.sel[r]), len(res.rows[r])
+            s0, r0 = int(g.sel_off_h[r]), int(g.rows_off_h[r])
+            assert np.array_equal(sel[s0:s0 + n_sel], res.sel[r]), r
+            assert np.array_equal(rows[r0:r0 + n_rows], res.rows[r]), r
+    else:
+        cap = np.concatenate([[0], np.cumsum(10 * lay.seq_len)]).astype(np.int32)      # NOT clipped to T_r
+        n_sel = int(g.sel_off_h[-1])
+        sel = torch.full((n_sel,), -1, dtype=torch.int32, device=g.dev)
+        rows = torch.full((int(cap[-1]),), -1, dtype=torch.int32, device=g.dev)
+        off_out = torch.zeros(lay.num_reqs + 1, dtype=torch.int32, device=g.dev)
+        sx.score_select_ex(g.pool, g.batch, g.q_new, g.sel_off, torch.from_numpy(cap).to(g.dev), sel, rows, off_out,
+                           overflow_blocks=0, tail_tokens=0)
+        torch.cuda.synchronize()
+        off_h, rows_h, sel_h = off_out.cpu().numpy(), rows.cpu().numpy(), sel.cpu().numpy()
+        for r in range(lay.num_reqs):
+            assert np.array_equal(rows_h[off_h[r]:off_h[r + 1]], res.rows[r]), r
+            s0 = int(g.sel_off_h[r])
+            assert np.array_equal(sel_h[s0:s0 + len(res.sel[r])], res.sel[r]), r
+        assert np.all(rows_h[off_h[-1]:] == -1)                                       # nothing written past the end
+
+
+def test_copy_on_write_two_layers_each_with_its_own_tables():
+    """COW state (v_block_table) is per layer. Two layers of one request batch, each with its own
+    descriptor, both end with the oracle's tables and pools; the all-layer realign refuses the COW descriptor."""
+    GpuLayer, dev_to_bits = _gpu()
+    from paper_2606_01751_b200 import binding as sx
+    lay = wl.config_c4(scale=0.125, num_reqs=3, cow=True)
+    gs = []
+    for layer in range(2):
+        lt = wl.build_layer(lay, layer)
+        carve_margins(lay, lt)
+        res, pk, pv, kt, vt = oracle_layer(lay, lt, mode="sparse")
+        g = GpuLayer(lay, lt)                       # own DeviceBatch -> own block tables
+        g.step_sparse()
+        torch.cuda.synchronize()
+        assert np.array_equal(g.batch.v_block_table.cpu().numpy(), vt) and np.array_equal(dev_to_bits(g.pool_v), pv)
+        assert np.array_equal(g.batch.k_block_table.cpu().numpy(), kt)
+        out = orc.bf16_to_f64(dev_to_bits(g.out))
+        for r in range(lay.num_reqs):
+            r0, r1 = g.rows_off_h[r], g.rows_off_h[r + 1]
+            assert np.array_equal(g.rows_R.cpu().numpy()[r0:r1], res.rows[r])
+            check_close("cow layer %d req %d" % (layer, r), out[r0:r1], res.out[r])
+        gs.append(g)
+    with pytest.raises(sx.SparseXError):
+        sx.rope_realign_layers([g.pool for g in gs], gs[0].batch)

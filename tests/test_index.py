@@ -63,6 +63,44 @@ def test_oracle_hand_cases():
     assert o2.evict(used=92, total=100, threshold=0.9) == []
 
 
+def test_oracle_eviction_with_two_namespaces_on_one_block():
+    """Several virtual blocks may sit on one physical block (other namespace keys). Eviction
+    frees PHYSICAL blocks: one referenced or non-frozen view pins the block; an evictable block is reported once
+    and all its views leave together. Expected lists typed by hand."""
+    o = IndexOracle(BS)
+    a, b, c = np.arange(0, 16), np.arange(16, 32), np.arange(32, 48)
+    o.insert(a, key=1, old_pos=0, blocks=[50], frozen=True)
+    o.insert(a, key=2, old_pos=0, blocks=[50], frozen=True)    # second namespace, same physical block 50
+    o.insert(b, key=1, old_pos=16, blocks=[51], frozen=True)
+    o.insert(b, key=2, old_pos=16, blocks=[51], frozen=False)  # block 51 also carries a NON-frozen view
+    o.insert(c, key=1, old_pos=32, blocks=[52], frozen=True)
+    o.plan_request(0, a, [(0, 16)], key=2)                     # namespace 2 references block 50
+    # 50: view (key 2) referenced -> pinned; 51: one view not frozen -> pinned; 52: free to go
+    assert o.evict(used=100, total=100, threshold=0.5) == [52]
+    assert len(o) == 4
+    o.release([50])                                            # now every view of 50 is frozen and unreferenced
+    assert o.evict(used=100, total=100, threshold=0.5) == [50]  # reported ONCE, both views gone
+    assert len(o) == 2
+    assert o.plan_request(1, a, [(0, 16)], key=1)[0] == 0 and o.plan_request(1, a, [(0, 16)], key=2)[0] == 0
+    assert o.evict(used=100, total=100, threshold=0.5) == []   # 51 stays pinned by its non-frozen view
+
+
+def test_eviction_with_two_namespaces_matches_oracle(idx_mod):
+    ix, o = idx_mod.SegmentIndex(BS), IndexOracle(BS)
+    a, b, c = (np.arange(i * 16, i * 16 + 16, dtype=np.int32) for i in range(3))
+    for (t, key, old, blk, fr) in [(a, 1, 0, 50, True), (a, 2, 0, 50, True), (b, 1, 16, 51, True),
+                                   (b, 2, 16, 51, False), (c, 1, 32, 52, True)]:
+        assert ix.insert(t, key, old, np.asarray([blk], np.int32), fr) == o.insert(t, key, old, [blk], fr)
+    h1 = ix.plan_request(0, a, [(0, 16)], 2)
+    h2 = o.plan_request(0, a, [(0, 16)], key=2)
+    assert h1[0] == h2[0] == 1
+    assert ix.evict(100, 100, 0.5).tolist() == o.evict(100, 100, 0.5) == [52]
+    assert ix.release(np.asarray([50], np.int32)) == o.release([50]) == 0
+    assert ix.evict(100, 100, 0.5).tolist() == o.evict(100, 100, 0.5) == [50]
+    assert len(ix) == len(o) == 2
+    assert ix.evict(100, 100, 0.5).tolist() == o.evict(100, 100, 0.5) == []
+
+
 # ----------------------------------------------------------------------------- C++ against the oracle
 
 def test_header_symbols(idx_mod):
@@ -94,6 +132,11 @@ def test_random_traffic_matches_oracle(idx_mod, seed):
             frozen = bool(rng.random() < 0.5)
             assert ix.insert(toks, key, old, blocks, frozen) == o.insert(toks, key, old, blocks, frozen)
             lib_docs.append((toks, key))
+            if rng.random() < 0.3:     # a second namespace viewing the SAME physical blocks
+                key2 = key % 3 + 1
+                fr2 = bool(rng.random() < 0.7)
+                assert ix.insert(toks, key2, old, blocks, fr2) == o.insert(toks, key2, old, blocks, fr2)
+                lib_docs.append((toks, key2))
         elif op == "plan":
             parts, cands, pos = [], [], 0
             for _ in range(int(rng.integers(1, 5))):
