@@ -19,7 +19,8 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 sys.path.insert(0, os.path.dirname(HERE))
 sys.path.insert(0, os.path.dirname(os.path.dirname(HERE)))
 
-from helpers import carve_margins, carve_margins_fresh  # noqa: E402
+from helpers import carve_margins, carve_margins_fresh, oracle_scores_full_layer  # noqa: E402
+from oracle import sx_oracle as orc  # noqa: E402
 from paper_2606_01751_b200 import workloads as wl  # noqa: E402
 
 
@@ -37,7 +38,16 @@ def main():
                 f.write("# written by tests/golden/make_carve.py (fp64 oracle only); columns: batch token index, scale\n")
                 for tok, scale in log:
                     f.write("%d %.2f\n" % (tok, scale))
-            print(name, hist, len(log), "ops, %.0f s" % (time.time() - t0), flush=True)
+            # the recompute set the oracle selects on the carved boundary layer (R = I_nr U S_key, Alg. 1 l.537-539):
+            # bench.py's CPU legs scale the oracle's sparse-attention time by sum_{r in R} (r + 1) of THIS set
+            s = oracle_scores_full_layer(lay, lt)[0]
+            sel, rows = orc.select_topk(s, lay.is_new_mask(0), int(lay.k_per_req[0]), lay.cached_mask(0))
+            with open(os.path.join(HERE, "rows_C3_L3.txt"), "w") as f:
+                f.write("# R = I_nr U S_key of the boundary-layer selection of C3 (layer 3, carved by carve_C3_L3.txt), "
+                        "fp64 oracle; %d rows, k = %d\n" % (len(rows), len(sel)))
+                f.write("# written by tests/golden/make_carve.py (fp64 oracle only); one position per line\n")
+                f.write("\n".join(str(int(r)) for r in rows) + "\n")
+            print(name, hist, len(log), "ops, %d rows, %.0f s" % (len(rows), time.time() - t0), flush=True)
             continue
         lay = wl.CONFIGS[name]()
         lt = wl.build_layer(lay, 0)
