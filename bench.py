@@ -395,30 +395,40 @@ def measure(cfg, steps, warmup, ctx, want_e2e=True, want_clocks=True):
 
 
 def measure_s6(ctx, reps=10):
-    """Supplementary HBM-regime cases: stage (c) alone with fewer than 64 (row, head) pairs per
-    KV head (and one with 112): K and V of the whole context are streamed once. Both dispatch choices are timed:
-    the default padded tensor-core tile with key splits, and the CUDA-core kernels (SX_ATTN_CUDA_CORE).
-    Achieved GB/s = 4*T*Hkv*128 B / time, L2 flushed between repetitions."""
+    """Supplementary HBM-regime cases: stage (c) alone with few (row, head) pairs per KV head: K and V
+    of the whole context are streamed once. Both dispatch choices are timed: the library's default (the padded
+    tensor-core tile with key splits that merge themselves) and the CUDA-core kernels (SX_ATTN_CUDA_CORE, north_star's
+    rule below 64 pairs per KV head).
+    Achieved GB/s = 4*T*Hkv*128 B / time, L2 flushed between repetitions. "chained4": the same call on the pools of
+    four consecutive layers back to back (536 MB of K/V, larger than L2, no flush): what a layer stack sees, with the
+    launch of each call overlapping the tail of the previous one (programmatic dependent launch)."""
     torch, sx, dev, peaks = ctx["torch"], ctx["sx"], ctx["dev"], ctx["peaks"]
     from paper_2606_01751_b200.layer import GpuLayer
     flush = torch.empty(512 << 20, dtype=torch.uint8, device=dev)
     out = {}
-    # (i) C3 pool, last 1 / 2 / 8 positions: 4 / 8 / 32 pairs per KV head -> CUDA-core paths
-    # (ii) C5 pool, last 16 positions: 112 pairs per KV head -> tcgen05 tiles with key splits
+
+    def frac(t_ms, nbytes):
+        gbs = nbytes / (t_ms * 1e-3) / 1e9
+        return {"ms": round(t_ms, 4), "hbm_gbs": round(gbs, 1), "hbm_frac": round(gbs / peaks["hbm_gbs"], 4),
+                "hbm_frac_nominal": round(gbs / NOMINAL_HBM_GBS, 4)}
+    # (i) C3 pool, last 1 / 2 / 8 positions: 4 / 8 / 32 pairs per KV head; (ii) C5 pool, last 16 positions: 112 pairs
     for cfg, layer, lasts in (("C3", 4, (1, 2, 8)), ("C5", 0, (16,))):
         lay = wl.CONFIGS[cfg]()
-        gl = GpuLayer(lay, DevLayer(lay, layer, dev, torch), dev)
+        n_l = 4 if cfg == "C3" else 1
+        gls = [GpuLayer(lay, DevLayer(lay, layer + i, dev, torch), dev) for i in range(n_l)]
         T, hq, hkv = lay.total_tokens, lay.num_q_heads, lay.num_kv_heads
-        sx.rope_realign(gl.pool, gl.batch)
         all_rows = torch.arange(T, dtype=torch.int32, device=dev)
-        sx.scatter_kv(gl.pool, gl.batch, gl.k_fresh, gl.v_fresh, all_rows, gl.batch.tok_off, max_rows=T)
+        for gl in gls:
+            sx.rope_realign(gl.pool, gl.batch)
+            sx.scatter_kv(gl.pool, gl.batch, gl.k_fresh, gl.v_fresh, all_rows, gl.batch.tok_off, max_rows=T)
+        gl = gls[0]
         for n in lasts:
             rows = torch.arange(T - n, T, dtype=torch.int32, device=dev)
             off = torch.tensor([0, n], dtype=torch.int32, device=dev)
             q = gl.q_full[T - n:T].contiguous()
             o = torch.empty((n, hq, 128), dtype=torch.int16, device=dev)
             res = {}
-            for label, cc in (("tcgen05_splits", False), ("cuda_core", True)):
+            for label, cc, pair in (("tcgen05_splits", False, None), ("cuda_core", True, None)):
                 if cc and n * hq // hkv >= 64:
                     continue                    # the CUDA-core kernels are for fewer than 64 pairs per KV head
                 ms = []
@@ -426,17 +436,27 @@ def measure_s6(ctx, reps=10):
                     flush.zero_()
                     a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
                     a.record()
-                    sx.sparse_attn(gl.pool, gl.batch, q, o, rows_R=rows, rows_off=off, total_rows=n, cuda_core=cc)
+                    sx.sparse_attn(gl.pool, gl.batch, q, o, rows_R=rows, rows_off=off, total_rows=n, cuda_core=cc,
+                                   cta_pair=pair)
                     b.record()
                     torch.cuda.synchronize()
                     if i >= 3:
                         ms.append(a.elapsed_time(b))
-                t = float(np.median(ms))
-                gbs = 4.0 * T * hkv * 128 / (t * 1e-3) / 1e9
-                res[label] = {"ms": round(t, 4), "hbm_gbs": round(gbs, 1), "hbm_frac": round(gbs / peaks["hbm_gbs"], 4),
-                              "hbm_frac_nominal": round(gbs / NOMINAL_HBM_GBS, 4)}
+                res[label] = frac(float(np.median(ms)), 4.0 * T * hkv * 128)
+            if n_l > 1:
+                ms = []
+                for i in range(reps + 3):
+                    a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+                    a.record()
+                    for g2 in gls:
+                        sx.sparse_attn(g2.pool, g2.batch, q, o, rows_R=rows, rows_off=off, total_rows=n)
+                    b.record()
+                    torch.cuda.synchronize()
+                    if i >= 3:
+                        ms.append(a.elapsed_time(b) / n_l)
+                res["tcgen05_splits_chained4"] = frac(float(np.median(ms)), 4.0 * T * hkv * 128)
             out["%s_last%d_rows_%d_pairs_per_kv_head" % (cfg, n, n * hq // hkv)] = res
-        del gl
+        del gls, gl
         torch.cuda.empty_cache()
     del flush
     torch.cuda.empty_cache()
@@ -797,7 +817,7 @@ def run_reference(args):
                        "sample_fraction_of_step": t_sample / total, "est_ms_per_whole_step": round(total * 1e3, 1)},
             "cpu_baseline": {"value": round(v, 2), "unit": UNIT, "cores": cs.cores, "kind": "oracle", "estimated": True,
                              "sample": cs.describe(), "sample_seconds": round(t_sample, 2),
-                             "measured": cpu_measured(cs.orc)},
+                             "measured": (cpu_measured(cs.orc) if not args.no_cpu_measured else None)},
             "e2e": {"value": round(v, 2), "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
             "gpu_launches": 0}
     print(json.dumps(line), flush=True)
@@ -811,6 +831,8 @@ def main():
     ap.add_argument("--config", default="C3", choices=list(wl.CONFIGS) + ["S6"])
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--no-cpu", action="store_true")
+    ap.add_argument("--no-cpu-measured", action="store_true",
+                    help="reference arm: skip the fully timed oracle runs (C1 layer, C2 request)")
     ap.add_argument("--no-others", action="store_true", help="skip the short runs of the other BASELINE configs")
     ap.add_argument("--cta-pair", action="store_true",
                     help="force stage (c) onto 2-CTA clusters (SX_ATTN_CTA_PAIR, tcgen05.mma.cta_group::2)")

@@ -200,18 +200,21 @@ sx_status sx_score_select_ex(const sx_pool *pool, const sx_batch *batch, const v
  *   then its capacity) or = total_tokens (mode 1); q / out / lse are sized by total_rows.
  * O[n][h] = sum_{j <= pos(n)} softmax_j(<q, k_j>/sqrt(128)) v_j with kv head h / g, K and V read
  * through the block tables. Kernels, chosen from host-visible sizes only:
- *   - default: tcgen05 tensor-core tiles, bf16 x bf16 -> fp32 accumulate, fp32 softmax, P rounded to bf16 before
- *     PV. When the row set fills fewer than 148 CTAs (few query tiles against a long context) the key range is
- *     cut into splits whose fp32 partial results are merged in a fixed order; uses ws in that case.
+ *   - general kernel: tcgen05 tensor-core tiles with the query rows on the M dimension, bf16 x bf16 -> fp32
+ *     accumulate, fp32 softmax, P rounded to bf16 before PV. When the row set fills fewer than 148 CTAs (few query
+ *     tiles against a long context) the key range is cut into splits that merge themselves in a fixed order (the
+ *     splits of a row pair wait for one another through an arrival word in ws: one launch); uses ws in that case.
  *   - mode | SX_ATTN_CUDA_CORE: row sets with total_rows * g < 64 * num_reqs (fewer than 64 query rows per
  *     KV head on average; g = Hq/Hkv <= 32) take CUDA-core split-KV kernels, fp32 FMA throughout (the rule of
  *     BASELINE.json north_star; measured slower than the padded tensor-core tile on B200). Uses ws.
- *   - CTA pairs: when the tensor-core path runs without key splits it exists in two forms with the same arithmetic
+ *   - CTA pairs: when the general kernel runs without key splits it exists in two forms with the same arithmetic
  *     per row (hence the same results): one CTA per pair of query tiles, or clusters of two CTAs on adjacent pairs
  *     with M = 256 MMAs (tcgen05.mma.cta_group::2), where every K/V tile is fetched once per cluster, half into
  *     each CTA. Measured (S10): clusters are 1-2 % faster for a batch of ONE request (long uniform
  *     launches) and 5-6 % slower for batches of several requests, so that is the default rule;
  *     mode | SX_ATTN_CTA_PAIR / mode | SX_ATTN_SINGLE_CTA force one or the other.
+ * Every kernel is launched with programmatic dependent launch allowed: its prologue may overlap the tail of the
+ * previous kernel in the stream; it touches global memory only after that kernel has completed.
  * All are deterministic and meet the same tolerance against fp64. */
 sx_status sx_sparse_attn(const sx_pool *pool, const sx_batch *batch, int32_t mode, const void *q,
                          const int32_t *rows_R, const int32_t *rows_off, int32_t total_rows,

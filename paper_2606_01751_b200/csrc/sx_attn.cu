@@ -27,9 +27,13 @@
 //   * causality with a sparse, sorted row list: key tiles run up to the largest position of the
 //     query tile; each row masks keys beyond its own position.
 #include <math.h>
+#include <stdlib.h>
+
+#include <atomic>
 
 #include "sx_internal.h"
 #include "sx_ptx.cuh"
+#include "sx_split_merge.cuh"
 
 namespace sx {
 
@@ -60,6 +64,8 @@ struct AttnParams {
   int kv_splits;     // the key range of a CTA is cut into this many contiguous parts (consecutive blocks)
   float *part_o;     // PV variant with kv_splits > 1: [split][total_rows][Hq][128] normalised partial O (fp32)
   float *part_lse;   //                                 [split][total_rows][Hq]      partial log-sum-exp
+  unsigned long long *tickets;  // kv_splits > 1: one arrival word per (request, KV head, row pair), see split_arrive
+  unsigned long long epoch;     // unique per launch (host counter): words left by earlier launches count as zero
   float scale_log2;  // log2(e) / sqrt(128)
   float scale;       // 1 / sqrt(128)
 };
@@ -118,65 +124,8 @@ attn_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_constant__ CU
   uint8_t *smem = reinterpret_cast<uint8_t *>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~uintptr_t(1023));
   AttnBars *bars = reinterpret_cast<AttnBars *>(smem + Cfg::kOffBar);
 
-  // ---- which (request, KV head, pair of row tiles) is this CTA; heavy (late) pairs of a request first
   const int g = p.group, rpt = p.rows_per_tile, rpc = 2 * rpt;
   const int rank = kPair ? (int)cluster_ctarank() : 0;
-  // consecutive blocks share a (request, KV head, row pair) and take one key split each
-  // (kPair: consecutive blocks are the two CTAs of a cluster and take adjacent row pairs)
-  const int split = kPair ? 0 : (int)blockIdx.x % p.kv_splits;
-  const int bid = kPair ? (int)blockIdx.x >> 1 : (int)blockIdx.x / p.kv_splits;
-  int req = 0, base = 0, pairs = 0, n_r = 0, units = 0;
-  for (; req < p.num_reqs; ++req) {
-    n_r = p.rows_off[req + 1] - p.rows_off[req];
-    pairs = (n_r + rpc - 1) / rpc;
-    units = kPair ? (pairs + 1) / 2 : pairs;
-    if (bid < base + units * p.num_kv_heads) break;
-    base += units * p.num_kv_heads;
-  }
-  if (req >= p.num_reqs) return;  // (both CTAs of a cluster leave together)
-  const int local = bid - base;
-  const int kvh = local % p.num_kv_heads;
-  // kPair: rank 0 takes the later pair; with an odd number of pairs the last cluster's rank 1 has no rows
-  // (pair = -1) and only stages its halves of K/V and runs masked softmax tiles
-  const int pair = kPair ? pairs - 1 - (2 * (local / p.num_kv_heads) + rank) : pairs - 1 - local / p.num_kv_heads;
-  const int row_base = pair >= 0 ? p.rows_off[req] + pair * rpc : p.total_rows;  // first row of query tile 0
-  const int T = p.seq_len[req];
-  const int n_pages = (T + kPage - 1) / kPage;
-  // valid rows and number of key tiles of each query tile of row pair `pr`
-  auto tile_info = [&](int pr, int (&nr)[2], int (&nt)[2]) {
-    const int cta_rows = pr >= 0 ? min(rpc, n_r - pr * rpc) : 0;
-    nr[0] = min(rpt, cta_rows);
-    nr[1] = cta_rows - nr[0];
-#pragma unroll
-    for (int i = 0; i < 2; ++i) {
-      if (nr[i] > 0) {
-        const int last = p.rows_off[req] + pr * rpc + i * rpt + nr[i] - 1;
-        const int pos_max = p.rows ? p.rows[last] : last - p.rows_off[req];
-        nt[i] = pos_max / kTile + 1;
-      } else {
-        nt[i] = 0;
-      }
-    }
-  };
-  int nrows[2], n_t[2];
-  tile_info(pair, nrows, n_t);
-  if (kPair) {  // the cluster's common tile counts (rank 0 holds the later rows, but tile i of either may lead)
-    int nr_o[2], nt_o[2];
-    tile_info(pair + (rank ? 1 : -1), nr_o, nt_o);
-    n_t[0] = max(n_t[0], nt_o[0]);
-    n_t[1] = max(n_t[1], nt_o[1]);
-  }
-  // key tiles [t0, t0 + n_tiles) of this CTA; n_t[i] and every loop below count tiles from t0
-  int t0 = 0;
-  if (!kPair && p.kv_splits > 1) {
-    const int all = max(n_t[0], n_t[1]);
-    const int per = (all + p.kv_splits - 1) / p.kv_splits;
-    t0 = split * per;
-    n_t[0] = max(0, min(n_t[0], t0 + per) - t0);
-    n_t[1] = max(0, min(n_t[1], t0 + per) - t0);
-  }
-  const int n_tiles = max(n_t[0], n_t[1]);
-
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
   // Roles. The SM sub-partition arbiter favours the highest warp id among eligible warps, so the
   // latency-critical single-thread roles take the highest ids of their sub-partition:
@@ -184,6 +133,9 @@ attn_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_constant__ CU
   //   warp 8: TMA producer (Q, even ring items), warp 9: MMA issuer, warp 10: TMA producer (odd items).
   constexpr int kWarpProd0 = 8, kWarpMma = 9, kWarpProd1 = 10;
 
+  // ---- prologue that touches no global memory: it may overlap the tail of the previous kernel in the stream
+  // (programmatic dependent launch); the next kernel's prologue may in turn overlap this kernel
+  griddep_launch();
   if (warp == kWarpProd0 && lane == 0) {
     tma_prefetch_desc(&tm_q);
     tma_prefetch_desc(&tm_k);
@@ -224,11 +176,75 @@ attn_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_constant__ CU
     }
     fence_proxy_async_smem();
   }
+  griddep_wait();  // from here on: global memory (row lists, tables, pools may be outputs of the previous kernel)
+
+  // ---- which (request, KV head, pair of row tiles) is this CTA; heavy (late) pairs of a request first
+  // consecutive blocks share a (request, KV head, row pair) and take one key split each
+  // (kPair: consecutive blocks are the two CTAs of a cluster and take adjacent row pairs)
+  const int split = kPair ? 0 : (int)blockIdx.x % p.kv_splits;
+  const int bid = kPair ? (int)blockIdx.x >> 1 : (int)blockIdx.x / p.kv_splits;
+  int req = 0, base = 0, pairs = 0, n_r = 0, units = 0;
+  for (; req < p.num_reqs; ++req) {
+    n_r = p.rows_off[req + 1] - p.rows_off[req];
+    pairs = (n_r + rpc - 1) / rpc;
+    units = kPair ? (pairs + 1) / 2 : pairs;
+    if (bid < base + units * p.num_kv_heads) break;
+    base += units * p.num_kv_heads;
+  }
+  const bool active = req < p.num_reqs;  // (the grid is an upper bound; both CTAs of a cluster agree)
+  if (!active) req = 0;
+  const int local = active ? bid - base : 0;
+  const int kvh = local % p.num_kv_heads;
+  // kPair: rank 0 takes the later pair; with an odd number of pairs the last cluster's rank 1 has no rows
+  // (pair = -1) and only stages its halves of K/V and runs masked softmax tiles
+  const int pair = !active ? -1
+                           : (kPair ? pairs - 1 - (2 * (local / p.num_kv_heads) + rank) : pairs - 1 - local / p.num_kv_heads);
+  const int row_base = pair >= 0 ? p.rows_off[req] + pair * rpc : p.total_rows;  // first row of query tile 0
+  const int T = p.seq_len[req];
+  const int n_pages = (T + kPage - 1) / kPage;
+  // valid rows and number of key tiles of each query tile of row pair `pr`
+  auto tile_info = [&](int pr, int (&nr)[2], int (&nt)[2]) {
+    const int cta_rows = pr >= 0 ? min(rpc, n_r - pr * rpc) : 0;
+    nr[0] = min(rpt, cta_rows);
+    nr[1] = cta_rows - nr[0];
+#pragma unroll
+    for (int i = 0; i < 2; ++i) {
+      if (nr[i] > 0) {
+        const int last = p.rows_off[req] + pr * rpc + i * rpt + nr[i] - 1;
+        const int pos_max = p.rows ? p.rows[last] : last - p.rows_off[req];
+        nt[i] = pos_max / kTile + 1;
+      } else {
+        nt[i] = 0;
+      }
+    }
+  };
+  int nrows[2], n_t[2];
+  tile_info(pair, nrows, n_t);
+  if (kPair && active) {  // the cluster's common tile counts (rank 0 holds the later rows, but tile i of either may lead)
+    int nr_o[2], nt_o[2];
+    tile_info(pair + (rank ? 1 : -1), nr_o, nt_o);
+    n_t[0] = max(n_t[0], nt_o[0]);
+    n_t[1] = max(n_t[1], nt_o[1]);
+  }
+  // key tiles [t0, t0 + n_tiles) of this CTA; n_t[i] and every loop below count tiles from t0
+  int t0 = 0;
+  if (!kPair && p.kv_splits > 1) {
+    const int all = max(n_t[0], n_t[1]);
+    const int per = (all + p.kv_splits - 1) / p.kv_splits;
+    t0 = split * per;
+    n_t[0] = max(0, min(n_t[0], t0 + per) - t0);
+    n_t[1] = max(0, min(n_t[1], t0 + per) - t0);
+  }
+  const int n_tiles = max(n_t[0], n_t[1]);
+
   tc_fence_before();
   if (kPair) cluster_sync(); else __syncthreads();
   tc_fence_after();
   const uint32_t tmem = bars->tmem_base;
 
+  if (!active) {
+    // nothing to do (grid overshoot): fall through to the common exit
+  } else
   if (warp >= 8) {
     setmaxnreg_dec<56>();
     if (warp == kWarpProd0 || warp == kWarpProd1) {
@@ -623,6 +639,23 @@ attn_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_constant__ CU
       }
       // a split that holds no visible key of the row reports -inf: the merge skips its (undefined) O
       if (valid) p.part_lse[prow] = (my_tiles > 0 && m_used > -INFINITY) ? m_used * p.scale + logf(l) : -INFINITY;
+      // ---- fused merge: when every split of this (request, KV head, row pair) has arrived, each of them
+      // combines its share of the (row, head) pairs
+      __threadfence();
+      named_bar_sync(2, 256);
+      if (threadIdx.x == 0) {
+        split_arrive(p.tickets + bid, p.epoch);
+        split_wait_all(p.tickets + bid, p.epoch, p.kv_splits);
+        __threadfence();
+      }
+      named_bar_sync(2, 256);
+      const int n_pairs = (nrows[0] + nrows[1]) * g;  // (row, head) pairs of this row pair, rows consecutive in R
+      const size_t stride = (size_t)p.total_rows * p.num_q_heads;
+      for (int pi = split + p.kv_splits * warp; pi < n_pairs; pi += 8 * p.kv_splits) {
+        const int rl = pi / g, hl = pi - rl * g;
+        merge_splits(p.part_o, p.part_lse, p.kv_splits, stride, (size_t)(row_base + rl) * p.num_q_heads + kvh * g + hl,
+                     lane, p.out, p.lse);
+      }
     } else if (my_tiles > 0 || !kWithPV) {  // (an LSE key split that holds no tile of the row still reports -inf)
       if (kWithPV) {
         mbar_wait(&bars->o_full[qt], 0);
@@ -662,56 +695,28 @@ attn_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_constant__ CU
   }
 }
 
-// Combine the key splits of attn_kernel<true>: out = sum_s exp(lse_s - lse) O_s, in the fixed order 0..splits-1.
-// One warp per (row, head), lane = 4 output dims: every load of the loop is independent of the others, so the
-// splits stream in with many requests in flight instead of one latency after the other.
-__global__ void __launch_bounds__(256)
-attn_merge_kernel(const float *__restrict__ part_o, const float *__restrict__ part_lse, int splits, int total_rows,
-                  int num_q_heads, const int32_t *__restrict__ rows_off, int num_reqs, __nv_bfloat16 *__restrict__ out,
-                  float *__restrict__ lse) {
-  const size_t rh = (size_t)blockIdx.x * 8 + (threadIdx.x >> 5);  // (row, head) index
-  const int lane = threadIdx.x & 31;
-  if (rh >= (size_t)rows_off[num_reqs] * num_q_heads) return;
-  const size_t stride = (size_t)total_rows * num_q_heads;
-  float mx = -INFINITY;
-  for (int s = lane; s < splits; s += 32) mx = fmaxf(mx, __ldg(part_lse + s * stride + rh));
-#pragma unroll
-  for (int d = 16; d > 0; d >>= 1) mx = fmaxf(mx, __shfl_xor_sync(0xffffffffu, mx, d));
-  float4 o = make_float4(0.f, 0.f, 0.f, 0.f);
-  float den = 0.f;
-#pragma unroll 8
-  for (int s = 0; s < splits; ++s) {
-    const float ls = __ldg(part_lse + s * stride + rh);
-    const float4 v = __ldg(reinterpret_cast<const float4 *>(part_o + (s * stride + rh) * kHeadDim) + lane);
-    if (ls != -INFINITY) {  // a split without a visible key of the row holds an undefined O: skipped
-      const float w = __expf(ls - mx);
-      den += w;
-      o.x = fmaf(v.x, w, o.x);
-      o.y = fmaf(v.y, w, o.y);
-      o.z = fmaf(v.z, w, o.z);
-      o.w = fmaf(v.w, w, o.w);
-    }
-  }
-  const float inv = 1.f / den;
-  uint2 pk;
-  pk.x = pack_bf16x2(o.x * inv, o.y * inv);
-  pk.y = pack_bf16x2(o.z * inv, o.w * inv);
-  reinterpret_cast<uint2 *>(out + rh * kHeadDim)[lane] = pk;
-  if (lse && lane == 0) lse[rh] = mx + logf(den);
-}
-
 // Row sets that fill tensor-core tiles but only a few CTAs (a handful of query tiles against a long context):
 // cut the key range so that ONE wave of CTAs exists (225 KB of shared memory: one CTA per SM; a few CTAs
-// spilling into a second wave would double the time); partial results are merged by attn_merge_kernel.
-// The partial buffer bounds splits * total_rows * Hq (each CTA covers at most 256 (row, head) pairs).
+// spilling into a second wave would double the time); the partial results are merged by the split that finishes
+// splits themselves once all of a row pair have arrived (split_arrive / merge_splits). The partial buffer bounds splits * total_rows * Hq (each CTA covers at most
+// 256 (row, head) pairs); one ticket word per (request, KV head, row pair) follows it.
 constexpr int kAttnSplitCtas = 148;
-size_t attn_part_bytes() { return (size_t)2 * kAttnSplitCtas * 256 * (kHeadDim + 1) * sizeof(float); }
+constexpr size_t kAttnPartFloats = (size_t)2 * kAttnSplitCtas * 256 * (kHeadDim + 1);
+size_t attn_part_bytes() { return kAttnPartFloats * sizeof(float) + kAttnSplitCtas * sizeof(unsigned long long); }
+unsigned long long *attn_tickets(float *part) { return reinterpret_cast<unsigned long long *>(part + kAttnPartFloats); }
+unsigned long long next_split_epoch() {
+  static std::atomic<unsigned long long> epoch{0};
+  return (epoch.fetch_add(1, std::memory_order_relaxed) + 1) & ((1ull << 56) - 1);
+}
 
 int attn_pv_splits(const sx_pool *pool, const sx_batch *b, int32_t total_rows) {
   const int g = pool->num_q_heads / pool->num_kv_heads;
   const int grid = (total_rows / (2 * (kTile / g)) + b->num_reqs) * pool->num_kv_heads;
   if (grid >= 148) return 1;
   int s = kAttnSplitCtas / grid;
+#ifdef SX_TUNING
+  if (const char *e = getenv("SX_ATTN_SPLITS")) if (atoi(e) > 0) s = atoi(e);
+#endif
   const int tiles = (b->max_seq_len + kTile - 1) / kTile;
   if (s > tiles / 2) s = tiles / 2;  // at least two key tiles per split
   if (s > 64) s = 64;
@@ -759,6 +764,8 @@ sx_status launch_attn(const sx_pool *pool, const sx_batch *b, bool with_pv, cons
   p.kv_splits = kv_splits < 1 ? 1 : kv_splits;
   p.part_o = part;
   p.part_lse = part ? part + (size_t)p.kv_splits * total_rows * pool->num_q_heads * kHeadDim : nullptr;
+  p.tickets = part ? attn_tickets(part) : nullptr;
+  p.epoch = part ? next_split_epoch() : 0;
   p.scale = (float)(1.0 / sqrt((double)kHeadDim));
   p.scale_log2 = (float)(kLog2e / sqrt((double)kHeadDim));
   const int grid = (total_rows / (2 * rpt) + b->num_reqs) * pool->num_kv_heads;  // >= sum_r ceil(n_r / 2rpt) * Hkv
@@ -768,40 +775,24 @@ sx_status launch_attn(const sx_pool *pool, const sx_batch *b, bool with_pv, cons
     e = cudaFuncSetAttribute(attn_kernel<true, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, AttnCfg::kSmemBytes);
     if (e != cudaSuccess) return set_error(SX_ERR_CUDA, "attn smem attr: %s", cudaGetErrorString(e));
     const int clusters = (total_rows / (4 * rpt) + b->num_reqs) * pool->num_kv_heads;
-    cudaLaunchConfig_t cfg = {};
-    cfg.gridDim = dim3(2 * clusters);
-    cfg.blockDim = dim3(kAttnThreads);
-    cfg.dynamicSmemBytes = AttnCfg::kSmemBytes;
-    cfg.stream = st;
-    cudaLaunchAttribute attr[1];
-    attr[0].id = cudaLaunchAttributeClusterDimension;
-    attr[0].val.clusterDim.x = 2;
-    attr[0].val.clusterDim.y = 1;
-    attr[0].val.clusterDim.z = 1;
-    cfg.attrs = attr;
-    cfg.numAttrs = 1;
-    e = cudaLaunchKernelEx(&cfg, attn_kernel<true, true>, tm_q, tm_k, tm_v, p);
+    e = launch_pdl(attn_kernel<true, true>, dim3(2 * clusters), dim3(kAttnThreads), AttnCfg::kSmemBytes, st, 2, tm_q,
+                   tm_k, tm_v, p);
     if (e != cudaSuccess) return set_error(SX_ERR_CUDA, "attn pair launch: %s", cudaGetErrorString(e));
     return check_launch("attn_kernel<pv,pair>");
   }
   if (with_pv) {
     e = cudaFuncSetAttribute(attn_kernel<true, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, AttnCfg::kSmemBytes);
     if (e != cudaSuccess) return set_error(SX_ERR_CUDA, "attn smem attr: %s", cudaGetErrorString(e));
-    attn_kernel<true, false><<<grid * p.kv_splits, kAttnThreads, AttnCfg::kSmemBytes, st>>>(tm_q, tm_k, tm_v, p);
-    if (p.kv_splits > 1) {
-      sx_status ms = check_launch("attn_kernel<pv>");
-      if (ms != SX_OK) return ms;
-      const int blocks = (int)(((size_t)total_rows * pool->num_q_heads + 7) / 8);
-      attn_merge_kernel<<<blocks, 256, 0, st>>>(p.part_o, p.part_lse, p.kv_splits, total_rows, pool->num_q_heads, rows_off,
-                                                b->num_reqs, p.out, lse);
-      return check_launch("attn_merge_kernel");
-    }
+    e = launch_pdl(attn_kernel<true, false>, dim3(grid * p.kv_splits), dim3(kAttnThreads), AttnCfg::kSmemBytes, st, 1,
+                   tm_q, tm_k, tm_v, p);
   } else {
     e = cudaFuncSetAttribute(attn_kernel<false, false>, cudaFuncAttributeMaxDynamicSharedMemorySize,
                              AttnCfg::kSmemBytes);
     if (e != cudaSuccess) return set_error(SX_ERR_CUDA, "lse smem attr: %s", cudaGetErrorString(e));
-    attn_kernel<false, false><<<grid * p.kv_splits, kAttnThreads, AttnCfg::kSmemBytes, st>>>(tm_q, tm_k, tm_v, p);
+    e = launch_pdl(attn_kernel<false, false>, dim3(grid * p.kv_splits), dim3(kAttnThreads), AttnCfg::kSmemBytes, st, 1,
+                   tm_q, tm_k, tm_v, p);
   }
+  if (e != cudaSuccess) return set_error(SX_ERR_CUDA, "attn launch: %s", cudaGetErrorString(e));
   return check_launch(with_pv ? "attn_kernel<pv>" : "attn_kernel<lse>");
 }
 

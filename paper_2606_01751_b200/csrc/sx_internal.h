@@ -50,6 +50,8 @@ sx_status launch_attn(const sx_pool *pool, const sx_batch *b, bool with_pv, cons
                       float *part, bool cta_pair, cudaStream_t st);
 int attn_pv_splits(const sx_pool *pool, const sx_batch *b, int32_t total_rows);
 size_t attn_part_bytes();
+unsigned long long *attn_tickets(float *part);  // arrival words of the key splits, behind the partial buffer
+unsigned long long next_split_epoch();          // unique per split launch in this process (sx_split_merge.cuh)
 int attn_lse_splits(const sx_pool *pool, const sx_batch *b, int32_t total_rows);
 // CUDA-core split-KV attention for fewer than 64 (row, head) pairs per KV head; part = ws.small_part
 sx_status launch_attn_small(const sx_pool *pool, const sx_batch *b, const void *q, const int32_t *rows,
@@ -69,5 +71,32 @@ sx_status run_check_rows(const sx_batch *b, const int32_t *rows, const int32_t *
 sx_status make_tmap_pool(CUtensorMap *out, const void *base, int num_blocks, int num_kv_heads);
 sx_status make_tmap_q(CUtensorMap *out, const void *base, int total_rows, int num_q_heads, int group,
                       int rows_per_tile);
+
+// Launch with programmatic dependent launch allowed (and optionally a cluster dimension): the kernel must call
+// griddep_wait() (sx_ptx.cuh) before its first global-memory access.
+template <typename... KArgs, typename... Args>
+inline cudaError_t launch_pdl(void (*kern)(KArgs...), dim3 grid, dim3 block, size_t smem, cudaStream_t st, int cluster,
+                              Args &&...args) {
+  cudaLaunchConfig_t cfg = {};
+  cfg.gridDim = grid;
+  cfg.blockDim = block;
+  cfg.dynamicSmemBytes = smem;
+  cfg.stream = st;
+  cudaLaunchAttribute attr[2];
+  int n = 0;
+  attr[n].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+  attr[n].val.programmaticStreamSerializationAllowed = 1;
+  ++n;
+  if (cluster > 1) {
+    attr[n].id = cudaLaunchAttributeClusterDimension;
+    attr[n].val.clusterDim.x = cluster;
+    attr[n].val.clusterDim.y = 1;
+    attr[n].val.clusterDim.z = 1;
+    ++n;
+  }
+  cfg.attrs = attr;
+  cfg.numAttrs = n;
+  return cudaLaunchKernelEx(&cfg, kern, static_cast<KArgs>(args)...);
+}
 
 }  // namespace sx

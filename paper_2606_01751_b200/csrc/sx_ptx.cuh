@@ -53,10 +53,17 @@ __device__ __forceinline__ bool mbar_try_wait_hint(uint64_t *bar, uint32_t parit
 }
 // Spin with a watchdog: a protocol bug traps (launch error) instead of hanging the GPU. The watchdog counts
 // polls (one add and compare per poll; a clock64 comparison had been a third of the waiting warps' instructions).
+#ifndef SX_WAIT_HINT
+#define SX_WAIT_HINT 2000
+#endif
 __device__ __forceinline__ void mbar_wait(uint64_t *bar, uint32_t parity) {
   if (mbar_try_wait(bar, parity)) return;
   uint32_t polls = 0;
-  while (!mbar_try_wait_hint(bar, parity, 2000u)) {
+#if SX_WAIT_HINT > 0
+  while (!mbar_try_wait_hint(bar, parity, SX_WAIT_HINT)) {
+#else
+  while (!mbar_try_wait(bar, parity)) {
+#endif
     if (++polls > (1u << 26)) __trap();  // seconds, whatever the hint is worth
   }
 }
@@ -362,6 +369,15 @@ __device__ __forceinline__ float lds_f1(uint32_t saddr) {
   asm volatile("ld.shared.f32 %0, [%1];" : "=f"(v) : "r"(saddr));
   return v;
 }
+
+// ------------------------------------------------------------------------------------ programmatic dependent launch
+// A kernel launched with cudaLaunchAttributeProgrammaticStreamSerialization may start while its predecessor in the
+// stream still runs, once every CTA of the predecessor has executed griddep_launch() (or exited). It must call
+// griddep_wait() before it touches ANY global memory (the wait returns when the predecessor grid has completed and
+// its writes are visible); everything before the wait (barrier init, TMEM allocation, tensor-map prefetch) overlaps
+// the predecessor's tail. Without the launch attribute both are no-ops.
+__device__ __forceinline__ void griddep_wait() { asm volatile("griddepcontrol.wait;" ::: "memory"); }
+__device__ __forceinline__ void griddep_launch() { asm volatile("griddepcontrol.launch_dependents;" ::: "memory"); }
 
 // ------------------------------------------------------------------------------------ misc math
 __device__ __forceinline__ float ex2_approx(float x) {

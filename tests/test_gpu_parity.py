@@ -278,13 +278,14 @@ SMALL_CASES = {
 }
 
 
-@pytest.mark.parametrize("cuda_core", [True, False], ids=["cuda-core", "tcgen05-splits"])
+@pytest.mark.parametrize("path", ["cuda-core", "tcgen05-splits"])
 @pytest.mark.parametrize("case", list(SMALL_CASES))
-def test_small_row_sets(case, cuda_core):
+def test_small_row_sets(case, path):
     """Fewer than 64 (row, head) pairs per KV head: with SX_ATTN_CUDA_CORE sx_sparse_attn takes the CUDA-core
-    split-KV kernels (the north_star rule), by default the padded tensor-core tile with key splits (measured
-    faster on B200); same definition O-c, same tolerance on both."""
+    split-KV kernels (the north_star rule), by default the padded tensor-core tile with key splits that merge
+    themselves in one launch (measured faster on B200); same definition O-c, same tolerance on both."""
     GpuLayer, dev_to_bits = _gpu()
+    cuda_core = path == "cuda-core"
     name, pick = SMALL_CASES[case]
     lay, lt, res, pk, pv, kt, vt = prepared(name)
     g = GpuLayer(lay, lt)
@@ -383,7 +384,8 @@ def test_overflow_and_tail_fallback(ov, tail, prefix):
 @pytest.mark.parametrize("name,nlast", [("C5-1/16", 16), ("C1", 40), ("C3-eighth", 24)])
 def test_few_rows_tensor_core_path_with_key_splits(name, nlast):
     """At least 64 (row, head) pairs per KV head but only a few query tiles against a long context: the tcgen05
-    kernel cuts the key range into splits (partial O and LSE in the workspace) and merges them."""
+    kernel cuts the key range into splits (partial O and LSE in the workspace) that merge themselves in fixed order
+    once all splits of a row pair have arrived."""
     GpuLayer, dev_to_bits = _gpu()
     lay, lt, res, pk, pv, kt, vt = prepared(name)
     g = GpuLayer(lay, lt)
@@ -560,3 +562,31 @@ def test_copy_on_write_two_layers_each_with_its_own_tables():
         gs.append(g)
     with pytest.raises(sx.SparseXError):
         sx.rope_realign_layers([g.pool for g in gs], gs[0].batch)
+
+
+@pytest.mark.parametrize("nrows", [3, 14, 30])
+def test_reference_moves_and_rescales_with_key_splits(nrows):
+    """The attention kernel rescales O lazily (only when a row maximum grows by more than 2^24). Keys whose norm
+    grows with the position (x1 ... x8) make later tiles exceed the reference of earlier ones many times over, in
+    every row and in every key split; rows in the middle of the context exercise the causal mask inside a tile."""
+    GpuLayer, dev_to_bits = _gpu()
+    lay, lt, res, pk, pv, kt, vt = prepared("C1")
+    t = int(lay.seq_len[0])
+    pk = pk.copy()
+    for pos in range(t):                       # key norm grows stepwise with the position
+        scale = 1.0 + 7.0 * (pos // 256) / (t // 256 - 1)
+        blk, off = int(kt[0][pos // 16]), pos % 16
+        pk[blk, :, off, :] = orc.f64_to_bf16(orc.bf16_to_f64(pk[blk, :, off, :]) * scale)
+    g = GpuLayer(lay, lt)
+    g.pool_k.copy_(torch.from_numpy(pk.view(np.int16)))
+    g.pool_v.copy_(torch.from_numpy(pv.view(np.int16)))
+    rows = np.unique(np.concatenate([np.arange(t - nrows + 2, t), [700, t // 2 + 5]])).astype(np.int32)
+    assert len(rows) == nrows
+    g.rows_off = torch.tensor([0, len(rows)], dtype=torch.int32, device=g.dev)
+    g.sel_off = torch.zeros(2, dtype=torch.int32, device=g.dev)
+    g.stage_rows(torch.zeros(0, dtype=torch.int32, device=g.dev), torch.from_numpy(rows).to(g.dev))
+    g.attend()
+    torch.cuda.synchronize()
+    ref_o, ref_l = orc.attention(pk, pv, kt[0], vt[0], t, lt.q_full[rows], rows, lay.num_q_heads, want_lse=True)
+    check_close("key splits, growing key norms", orc.bf16_to_f64(dev_to_bits(g.out)), ref_o)
+    assert np.max(np.abs(g.lse.cpu().numpy().astype(np.float64) - ref_l)) < 2e-3

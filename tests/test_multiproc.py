@@ -43,11 +43,12 @@ def test_reference_arm_rank0_only():
     for rank in (0, 1):
         env["RANK"] = str(rank)
         r = subprocess.run([sys.executable, os.path.join(ROOT, "bench.py"), "--impl", "reference", "--config", "C1",
-                            "--steps", "1", "--warmup", "0", "--gpus", "2", "--cpu-seconds", "1"],
+                            "--steps", "1", "--warmup", "0", "--gpus", "2", "--no-cpu-measured"],
                            env=env, capture_output=True, text=True, timeout=300)
         assert r.returncode == 0, r.stderr
         outs.append(r.stdout.strip())
     line = json.loads(outs[0].splitlines()[-1])
     assert line["impl"] == "reference" and line["n_gpus"] == 2 and line["value"] > 0
     assert line["cpu_baseline"]["kind"] == "oracle" and line["e2e"]["h2d_bytes_per_step"] == 0
+    assert line["estimated"] is True and 0 < line["config"]["sample_fraction_of_step"] <= 1.0
     assert outs[1] == ""
