@@ -300,9 +300,8 @@ sx_status sx_score_select_ex(const sx_pool *pool, const sx_batch *batch, const v
   if (batch->total_new > 0) {
     if (!lse) {  // sweep 1: row normaliser of Eq. (1) for the Sparse-Q rows
       float *lse_ws = reinterpret_cast<float *>(base + w.lse_new);
-      lse_splits = attn_lse_splits(pool, batch, batch->total_new);
-      st = launch_attn(pool, batch, /*with_pv=*/false, q_new, batch->new_idx, batch->new_off, batch->total_new,
-                       nullptr, lse_ws, lse_splits, nullptr, /*cta_pair=*/false, s);
+      lse_splits = sx::lse_splits(pool, batch);
+      st = launch_lse(pool, batch, q_new, lse_ws, lse_splits, s);
       if (st != SX_OK) return st;
       lse = lse_ws;
       lse_by_token = 0;
@@ -374,7 +373,7 @@ sx_status sx_sparse_attn(const sx_pool *pool, const sx_batch *batch, int32_t mod
     if (st != SX_OK) return st;
     part = reinterpret_cast<float *>(static_cast<char *>(ws) + ws_layout(pool, batch).attn_part);
   }
-  return launch_attn(pool, batch, true, q, rows_R, rows_off, total_rows, out, lse, splits, part, want_cta_pair, s);
+  return launch_attn(pool, batch, q, rows_R, rows_off, total_rows, out, lse, splits, part, want_cta_pair, s);
 }
 
 }  // extern "C"

@@ -1,8 +1,7 @@
 // sx_attn.cu -- stage (c): causal attention of the sparse query set R over the full paged K/V
 //   O[R] = SparseAttn(Q[R], K_cur[1:T], V_cur[1:T], M_causal)          Alg. 1 l.546-548 (sparse)
 //   full causal attention on all positions                                Alg. 1 l.507-511 (layers <= l*)
-// and, with kWithPV = false, the first sweep of stage (b): the softmax normaliser (log-sum-exp) of
-// the Sparse-Q rows of Eq. (1).
+// (The first sweep of stage (b), the log-sum-exp of the Sparse-Q rows, has its own kernel: sx_lse.cu.)
 //
 // tcgen05 design, one CTA per (request, KV head, PAIR of 128-row query tiles):
 //   * GQA packing: the M = 128 rows of a query tile are (row of R, query head of the KV group)
@@ -64,8 +63,7 @@ struct AttnParams {
   int kv_splits;     // the key range of a CTA is cut into this many contiguous parts (consecutive blocks)
   float *part_o;     // PV variant with kv_splits > 1: [split][total_rows][Hq][128] normalised partial O (fp32)
   float *part_lse;   //                                 [split][total_rows][Hq]      partial log-sum-exp
-  unsigned long long *tickets;  // kv_splits > 1: one arrival word per (request, KV head, row pair), see split_arrive
-  unsigned long long epoch;     // unique per launch (host counter): words left by earlier launches count as zero
+  unsigned long long *tickets;  // kv_splits > 1: one rendezvous word per (request, KV head, row pair), see split_arrive
   float scale_log2;  // log2(e) / sqrt(128)
   float scale;       // 1 / sqrt(128)
 };
@@ -80,43 +78,23 @@ struct AttnCfg {
 struct AttnBars {
   uint64_t q_full;
   uint64_t kv_full[kKvStagesPair], kv_empty[kKvStagesPair];
-  uint64_t s_full[2][2];  // [query tile][buffer]: S = Q K^T landed in TMEM   (buffer 1: LSE-only variant)
-  uint64_t s_free[2][2];  // softmax -> MMA. PV variant: [0] all of P written, [1] S is in registers;
-                          // LSE-only: S of buffer b consumed. 128 arrivals
-  uint64_t p_half[2];     // softmax -> MMA: keys [0, 64) of P written (PV variant); 128 arrivals
+  uint64_t s_full[2];     // [query tile]: S = Q K^T landed in TMEM
+  uint64_t s_free[2][2];  // softmax -> MMA: [i][0] all of P_i written, [i][1] S_i is in registers; 128 arrivals
+  uint64_t p_half[2];     // softmax -> MMA: keys [0, 64) of P written; 128 arrivals
   uint64_t o_full[2];     // last PV of the query tile completed
   uint64_t v_landed;      // CTA-pair variant: the V tile that holds keys >= T is in shared memory (both CTAs)
   uint32_t tmem_base;
 };
-
-// exp2 on the FMA pipe for two values at once: x = n + f, n = rint(x), |f| <= 1/2;
-// 2^f by a cubic (max relative error 7.5e-5, below the bf16 rounding of P), 2^n by exponent arithmetic.
-__device__ __forceinline__ float2 ex2_poly2(float2 x) {
-  const float kMagic = 12582912.f;  // 1.5 * 2^23: adding it leaves rint(x) in the low mantissa bits
-  x.x = fmaxf(x.x, -126.f);
-  x.y = fmaxf(x.y, -126.f);
-  const float2 t = __fadd2_rn(x, make_float2(kMagic, kMagic));
-  const float2 n = __fadd2_rn(t, make_float2(-kMagic, -kMagic));
-  const float2 f = __ffma2_rn(n, make_float2(-1.f, -1.f), x);
-  float2 p = __ffma2_rn(make_float2(0.0551716648f, 0.0551716648f), f, make_float2(0.2426111251f, 0.2426111251f));
-  p = __ffma2_rn(p, f, make_float2(0.6932609677f, 0.6932609677f));
-  p = __ffma2_rn(p, f, make_float2(0.9999280572f, 0.9999280572f));
-  float2 r;
-  r.x = __int_as_float(__float_as_int(p.x) + (__float_as_int(t.x) << 23));
-  r.y = __int_as_float(__float_as_int(p.y) + (__float_as_int(t.y) << 23));
-  return r;
-}
 
 // kPair (PV variant without key splits): a cluster of two CTAs works on two ADJACENT pairs of query tiles of one
 // (request, KV head) with tcgen05.mma.cta_group::2 (M = 256): every K/V tile is fetched once per cluster, each
 // CTA staging half of it (K: 64 of the 128 keys; V: 64 of the 128 dims), so L2 -> SM traffic and the
 // shared-memory operand reads of B are halved. CTA rank 0 issues all MMAs; both CTAs run the softmax of their own
 // rows over the cluster's common number of key tiles (rows with fewer visible keys see fully masked tiles).
-template <bool kWithPV, bool kPair>
+template <bool kPair>
 __global__ void __launch_bounds__(kAttnThreads, 1)
 attn_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_constant__ CUtensorMap tm_k,
             const __grid_constant__ CUtensorMap tm_v, const AttnParams p) {
-  static_assert(kWithPV || !kPair, "the CTA-pair variant exists for the PV kernel only");
   using Cfg = AttnCfg;
   constexpr int kStages = kPair ? kKvStagesPair : kKvStages;
   constexpr int kStageBytes = kPair ? kHalfBytes : kTileBytes;  // bytes of one ring item in THIS CTA
@@ -139,7 +117,7 @@ attn_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_constant__ CU
   if (warp == kWarpProd0 && lane == 0) {
     tma_prefetch_desc(&tm_q);
     tma_prefetch_desc(&tm_k);
-    if (kWithPV) tma_prefetch_desc(&tm_v);
+    tma_prefetch_desc(&tm_v);
     mbar_init(&bars->q_full, 1);
     for (int i = 0; i < kStages; ++i) {
       mbar_init(&bars->kv_full[i], 1);
@@ -147,10 +125,8 @@ attn_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_constant__ CU
     }
     // kPair: the softmax threads of BOTH CTAs arrive on rank 0's p_half / s_free
     for (int i = 0; i < 2; ++i) {
-      for (int b = 0; b < 2; ++b) {
-        mbar_init(&bars->s_full[i][b], 1);
-        mbar_init(&bars->s_free[i][b], kPair ? 8 : 128);
-      }
+      mbar_init(&bars->s_full[i], 1);
+      for (int b = 0; b < 2; ++b) mbar_init(&bars->s_free[i][b], kPair ? 8 : 128);
       mbar_init(&bars->o_full[i], 1);
       mbar_init(&bars->p_half[i], kPair ? 8 : 128);
     }
@@ -276,14 +252,14 @@ attn_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_constant__ CU
       // kPair: 8 boxes per item: K item = this CTA's 64 keys (4 pages) x both halves -> [half][64 keys][128 B],
       //        the keys being 32 of each 64-key half of the tile: pages {2r, 2r+1, 4+2r, 5+2r} for rank r;
       //        V item = all 8 pages x the CTA's own 64-column half -> [128 keys][128 B].
-      const int n_items = kWithPV ? 2 * n_tiles : n_tiles;
+      const int n_items = 2 * n_tiles;
       const int pgi = lane >> 1;
       const int pg_k = kPair ? 2 * rank + (pgi & 1) + 4 * (pgi >> 1) : pgi, half_k = lane & 1;
       const int pg_v = kPair ? lane : (lane >> 1), half_v = kPair ? rank : (lane & 1);
       const int n_boxes = kPair ? 8 : 16;
       auto table_entry = [&](int it) -> int {
-        const int t = t0 + (kWithPV ? (it >> 1) : it);
-        const bool is_v = kWithPV && (it & 1);
+        const int t = t0 + (it >> 1);
+        const bool is_v = it & 1;
         int lp = t * 8 + (is_v ? pg_v : pg_k);
         if (lp > n_pages - 1) lp = n_pages - 1;  // pages past the sequence: any valid page (keys are masked)
         return (is_v ? p.v_table : p.k_table)[(size_t)req * p.max_pages + lp];
@@ -293,7 +269,7 @@ attn_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_constant__ CU
       int blk = (it < n_items && lane < n_boxes) ? table_entry(it) : 0;
       for (; it < n_items; it += 2) {
         const int blk_next = (it + 2 < n_items && lane < n_boxes) ? table_entry(it + 2) : 0;
-        const bool is_v = kWithPV && (it & 1);
+        const bool is_v = it & 1;
         const int s = it % kStages, u = it / kStages;
         mbar_wait_relaxed(&bars->kv_empty[s], (u & 1) ^ 1);   // the ring is several tiles deep: no hurry
         if (lane == 0 && rank == 0) mbar_expect_tx(&bars->kv_full[s], kTileBytes);  // both CTAs' bytes
@@ -317,7 +293,7 @@ attn_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_constant__ CU
       // descriptors are a base value plus small constants (the address field is (addr >> 4)).
       if (rank == 0 && elect_one()) {
         // PV variant: S = Q K^T is issued as two 64-key halves (N = 64), see issue_qk_half
-        constexpr uint32_t idesc_qk = umma_idesc_bf16(kPair ? 256 : 128, kWithPV ? 64 : 128, 0, 0);
+        constexpr uint32_t idesc_qk = umma_idesc_bf16(kPair ? 256 : 128, 64, 0, 0);
         constexpr uint32_t idesc_pv = umma_idesc_bf16(kPair ? 256 : 128, 128, 0, 1);
         constexpr uint32_t kSlotStep = kStageBytes >> 4;
         constexpr int kKHalf = kPair ? kHalfBytes / 2 : kHalfBytes;  // bytes between the two 64-column halves of K
@@ -334,20 +310,7 @@ attn_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_constant__ CU
           if (kPair) mbar_wait_cluster(bar, parity); else mbar_wait(bar, parity);
         };
         mbar_wait(&bars->q_full, 0);
-        // S_i[buffer b] = Q_i K(slot)^T
-        auto issue_qk = [&](int i, int b, int slot) {
-          const uint32_t qd = q_lo + (uint32_t)i * (kTileBytes >> 4), kd = k_lo + (uint32_t)slot * kSlotStep;
-          const uint32_t d = tmem + (kWithPV ? i * 128 : (i * 2 + b) * 128);
-#pragma unroll
-          for (int kk = 0; kk < 8; ++kk) {
-            const uint32_t oq = ((kk >> 2) * kHalfBytes + (kk & 3) * 32) >> 4;
-            const uint32_t ok = ((kk >> 2) * kKHalf + (kk & 3) * 32) >> 4;
-            if (kPair) umma_ss2_pair(d, qd + oq, qk_hi, kd + ok, qk_hi, idesc_qk, kk > 0);
-            else umma_ss2(d, qd + oq, qk_hi, kd + ok, qk_hi, idesc_qk, kk > 0);
-          }
-          commit(&bars->s_full[i][b]);
-        };
-        // PV variant: keys [64h, 64h + 64) of the tile in `slot` -> columns [64h, 64h + 64) of S_i, no commit
+        // keys [64h, 64h + 64) of the tile in `slot` -> columns [64h, 64h + 64) of S_i, no commit
         auto issue_qk_half = [&](int i, int slot, int h) {
           const uint32_t qd = q_lo + (uint32_t)i * (kTileBytes >> 4);
           const uint32_t kd = k_lo + (uint32_t)slot * kSlotStep + (uint32_t)h * kKSub;
@@ -360,7 +323,7 @@ attn_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_constant__ CU
             else umma_ss2(d, qd + oq, qk_hi, kd + ok, qk_hi, idesc_qk, kk > 0);
           }
         };
-        if (kWithPV) {
+        {
           // ring item 2t+1 = V(t), 2t+2 = K(t+1): (slot, phase) advanced incrementally
           int sv = 1, sk = 2, phv = 0, phk = 0;
           if (n_tiles > 0) {  // (a key split may hold no tile of this CTA's rows)
@@ -371,7 +334,7 @@ attn_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_constant__ CU
               if (n_t[i] > 0) {
                 issue_qk_half(i, 0, 0);
                 issue_qk_half(i, 0, 1);
-                commit(&bars->s_full[i][0]);
+                commit(&bars->s_full[i]);
               }
             }
             commit(&bars->kv_empty[0]);
@@ -414,7 +377,7 @@ attn_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_constant__ CU
                 if (t == n_t[i] - 1) commit(&bars->o_full[i]);
                 if (t + 1 < n_t[i]) {
                   issue_qk_half(i, sk, 0);
-                  commit(&bars->s_full[i][0]);
+                  commit(&bars->s_full[i]);
                 }
               }
             }
@@ -424,22 +387,6 @@ attn_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_constant__ CU
             if (sv >= kStages) { sv -= kStages; phv ^= 1; }
             sk += 2;
             if (sk >= kStages) { sk -= kStages; phk ^= 1; }
-          }
-        } else {
-          int slot = 0, ph = 0;
-          for (int t = 0; t < n_tiles; ++t) {
-            const int b = t & 1;
-            mbar_wait(&bars->kv_full[slot], ph);
-#pragma unroll
-            for (int i = 0; i < 2; ++i) {
-              if (t < n_t[i]) {
-                if (t >= 2) mbar_wait(&bars->s_free[i][b], ((t >> 1) + 1) & 1);
-                tc_fence_after();
-                issue_qk(i, b, slot);
-              }
-            }
-            commit(&bars->kv_empty[slot]);
-            if (++slot == kStages) { slot = 0; ph ^= 1; }
           }
         }
       }
@@ -455,7 +402,7 @@ attn_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_constant__ CU
     const int grow = row_base + qt * rpt + n_local;  // batch-wide row index
     const int pos = valid ? (p.rows ? p.rows[grow] : grow - p.rows_off[req]) : 0;
     const uint32_t lane_addr = (uint32_t)(quarter * 32) << 16;
-    const uint32_t tmem_s = tmem + lane_addr + (kWithPV ? qt * 128 : qt * 256);
+    const uint32_t tmem_s = tmem + lane_addr + qt * 128;
     const uint32_t tmem_o = tmem + lane_addr + 256 + qt * 128;
     const int my_tiles = qt ? n_t[1] : n_t[0];
     // kPair: P-ready arrivals go to rank 0's barriers (the issuer lives there)
@@ -467,17 +414,16 @@ attn_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_constant__ CU
                         // by l + l_fix, the log-sum-exp output stays that of the unrounded exponentials (l)
 
     for (int t = 0; t < my_tiles; ++t) {
-      const int b = kWithPV ? 0 : (t & 1);
-      mbar_wait(&bars->s_full[qt][b], kWithPV ? (t & 1) : ((t >> 1) & 1));
+      mbar_wait(&bars->s_full[qt], t & 1);
       tc_fence_after();
       // S row -> registers in two waves so that the maximum of the first 64 columns is formed while the
       // second 64 are still in flight
       uint32_t sr[4][32];
-      tmem_ld32(tmem_s + b * 128, sr[0]);
-      tmem_ld32(tmem_s + b * 128 + 32, sr[1]);
+      tmem_ld32(tmem_s, sr[0]);
+      tmem_ld32(tmem_s + 32, sr[1]);
       tmem_wait_ld();
-      tmem_ld32(tmem_s + b * 128 + 64, sr[2]);
-      tmem_ld32(tmem_s + b * 128 + 96, sr[3]);
+      tmem_ld32(tmem_s + 64, sr[2]);
+      tmem_ld32(tmem_s + 96, sr[3]);
 
       const int nvalid = pos - (t0 + t) * kTile + 1;  // keys [0, nvalid) of this tile are visible to this row
       // three independent 3-input max chains: tm[0], tm[1] over the columns whose exponential goes to MUFU, tm[2]
@@ -488,9 +434,7 @@ attn_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_constant__ CU
         if (c == 2) {
           tmem_wait_ld();
           tc_fence_before();
-          if (!kWithPV) {
-            mbar_arrive(&bars->s_free[qt][b]);
-          } else if (kPair) {  // S is in registers: columns [64, 128) may take the next tile's S
+          if (kPair) {  // S is in registers: columns [64, 128) may take the next tile's S
             __syncwarp();
             if (lane == 0) mbar_arrive_cluster(s_loaded_r0);
           } else {
@@ -524,7 +468,7 @@ attn_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_constant__ CU
         alpha = ex2_approx((m_used - m_new) * p.scale_log2);
         m_used = m_new;
       }
-      if (kWithPV && t > 0 && __any_sync(0xffffffffu, upd)) {
+      if (t > 0 && __any_sync(0xffffffffu, upd)) {
         // s_full(t) was committed after PV(t-1): O is quiescent until this thread arrives on p_half
 #pragma unroll
         for (int c = 0; c < 4; ++c) {
@@ -541,7 +485,7 @@ attn_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_constant__ CU
       const float2 sc2 = make_float2(p.scale_log2, p.scale_log2), nm2 = make_float2(neg_m, neg_m);
       float2 rsum2 = make_float2(0.f, 0.f);
 
-      if (kWithPV && (t0 + t + 1) * kTile > T) {
+      if ((t0 + t + 1) * kTile > T) {
         // V rows of keys beyond the sequence may hold anything (even NaN patterns): zero them
         // (kPair: this CTA's V half completes on rank 0's barrier; rank 0's issuer passes the news on. Only the
         // last tile of the sequence qualifies, so v_landed is used once.)
@@ -565,7 +509,7 @@ attn_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_constant__ CU
       // at once, so the first half of PV runs while the second half of the exponentials is computed
 #pragma unroll
       for (int h = 0; h < 2; ++h) {
-        uint32_t pk[kWithPV ? 32 : 1];
+        uint32_t pk[32];
 #pragma unroll
         for (int cc = 0; cc < 2; ++cc) {
           const int c = 2 * h + cc;
@@ -580,11 +524,11 @@ attn_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_constant__ CU
               e.y = ex2_approx(x.y);
             }
             rsum2 = __fadd2_rn(rsum2, e);
-            if (kWithPV) pk[cc * 16 + (i >> 1)] = pack_bf16x2(e.x, e.y);
+            pk[cc * 16 + (i >> 1)] = pack_bf16x2(e.x, e.y);
           }
         }
-        if (kWithPV) {
-          tmem_st32(tmem_s + h * 32, *reinterpret_cast<uint32_t(*)[32]>(&pk[0]));
+        {
+          tmem_st32(tmem_s + h * 32, pk);
           tmem_wait_st();
           tc_fence_before();
           if (kPair) {  // one arrival per warp: 8 (4 of them remote) instead of 256 per hand-off
@@ -596,7 +540,7 @@ attn_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_constant__ CU
         }
       }
       const float radd = rsum2.x + rsum2.y;
-      if (kWithPV) {
+      {
         // PV uses the bf16-ROUNDED probabilities while the row sum adds the unrounded ones. With a lazily updated
         // reference the largest P of a row is not 1, and for a peaked row its 2^-9 rounding would go straight
         // into O = sum(P v) / l. The largest term of every tile therefore enters the normaliser of O with its
@@ -616,7 +560,7 @@ attn_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_constant__ CU
 
     // ---- epilogue
     const size_t out_row = (size_t)grow * p.num_q_heads + kvh * g + hh;
-    if (kWithPV && p.kv_splits > 1) {
+    if (p.kv_splits > 1) {
       // key split: normalised partial O in fp32 and its log-sum-exp go to the workspace (attn_merge_kernel)
       const size_t prow = (size_t)split * p.total_rows * p.num_q_heads + out_row;
       float4 *dst = reinterpret_cast<float4 *>(p.part_o + prow * kHeadDim);
@@ -644,8 +588,8 @@ attn_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_constant__ CU
       __threadfence();
       named_bar_sync(2, 256);
       if (threadIdx.x == 0) {
-        split_arrive(p.tickets + bid, p.epoch);
-        split_wait_all(p.tickets + bid, p.epoch, p.kv_splits);
+        split_arrive(p.tickets + bid);
+        split_wait_all(p.tickets + bid, p.kv_splits);
         __threadfence();
       }
       named_bar_sync(2, 256);
@@ -656,8 +600,11 @@ attn_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_constant__ CU
         merge_splits(p.part_o, p.part_lse, p.kv_splits, stride, (size_t)(row_base + rl) * p.num_q_heads + kvh * g + hl,
                      lane, p.out, p.lse);
       }
-    } else if (my_tiles > 0 || !kWithPV) {  // (an LSE key split that holds no tile of the row still reports -inf)
-      if (kWithPV) {
+      // the partial buffers of this launch are not read after this point by this CTA
+      named_bar_sync(2, 256);
+      if (threadIdx.x == 0) split_depart(p.tickets + bid, p.kv_splits);
+    } else if (my_tiles > 0) {
+      {
         mbar_wait(&bars->o_full[qt], 0);
         tc_fence_after();
         const float inv = 1.f / (l + l_fix);
@@ -680,8 +627,7 @@ attn_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_constant__ CU
           }
         }
       }
-      if (p.lse && valid)
-        p.lse[(size_t)split * p.total_rows * p.num_q_heads + out_row] = m_used * p.scale + logf(l);
+      if (p.lse && valid) p.lse[out_row] = m_used * p.scale + logf(l);
     }
   }
 
@@ -704,10 +650,6 @@ constexpr int kAttnSplitCtas = 148;
 constexpr size_t kAttnPartFloats = (size_t)2 * kAttnSplitCtas * 256 * (kHeadDim + 1);
 size_t attn_part_bytes() { return kAttnPartFloats * sizeof(float) + kAttnSplitCtas * sizeof(unsigned long long); }
 unsigned long long *attn_tickets(float *part) { return reinterpret_cast<unsigned long long *>(part + kAttnPartFloats); }
-unsigned long long next_split_epoch() {
-  static std::atomic<unsigned long long> epoch{0};
-  return (epoch.fetch_add(1, std::memory_order_relaxed) + 1) & ((1ull << 56) - 1);
-}
 
 int attn_pv_splits(const sx_pool *pool, const sx_batch *b, int32_t total_rows) {
   const int g = pool->num_q_heads / pool->num_kv_heads;
@@ -725,16 +667,7 @@ int attn_pv_splits(const sx_pool *pool, const sx_batch *b, int32_t total_rows) {
   return s < 1 ? 1 : s;
 }
 
-// Key splits of the LSE-only sweep: enough CTAs for about four waves (a long single request gives few row
-// pairs: C5 has 57 x 4 KV heads), at most 8. The partial normalisers are merged by coltab_kernel.
-int attn_lse_splits(const sx_pool *pool, const sx_batch *b, int32_t total_rows) {
-  const int g = pool->num_q_heads / pool->num_kv_heads;
-  const int grid = (total_rows / (2 * (kTile / g)) + b->num_reqs) * pool->num_kv_heads;
-  int s = (4 * 148 + grid - 1) / grid;
-  return s < 1 ? 1 : (s > 8 ? 8 : s);
-}
-
-sx_status launch_attn(const sx_pool *pool, const sx_batch *b, bool with_pv, const void *q, const int32_t *rows,
+sx_status launch_attn(const sx_pool *pool, const sx_batch *b, const void *q, const int32_t *rows,
                       const int32_t *rows_off, int32_t total_rows, void *out, float *lse, int kv_splits,
                       float *part, bool cta_pair, cudaStream_t st) {
   const int g = pool->num_q_heads / pool->num_kv_heads;
@@ -765,35 +698,26 @@ sx_status launch_attn(const sx_pool *pool, const sx_batch *b, bool with_pv, cons
   p.part_o = part;
   p.part_lse = part ? part + (size_t)p.kv_splits * total_rows * pool->num_q_heads * kHeadDim : nullptr;
   p.tickets = part ? attn_tickets(part) : nullptr;
-  p.epoch = part ? next_split_epoch() : 0;
   p.scale = (float)(1.0 / sqrt((double)kHeadDim));
   p.scale_log2 = (float)(kLog2e / sqrt((double)kHeadDim));
   const int grid = (total_rows / (2 * rpt) + b->num_reqs) * pool->num_kv_heads;  // >= sum_r ceil(n_r / 2rpt) * Hkv
   cudaError_t e;
-  if (with_pv && p.kv_splits == 1 && cta_pair) {
+  if (p.kv_splits == 1 && cta_pair) {
     // CTA pairs: clusters of two CTAs over adjacent row pairs; sum_r ceil(pairs_r / 2) clusters per KV head
-    e = cudaFuncSetAttribute(attn_kernel<true, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, AttnCfg::kSmemBytes);
+    e = cudaFuncSetAttribute(attn_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, AttnCfg::kSmemBytes);
     if (e != cudaSuccess) return set_error(SX_ERR_CUDA, "attn smem attr: %s", cudaGetErrorString(e));
     const int clusters = (total_rows / (4 * rpt) + b->num_reqs) * pool->num_kv_heads;
-    e = launch_pdl(attn_kernel<true, true>, dim3(2 * clusters), dim3(kAttnThreads), AttnCfg::kSmemBytes, st, 2, tm_q,
+    e = launch_pdl(attn_kernel<true>, dim3(2 * clusters), dim3(kAttnThreads), AttnCfg::kSmemBytes, st, 2, tm_q,
                    tm_k, tm_v, p);
     if (e != cudaSuccess) return set_error(SX_ERR_CUDA, "attn pair launch: %s", cudaGetErrorString(e));
-    return check_launch("attn_kernel<pv,pair>");
+    return check_launch("attn_kernel<pair>");
   }
-  if (with_pv) {
-    e = cudaFuncSetAttribute(attn_kernel<true, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, AttnCfg::kSmemBytes);
-    if (e != cudaSuccess) return set_error(SX_ERR_CUDA, "attn smem attr: %s", cudaGetErrorString(e));
-    e = launch_pdl(attn_kernel<true, false>, dim3(grid * p.kv_splits), dim3(kAttnThreads), AttnCfg::kSmemBytes, st, 1,
-                   tm_q, tm_k, tm_v, p);
-  } else {
-    e = cudaFuncSetAttribute(attn_kernel<false, false>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                             AttnCfg::kSmemBytes);
-    if (e != cudaSuccess) return set_error(SX_ERR_CUDA, "lse smem attr: %s", cudaGetErrorString(e));
-    e = launch_pdl(attn_kernel<false, false>, dim3(grid * p.kv_splits), dim3(kAttnThreads), AttnCfg::kSmemBytes, st, 1,
-                   tm_q, tm_k, tm_v, p);
-  }
+  e = cudaFuncSetAttribute(attn_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, AttnCfg::kSmemBytes);
+  if (e != cudaSuccess) return set_error(SX_ERR_CUDA, "attn smem attr: %s", cudaGetErrorString(e));
+  e = launch_pdl(attn_kernel<false>, dim3(grid * p.kv_splits), dim3(kAttnThreads), AttnCfg::kSmemBytes, st, 1,
+                 tm_q, tm_k, tm_v, p);
   if (e != cudaSuccess) return set_error(SX_ERR_CUDA, "attn launch: %s", cudaGetErrorString(e));
-  return check_launch(with_pv ? "attn_kernel<pv>" : "attn_kernel<lse>");
+  return check_launch("attn_kernel");
 }
 
 }  // namespace sx

@@ -93,24 +93,6 @@ coltab_kernel(const ColsumParams p) {
   row[128 + ct] = __int_as_float(qpos);
 }
 
-// exp2 of two values on the FMA pipe: x = n + f, n = rint(x), |f| <= 1/2; cubic for 2^f (relative error
-// 7.5e-5, far inside the 5e-3 score tolerance), 2^n by exponent arithmetic. x <= ~0 here; clamp at -126.
-__device__ __forceinline__ float2 cs_ex2_poly2(float2 x) {
-  const float kMagic = 12582912.f;  // 1.5 * 2^23
-  x.x = fmaxf(x.x, -126.f);
-  x.y = fmaxf(x.y, -126.f);
-  const float2 t = __fadd2_rn(x, make_float2(kMagic, kMagic));
-  const float2 n = __fadd2_rn(t, make_float2(-kMagic, -kMagic));
-  const float2 f = __ffma2_rn(n, make_float2(-1.f, -1.f), x);
-  float2 p = __ffma2_rn(make_float2(0.0551716648f, 0.0551716648f), f, make_float2(0.2426111251f, 0.2426111251f));
-  p = __ffma2_rn(p, f, make_float2(0.6932609677f, 0.6932609677f));
-  p = __ffma2_rn(p, f, make_float2(0.9999280572f, 0.9999280572f));
-  float2 r;
-  r.x = __int_as_float(__float_as_int(p.x) + (__float_as_int(t.x) << 23));
-  r.y = __int_as_float(__float_as_int(p.y) + (__float_as_int(t.y) << 23));
-  return r;
-}
-
 // One consumer thread, one D tile: sum of exp2(s * c - lse_col) over its 64 columns (d[2][32] = raw scores of its key
 // against the 64 (query, head) columns; `col` = shared-memory address of their normalisers, positions 512 B further).
 template <bool kMask>
@@ -130,7 +112,7 @@ __device__ __forceinline__ float2 cs_consume(const uint32_t (&d)[2][32], uint32_
                               make_float2(-la, -lb));
         float2 e;
         if ((ii & 15) < 2 * SX_COLSUM_POLY) {
-          e = cs_ex2_poly2(x);
+          e = ex2_poly2(x);
         } else {
           e.x = ex2_approx(x.x);
           e.y = ex2_approx(x.y);

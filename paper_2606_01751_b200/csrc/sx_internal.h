@@ -45,14 +45,16 @@ sx_status launch_select(const sx_pool *pool, const sx_batch *b, const float *par
                         cudaStream_t st);
 size_t select_scratch_bytes(const sx_batch *b);
 // tcgen05 kernels. q_rows: bf16 [total_rows][Hq][128]; rows == nullptr => row n is position n - off[req].
-sx_status launch_attn(const sx_pool *pool, const sx_batch *b, bool with_pv, const void *q, const int32_t *rows,
+sx_status launch_attn(const sx_pool *pool, const sx_batch *b, const void *q, const int32_t *rows,
                       const int32_t *rows_off, int32_t total_rows, void *out, float *lse, int kv_splits,
                       float *part, bool cta_pair, cudaStream_t st);
 int attn_pv_splits(const sx_pool *pool, const sx_batch *b, int32_t total_rows);
 size_t attn_part_bytes();
-unsigned long long *attn_tickets(float *part);  // arrival words of the key splits, behind the partial buffer
-unsigned long long next_split_epoch();          // unique per split launch in this process (sx_split_merge.cuh)
-int attn_lse_splits(const sx_pool *pool, const sx_batch *b, int32_t total_rows);
+unsigned long long *attn_tickets(float *part);  // rendezvous words of the key splits, behind the partial buffer
+// first sweep of stage (b) (sx_lse.cu): partial log-sum-exps [kv_splits][total_new][Hq] of the Sparse-Q rows
+int lse_splits(const sx_pool *pool, const sx_batch *b);
+sx_status launch_lse(const sx_pool *pool, const sx_batch *b, const void *q_new, float *lse_ws, int kv_splits,
+                     cudaStream_t st);
 // CUDA-core split-KV attention for fewer than 64 (row, head) pairs per KV head; part = ws.small_part
 sx_status launch_attn_small(const sx_pool *pool, const sx_batch *b, const void *q, const int32_t *rows,
                             const int32_t *rows_off, int32_t total_rows, void *out, float *lse, float *part,

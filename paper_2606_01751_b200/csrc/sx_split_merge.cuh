@@ -8,35 +8,42 @@
 
 namespace sx {
 
-// Arrival of a key split on a workspace word that is never zeroed: the word holds (epoch << 8 | arrivals); a word
-// whose epoch is not this launch's counts as zero arrivals. Once all kv_splits splits of a (request, KV head, row
-// chunk) have arrived, EVERY one of them merges a share of the (row, head) pairs -- each pair in the fixed order
-// 0 .. kv_splits-1, so who merges what does not change the result. The splits of a launch are sized for one wave
+// Rendezvous of the key splits of one (request, KV head, row pair) on a workspace word that the host never
+// zeroes. The word holds (kSplitTag << 8 | count); anything else is memory that no launch has used yet and counts
+// as zero. Every split ARRIVES once its partial result is written (count 1 .. splits), waits until all have
+// arrived, merges its share of the (row, head) pairs -- each pair in the fixed order 0 .. splits-1, so who merges
+// what does not change the result -- and DEPARTS (count splits+1 .. 2 splits); the last one to depart puts the
+// word back to count 0. The protocol therefore depends on nothing but the word itself: it is safe under CUDA-graph
+// replay (same kernel parameters every time) and needs no memset. The splits of a launch are sized for one wave
 // (at most one CTA per SM), so the CTAs that wait here are all resident.
-// Fast path: one atomicAdd. Only an arriver that still finds another launch's epoch in the word installs this one
-// by compare-and-swap (its add, and any other add on the stale word, is overwritten by the install and repeated
-// through the loop; an add that lands after the install already carries the right epoch and counts).
-__device__ __forceinline__ void split_arrive(unsigned long long *w, unsigned long long epoch) {
-  unsigned long long old = atomicAdd(w, 1ull);
-  if ((old >> 8) == epoch) return;
+constexpr unsigned long long kSplitTag = 0x53784d65726765ull;  // 56 bits
+
+__device__ __forceinline__ void split_arrive(unsigned long long *w) {
+  unsigned long long old = atomicAdd(w, 1ull);  // fast path: one atomic
+  if ((old >> 8) == kSplitTag) return;
+  // first use of this memory: install the tag. The add above (and any other add on the untagged word) is overwritten
+  // by the install and repeated through this loop; an add that lands after the install already counts.
   unsigned long long cur = old + 1ull;
   for (;;) {
-    const unsigned long long cnt = ((cur >> 8) == epoch) ? (cur & 255ull) : 0ull;
-    const unsigned long long prev = atomicCAS(w, cur, (epoch << 8) | (cnt + 1ull));
+    const unsigned long long cnt = ((cur >> 8) == kSplitTag) ? (cur & 255ull) : 0ull;
+    const unsigned long long prev = atomicCAS(w, cur, (kSplitTag << 8) | (cnt + 1ull));
     if (prev == cur) return;
     cur = prev;
   }
 }
-__device__ __forceinline__ void split_wait_all(const unsigned long long *w, unsigned long long epoch, int splits) {
-  const unsigned long long want = (epoch << 8) | (unsigned long long)splits;
+__device__ __forceinline__ void split_wait_all(const unsigned long long *w, int splits) {
   uint32_t polls = 0;
   for (;;) {
     unsigned long long v;
     asm volatile("ld.acquire.gpu.global.u64 %0, [%1];" : "=l"(v) : "l"(w) : "memory");
-    if (v == want) return;
+    if ((v >> 8) == kSplitTag && (int)(v & 255ull) >= splits) return;
     __nanosleep(20);
     if (++polls > (1u << 24)) __trap();  // a protocol bug traps instead of hanging the GPU
   }
+}
+__device__ __forceinline__ void split_depart(unsigned long long *w, int splits) {
+  const unsigned long long old = atomicAdd(w, 1ull);
+  if ((int)(old & 255ull) == 2 * splits - 1) atomicExch(w, kSplitTag << 8);  // everyone has left: count 0 again
 }
 
 // Combine the key splits of one (row, head) pair: out = sum_s exp(lse_s - lse) O_s in the fixed order 0..splits-1.

@@ -590,3 +590,34 @@ def test_reference_moves_and_rescales_with_key_splits(nrows):
     ref_o, ref_l = orc.attention(pk, pv, kt[0], vt[0], t, lt.q_full[rows], rows, lay.num_q_heads, want_lse=True)
     check_close("key splits, growing key norms", orc.bf16_to_f64(dev_to_bits(g.out)), ref_o)
     assert np.max(np.abs(g.lse.cpu().numpy().astype(np.float64) - ref_l)) < 2e-3
+
+
+def test_key_split_path_under_cuda_graph_replay():
+    """The self-merging key splits meet on a workspace word that no memset prepares; the rendezvous must come back to
+    its initial state by itself, so that a captured launch (identical kernel parameters on every replay) works any
+    number of times and keeps giving the bits of the eager call."""
+    GpuLayer, dev_to_bits = _gpu()
+    from paper_2606_01751_b200 import binding as sx
+    lay, lt, res, pk, pv, kt, vt = prepared("C1")
+    g = GpuLayer(lay, lt)
+    g.step_sparse()
+    t = int(lay.seq_len[0])
+    rows = torch.arange(t - 6, t, dtype=torch.int32, device=g.dev)
+    off = torch.tensor([0, 6], dtype=torch.int32, device=g.dev)
+    q = g.q_full[t - 6:t].contiguous()
+    out = torch.zeros((6, lay.num_q_heads, 128), dtype=torch.int16, device=g.dev)
+    sx.sparse_attn(g.pool, g.batch, q, out, rows_R=rows, rows_off=off, total_rows=6)
+    torch.cuda.synchronize()
+    eager = out.clone()
+    gr = torch.cuda.CUDAGraph()
+    with torch.cuda.graph(gr):
+        sx.sparse_attn(g.pool, g.batch, q, out, rows_R=rows, rows_off=off, total_rows=6)
+    for _ in range(4):
+        out.zero_()
+        gr.replay()
+        torch.cuda.synchronize()
+        assert torch.equal(out, eager)
+    out.zero_()
+    sx.sparse_attn(g.pool, g.batch, q, out, rows_R=rows, rows_off=off, total_rows=6)   # and eager again afterwards
+    torch.cuda.synchronize()
+    assert torch.equal(out, eager)
