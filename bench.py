@@ -282,8 +282,13 @@ def measure(cfg, steps, warmup, ctx, want_e2e=True, want_clocks=True):
     for _ in range(max(warmup, 3)):
         step()
     barrier()
+    # ---- timed region: K steps. C3 stack: CUDA events around every stage call inside the timed region (the
+    # roofline's kernel time; 66 event pairs in a 60 ms step cost nothing). Single-layer configs: no per-stage
+    # instrumentation in the timed region (two event records per stage call are a third of a launch-bound
+    # 0.1 ms step); their per-stage view comes from a second pass of the same steps.
+    two_pass = not stack
+    ev["on"] = not two_pass
     launches0 = sx.launch_count()
-    ev["on"] = True
     sampler = ClockSampler(local)
     if rank == 0 and want_clocks:
         sampler.start()
@@ -299,8 +304,17 @@ def measure(cfg, steps, warmup, ctx, want_e2e=True, want_clocks=True):
         barrier()
         step_ms.append(a.elapsed_time(b))
     clocks = sampler.stop() if (rank == 0 and want_clocks) else None
-    ev["on"] = False
     launches = sx.launch_count() - launches0     # kernels launched in the timed region, counted inside libsparsex.so
+    ev["on"] = False
+    if two_pass:   # second pass, same steps, with CUDA events around every stage call: the per-stage view
+        ev["on"] = True
+        for _ in range(steps):
+            if flush is not None:
+                flush.zero_()
+            barrier()
+            step()
+            barrier()
+        ev["on"] = False
     t_ms = du.max_over_ranks(float(np.sum(step_ms)), dev)
     ms_per_step = t_ms / steps
     stage_ms = {k: float(sum(x.elapsed_time(y) for x, y in v)) / steps for k, v in ev.items() if k != "on"}

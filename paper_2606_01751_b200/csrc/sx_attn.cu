@@ -60,6 +60,7 @@ struct AttnParams {
   float *lse;          // [total_rows][Hq] or nullptr
   int num_reqs, max_pages, num_q_heads, num_kv_heads, group, rows_per_tile;
   int total_rows;
+  int head_group;    // KV heads whose blocks are interleaved in the launch order (see the kernel)
   int kv_splits;     // the key range of a CTA is cut into this many contiguous parts (consecutive blocks)
   float *part_o;     // PV variant with kv_splits > 1: [split][total_rows][Hq][128] normalised partial O (fp32)
   float *part_lse;   //                                 [split][total_rows][Hq]      partial log-sum-exp
@@ -170,11 +171,18 @@ attn_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_constant__ CU
   const bool active = req < p.num_reqs;  // (the grid is an upper bound; both CTAs of a cluster agree)
   if (!active) req = 0;
   const int local = active ? bid - base : 0;
-  const int kvh = local % p.num_kv_heads;
+  // Order of the blocks of a request: KV heads in groups of p.head_group; inside a group heavy (late) row pairs
+  // first, the heads of the group interleaved. Blocks that run at the same time then share the K/V of head_group
+  // heads only (head_group * 2 * T * 256 B, L2-resident when the request has many row pairs per head), and a
+  // group is never so small that its heaviest block could start late enough to stretch the tail (launch_attn).
+  const int per_group = max(units, 1) * p.head_group;
+  const int grp = local / per_group, idx = local - grp * per_group;
+  const int gsz = min(p.head_group, p.num_kv_heads - grp * p.head_group);
+  const int kvh = grp * p.head_group + idx % gsz, unit = idx / gsz;
   // kPair: rank 0 takes the later pair; with an odd number of pairs the last cluster's rank 1 has no rows
   // (pair = -1) and only stages its halves of K/V and runs masked softmax tiles
   const int pair = !active ? -1
-                           : (kPair ? pairs - 1 - (2 * (local / p.num_kv_heads) + rank) : pairs - 1 - local / p.num_kv_heads);
+                           : (kPair ? pairs - 1 - (2 * unit + rank) : pairs - 1 - unit);
   const int row_base = pair >= 0 ? p.rows_off[req] + pair * rpc : p.total_rows;  // first row of query tile 0
   const int T = p.seq_len[req];
   const int n_pages = (T + kPage - 1) / kPage;
@@ -265,6 +273,9 @@ attn_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_constant__ CU
         return (is_v ? p.v_table : p.k_table)[(size_t)req * p.max_pages + lp];
       };
       const uint32_t full0 = kPair ? mapa_u32(smem_u32(&bars->kv_full[0]), 0) : 0;
+#ifdef SX_KV_EVICT_LAST
+      const uint64_t kv_pol = l2_policy_evict_last();
+#endif
       int it = (warp == kWarpProd1) ? 1 : 0;
       int blk = (it < n_items && lane < n_boxes) ? table_entry(it) : 0;
       for (; it < n_items; it += 2) {
@@ -279,10 +290,19 @@ attn_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_constant__ CU
           if (kPair) {
             uint8_t *dst = smem + Cfg::kOffKV + s * kStageBytes +
                            (is_v ? pg_v * 2048 : half_k * (kHalfBytes / 2) + (lane >> 1) * 2048);
+#ifdef SX_KV_EVICT_LAST
+            tma_load_2d_pair_hint(dst, is_v ? &tm_v : &tm_k, full0 + s * 8, (is_v ? half_v : half_k) * 64, row0, kv_pol);
+#else
             tma_load_2d_pair(dst, is_v ? &tm_v : &tm_k, full0 + s * 8, (is_v ? half_v : half_k) * 64, row0);
+#endif
           } else {
+#ifdef SX_KV_EVICT_LAST
+            tma_load_2d_hint(smem + Cfg::kOffKV + s * kTileBytes + half_k * kHalfBytes + pg_k * 2048,
+                             is_v ? &tm_v : &tm_k, &bars->kv_full[s], half_k * 64, row0, kv_pol);
+#else
             tma_load_2d(smem + Cfg::kOffKV + s * kTileBytes + half_k * kHalfBytes + pg_k * 2048,
                         is_v ? &tm_v : &tm_k, &bars->kv_full[s], half_k * 64, row0);
+#endif
           }
         }
         blk = blk_next;
@@ -701,6 +721,21 @@ sx_status launch_attn(const sx_pool *pool, const sx_batch *b, const void *q, con
   p.scale = (float)(1.0 / sqrt((double)kHeadDim));
   p.scale_log2 = (float)(kLog2e / sqrt((double)kHeadDim));
   const int grid = (total_rows / (2 * rpt) + b->num_reqs) * pool->num_kv_heads;  // >= sum_r ceil(n_r / 2rpt) * Hkv
+  {
+    // KV heads per group of the launch order. A group's heaviest block may only start once the earlier groups are
+    // done; if a group is small compared with the number of workers that late heavy block stretches the tail, so
+    // heads are grouped only when every head alone fills the machine several times over (U >= 2 * workers blocks
+    // per head: G = ceil(2 * workers / U) heads per group), else all heads are interleaved as before.
+    // Measured on C3 (S10): full layers (U = 256 clusters per head, G = 1): DRAM reads 1.9 -> 0.4 GB per
+    // launch and +4..10 % speed; sparse layers (U = 44): groups of 4 heads lost 9 %, so they keep G = Hkv.
+    const int workers = cta_pair ? 74 : 148;
+    const int per_req = total_rows / (b->num_reqs > 0 ? b->num_reqs : 1);
+    int units = per_req / ((cta_pair ? 4 : 2) * rpt);
+    if (units < 1) units = 1;
+    int gsz = (2 * workers + units - 1) / units;
+    if (units < 2 * workers || gsz > pool->num_kv_heads) gsz = pool->num_kv_heads;
+    p.head_group = gsz;
+  }
   cudaError_t e;
   if (p.kv_splits == 1 && cta_pair) {
     // CTA pairs: clusters of two CTAs over adjacent row pairs; sum_r ceil(pairs_r / 2) clusters per KV head
