@@ -103,7 +103,27 @@ typedef struct {
   /* RoPE: theta_i = rope_theta^(-2i/head_dim); rotation by angle delta*theta_i */
   double rope_theta;         /* host */
   int32_t rope_style;        /* host: 0 = pairs (i, i+head_dim/2) ("half-split"), 1 = pairs (2i, 2i+1) */
+  int32_t zero_copy;         /* host: 0 = reused K is re-aligned into private pages by sx_rope_realign;
+                                1 = zero-copy mode, see below                                            */
 } sx_batch;
+
+/* Zero-copy mode (batch->zero_copy = 1; the paper's remark that position-independent blocks can be SHARED between
+ * requests, taken to its end for K as well as V). Nothing is re-aligned up front: the caller
+ * points the k_block_table (and v_block_table) entries of reused pages straight at the cached source pages, whose
+ * keys are stored rotated for their OLD positions, and the stage kernels apply R_{delta_m} while they read:
+ *   - a logical page lp of request r that a segment m covers and whose k_block_table entry equals m's source page
+ *     for lp is read ROTATED by delta_m (same arithmetic, same bits as sx_rope_realign would have stored);
+ *     every other page (fresh, prefix hit, or already made private) is read as stored;
+ *   - sx_score_select[_ex] and sx_sparse_attn rotate each K tile in shared memory between its TMA load and the MMA
+ *     (attention then works on ONE query tile per CTA, the second softmax warpgroup becomes the rotator; CTA pairs
+ *     and the CUDA-core kernels are not available: SX_ERR_UNSUPPORTED);
+ *   - sx_scatter_kv needs batch->cow_private: the first row written to a still-shared page copies it to its private
+ *     page -- K rotated on the way, V bit-copied -- and flips the table entries; later calls see a private page;
+ *   - sx_rope_realign[_layers] refuses the descriptor (SX_ERR_INVALID_ARG): its destination would be the shared
+ *     source pages.
+ * Memory: a request holds private pages only for the positions it recomputes (|R| / 16 pages, worst case one page
+ * per recomputed token) instead of all of its reused pages. Cost: every sweep over K pays the rotation again
+ * (measured in DESIGN.md S9). The tables belong to ONE layer, as under copy-on-write. */
 
 /* Bytes of caller-provided workspace that any stage call on (pool, batch) may need. Host only. */
 sx_status sx_workspace_size(const sx_pool *pool, const sx_batch *batch, size_t *bytes);
@@ -117,6 +137,7 @@ sx_status sx_workspace_size(const sx_pool *pool, const sx_batch *batch, size_t *
  * only read. Uses ws. */
 sx_status sx_rope_realign(const sx_pool *pool, const sx_batch *batch, void *ws, size_t ws_bytes,
                           sx_stream stream);
+/* (both realign calls return SX_ERR_INVALID_ARG for a batch in zero-copy mode) */
 
 /* (a) for a stack of layers in ONE launch: pools[0..num_layers) are the per-layer pools (host array; same
  * num_blocks / num_kv_heads), all addressed through the same batch descriptor (block tables and segment map

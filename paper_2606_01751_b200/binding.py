@@ -43,7 +43,7 @@ class SxBatch(ctypes.Structure):
                 ("k_block_table", ctypes.c_void_p), ("v_block_table", ctypes.c_void_p),
                 ("cow_private", ctypes.c_void_p), ("segments", ctypes.c_void_p),
                 ("src_blocks", ctypes.c_void_p), ("new_off", ctypes.c_void_p), ("new_idx", ctypes.c_void_p),
-                ("rope_theta", ctypes.c_double), ("rope_style", ctypes.c_int32)]
+                ("rope_theta", ctypes.c_double), ("rope_style", ctypes.c_int32), ("zero_copy", ctypes.c_int32)]
 
 
 class SparseXError(RuntimeError):
@@ -152,7 +152,7 @@ class DeviceBatch:
             self.v_block_table.data_ptr(), self.cow_private.data_ptr() if use_cow else None,
             self.segments.data_ptr() if nseg else None, self.src_blocks.data_ptr() if nseg else None,
             self.new_off.data_ptr(), self.new_idx.data_ptr() if int(lay.new_off[-1]) else None,
-            float(lay.rope_theta), int(lay.rope_style))
+            float(lay.rope_theta), int(lay.rope_style), int(bool(getattr(lay, "zero_copy", False))))
         self._ws = None
         self._ws_pool_key = None
 

@@ -57,6 +57,8 @@ WsLayout ws_layout(const sx_pool *pool, const sx_batch *b) {
   off = align_up(off + select_scratch_bytes(b), 256);
   w.small_part = off;
   off = align_up(off + small_ws_bytes(b->num_reqs, pool->num_kv_heads, pool->num_q_heads / pool->num_kv_heads), 256);
+  w.page_seg = off;
+  off = align_up(off + sizeof(int32_t) * (size_t)b->num_reqs * b->max_pages_per_req, 256);
   w.total = off;
   return w;
 }
@@ -87,8 +89,22 @@ static sx_status validate(const sx_pool *pool, const sx_batch *b) {
   if (b->rope_style != 0 && b->rope_style != 1)
     return set_error(SX_ERR_UNSUPPORTED, "rope_style must be 0 (half-split) or 1 (interleaved)");
   if (!(b->rope_theta > 1.0)) return set_error(SX_ERR_INVALID_ARG, "rope_theta must be > 1");
+  if (b->zero_copy != 0 && b->zero_copy != 1) return set_error(SX_ERR_INVALID_ARG, "zero_copy must be 0 or 1");
   if (misaligned(pool->k) || misaligned(pool->v)) return set_error(SX_ERR_MISALIGNED, "pool.k / pool.v not 16-B aligned");
   return SX_OK;
+}
+
+// zero-copy mode: build the rotation table and the page classification in the workspace (one small launch)
+static sx_status zc_prepare(const sx_pool *pool, const sx_batch *b, void *ws, cudaStream_t s, ZcArgs *zc) {
+  *zc = ZcArgs();
+  if (!b->zero_copy || b->num_segments == 0) return SX_OK;
+  const WsLayout w = ws_layout(pool, b);
+  float2 *table = reinterpret_cast<float2 *>(static_cast<char *>(ws) + w.rope_table);
+  int32_t *page_seg = reinterpret_cast<int32_t *>(static_cast<char *>(ws) + w.page_seg);
+  zc->style = b->rope_style;
+  zc->table = table;
+  zc->page_seg = page_seg;
+  return launch_zc_prepare(b, table, page_seg, s);
 }
 
 static sx_status validate_ws(const sx_pool *pool, const sx_batch *b, const void *ws, size_t ws_bytes) {
@@ -204,7 +220,7 @@ extern "C" {
 
 const char *sx_last_error(void) { return g_err; }
 
-const char *sx_version(void) { return "sparsex-b200 0.2 (sm_100a; tcgen05/TMEM/TMA)"; }
+const char *sx_version(void) { return "sparsex-b200 0.3 (sm_100a; tcgen05/TMEM/TMA)"; }
 
 uint64_t sx_launch_count(void) { return g_launches.load(std::memory_order_relaxed); }
 
@@ -245,6 +261,8 @@ sx_status sx_rope_realign_layers(const sx_pool *pools, int32_t num_layers, const
   if (batch && batch->cow_private && num_layers > 1)
     return set_error(SX_ERR_UNSUPPORTED,
                      "copy-on-write tables are per layer: call sx_rope_realign with one sx_batch per layer");
+  if (batch && batch->zero_copy)
+    return set_error(SX_ERR_INVALID_ARG, "zero-copy mode: nothing to re-align (K is rotated as it is read)");
   for (int l = 0; l < num_layers; ++l) {
     sx_status st = validate(&pools[l], batch);
     if (st != SX_OK) return st;
@@ -272,6 +290,8 @@ sx_status sx_scatter_kv(const sx_pool *pool, const sx_batch *batch, const void *
   if (max_rows == 0) return SX_OK;
   if (!k_fresh || !v_fresh || !rows || !rows_off) return set_error(SX_ERR_INVALID_ARG, "scatter: NULL array");
   if (misaligned(k_fresh) || misaligned(v_fresh)) return set_error(SX_ERR_MISALIGNED, "k_fresh / v_fresh not 16-B aligned");
+  if (batch->zero_copy && !batch->cow_private)
+    return set_error(SX_ERR_INVALID_ARG, "zero-copy mode: scatter needs cow_private (shared source pages are never written)");
   return launch_scatter(pool, batch, k_fresh, v_fresh, rows, rows_off, max_rows, reinterpret_cast<cudaStream_t>(stream));
 }
 
@@ -297,18 +317,21 @@ sx_status sx_score_select_ex(const sx_pool *pool, const sx_batch *batch, const v
   const float *lse = lse_new;
   if (lse_by_token != 0 && lse_by_token != 1) return set_error(SX_ERR_INVALID_ARG, "lse_by_token must be 0 or 1");
   int lse_splits = 1;
+  ZcArgs zc;
   if (batch->total_new > 0) {
+    st = zc_prepare(pool, batch, ws, s, &zc);
+    if (st != SX_OK) return st;
     if (!lse) {  // sweep 1: row normaliser of Eq. (1) for the Sparse-Q rows
       float *lse_ws = reinterpret_cast<float *>(base + w.lse_new);
       lse_splits = sx::lse_splits(pool, batch);
-      st = launch_lse(pool, batch, q_new, lse_ws, lse_splits, s);
+      st = launch_lse(pool, batch, q_new, lse_ws, lse_splits, zc, s);
       if (st != SX_OK) return st;
       lse = lse_ws;
       lse_by_token = 0;
     }
     // sweep 2: column sums of A_sq (Eq. 2), one partial vector per KV head
     st = launch_colsum(pool, batch, q_new, lse, lse_by_token, lse_splits, partial,
-                       reinterpret_cast<float2 *>(base + w.col_tab), s);
+                       reinterpret_cast<float2 *>(base + w.col_tab), zc, s);
     if (st != SX_OK) return st;
   } else {
     cudaError_t e = cudaMemsetAsync(partial, 0, sizeof(float) * (size_t)pool->num_kv_heads * batch->total_tokens, s);
@@ -338,6 +361,7 @@ sx_status sx_sparse_attn(const sx_pool *pool, const sx_batch *batch, int32_t mod
   // 2-CTA clusters: forced by a flag, else for batches of one request (measured: +1-2 % there, -5 % on batches)
   const bool want_cta_pair =
       (mode & SX_ATTN_CTA_PAIR) != 0 || ((mode & SX_ATTN_SINGLE_CTA) == 0 && batch->num_reqs == 1);
+  const int mode_flags = mode;
   mode &= 1;
   if (total_rows < 0) return set_error(SX_ERR_INVALID_ARG, "total_rows < 0");
   if (total_rows == 0) return SX_OK;
@@ -359,6 +383,19 @@ sx_status sx_sparse_attn(const sx_pool *pool, const sx_batch *batch, int32_t mod
   // selects the CUDA-core kernels by the north_star rule (fewer than 64 pairs per KV head on average over the batch).
   const int g = pool->num_q_heads / pool->num_kv_heads;
   const bool allow_small = want_cuda_core;
+  if (batch->zero_copy && batch->num_segments > 0) {
+    // K tiles are rotated in shared memory by the second softmax warpgroup: one query tile per CTA, no CTA pairs
+    if (want_cuda_core || (mode_flags & SX_ATTN_CTA_PAIR))
+      return set_error(SX_ERR_UNSUPPORTED, "zero-copy mode: CUDA-core kernels / CTA pairs are not available");
+    st = validate_ws(pool, batch, ws, ws_bytes);
+    if (st != SX_OK) return st;
+    ZcArgs zc;
+    st = zc_prepare(pool, batch, ws, s, &zc);
+    if (st != SX_OK) return st;
+    const int splits = attn_pv_splits(pool, batch, total_rows, 1);
+    float *part = splits > 1 ? reinterpret_cast<float *>(static_cast<char *>(ws) + ws_layout(pool, batch).attn_part) : nullptr;
+    return launch_attn(pool, batch, q, rows_R, rows_off, total_rows, out, lse, splits, part, false, zc, s);
+  }
   if (allow_small && g <= 32 && (int64_t)total_rows * g < (int64_t)64 * batch->num_reqs) {
     st = validate_ws(pool, batch, ws, ws_bytes);
     if (st != SX_OK) return st;
@@ -366,14 +403,14 @@ sx_status sx_sparse_attn(const sx_pool *pool, const sx_batch *batch, int32_t mod
     return launch_attn_small(pool, batch, q, rows_R, rows_off, total_rows, out, lse,
                              reinterpret_cast<float *>(static_cast<char *>(ws) + w.small_part), s);
   }
-  const int splits = attn_pv_splits(pool, batch, total_rows);
+  const int splits = attn_pv_splits(pool, batch, total_rows, 2);
   float *part = nullptr;
   if (splits > 1) {
     st = validate_ws(pool, batch, ws, ws_bytes);
     if (st != SX_OK) return st;
     part = reinterpret_cast<float *>(static_cast<char *>(ws) + ws_layout(pool, batch).attn_part);
   }
-  return launch_attn(pool, batch, q, rows_R, rows_off, total_rows, out, lse, splits, part, want_cta_pair, s);
+  return launch_attn(pool, batch, q, rows_R, rows_off, total_rows, out, lse, splits, part, want_cta_pair, ZcArgs(), s);
 }
 
 }  // extern "C"

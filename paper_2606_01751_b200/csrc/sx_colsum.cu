@@ -16,6 +16,7 @@
 
 #include "sx_internal.h"
 #include "sx_ptx.cuh"
+#include "sx_rotate.cuh"
 
 namespace sx {
 
@@ -44,10 +45,13 @@ struct ColsumParams {
   float *partial;    // [Hkv][total_tokens]
   int num_reqs, max_pages, num_q_heads, num_kv_heads, group, rows_per_tile, total_tokens;
   float scale_log2;
+  const float2 *zc_table;     // zero-copy mode: (cos, sin) per segment and the page classification (sx_rotate.cuh)
+  const int32_t *zc_page_seg;
 };
 
 struct CsBars {
   uint64_t k_full;
+  uint64_t k_rot;  // zero-copy mode: the consumers have rotated the K tile (256 arrivals)
   uint64_t q_full[kCsStages], q_empty[kCsStages];
   uint64_t d_full[2], d_empty[2];
   uint64_t c_full[kCsColStages];
@@ -127,6 +131,9 @@ __device__ __forceinline__ float2 cs_consume(const uint32_t (&d)[2][32], uint32_
   return acc2;
 }
 
+// kZc: 0 = K is read as stored; 1 / 2 = zero-copy mode with half-split / interleaved RoPE pairs: the consumers rotate
+// the rows of the K tile that still are cached source pages before the first MMA reads the tile.
+template <int kZc>
 __global__ void __launch_bounds__(kCsThreads, 2)
 colsum_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_constant__ CUtensorMap tm_k,
               const ColsumParams p) {
@@ -168,6 +175,7 @@ colsum_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_constant__ 
     tma_prefetch_desc(&tm_q);
     tma_prefetch_desc(&tm_k);
     mbar_init(&bars->k_full, 1);
+    mbar_init(&bars->k_rot, 256);
     for (int i = 0; i < kCsStages; ++i) {
       mbar_init(&bars->q_full[i], 1);
       mbar_init(&bars->q_empty[i], 1);
@@ -237,7 +245,7 @@ colsum_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_constant__ 
       const uint64_t k_desc = umma_smem_desc(smem_u32(smem + kCsOffK), 16, 1024);
       const uint64_t q_desc = umma_smem_desc(smem_u32(smem + kCsOffQ), 16, 1024);
       const uint32_t k_lo = (uint32_t)k_desc, q_lo = (uint32_t)q_desc, hi32 = (uint32_t)(k_desc >> 32);
-      mbar_wait(&bars->k_full, 0);
+      mbar_wait(kZc ? &bars->k_rot : &bars->k_full, 0);
       int s = 0, ph = 0;
       for (int it = 0; it < n_it; ++it) {
         const int b = it & 1;
@@ -264,6 +272,13 @@ colsum_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_constant__ 
     const uint32_t lane_addr = (uint32_t)(quarter * 32) << 16;
     float2 acc2 = make_float2(0.f, 0.f);
     const float2 sc2 = make_float2(p.scale_log2, p.scale_log2);
+    if (kZc != 0 && n_it > 0) {
+      mbar_wait(&bars->k_full, 0);
+      rotate_k_tile<kZc - 1, 256>(smem + kCsOffK, kCsHalf, p.zc_page_seg + (size_t)req * p.max_pages + kt * 8,
+                                  n_pages - kt * 8, p.zc_table, (int)threadIdx.x);
+      fence_proxy_async_smem();
+      mbar_arrive(&bars->k_rot);
+    }
     for (int it = 0; it < n_it; ++it) {
       const int b = it & 1, cs = it & (kCsColStages - 1);
       mbar_wait(&bars->c_full[cs], (it / kCsColStages) & 1);
@@ -304,7 +319,8 @@ size_t colsum_tab_bytes(const sx_pool *pool, const sx_batch *b) {
 }
 
 sx_status launch_colsum(const sx_pool *pool, const sx_batch *b, const void *q_new, const float *lse_new,
-                        int lse_by_token, int lse_splits, float *partial, float2 *col_tab, cudaStream_t st) {
+                        int lse_by_token, int lse_splits, float *partial, float2 *col_tab, const ZcArgs &zc,
+                        cudaStream_t st) {
   const int g = pool->num_q_heads / pool->num_kv_heads;
   const int rpt = kTile / g;
   CUtensorMap tm_q, tm_k;
@@ -332,14 +348,17 @@ sx_status launch_colsum(const sx_pool *pool, const sx_batch *b, const void *q_ne
   p.rows_per_tile = rpt;
   p.total_tokens = b->total_tokens;
   p.scale_log2 = (float)(kLog2e / sqrt((double)kHeadDim));
+  p.zc_table = zc.table;
+  p.zc_page_seg = zc.page_seg;
   const int grid = (b->total_tokens / kTile + b->num_reqs) * pool->num_kv_heads;
-  cudaError_t e = cudaFuncSetAttribute(colsum_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, kCsSmemBytes);
+  auto kern = zc.style < 0 ? colsum_kernel<0> : (zc.style == 0 ? colsum_kernel<1> : colsum_kernel<2>);
+  cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, kCsSmemBytes);
   if (e != cudaSuccess) return set_error(SX_ERR_CUDA, "colsum smem attr: %s", cudaGetErrorString(e));
   const int n_qt = b->total_new / rpt + b->num_reqs;  // >= sum_r ceil(|I_nr(r)| / rpt)
   coltab_kernel<<<dim3(n_qt, pool->num_kv_heads), 128, 0, st>>>(p);
   s = check_launch("coltab_kernel");
   if (s != SX_OK) return s;
-  colsum_kernel<<<grid, kCsThreads, kCsSmemBytes, st>>>(tm_q, tm_k, p);
+  kern<<<grid, kCsThreads, kCsSmemBytes, st>>>(tm_q, tm_k, p);
   return check_launch("colsum_kernel");
 }
 

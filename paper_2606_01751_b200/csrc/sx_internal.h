@@ -27,6 +27,7 @@ struct WsLayout {
   size_t sel_scratch;  // int    [num_reqs][4*256 + 4*64] digit histograms and slice counters of the multi-CTA select
   size_t attn_part;    // float  key-split partials of the tcgen05 attention (few CTAs, long context)
   size_t small_part;   // float  split-KV partials of the CUDA-core attention path (sx_attn_small.cu)
+  size_t page_seg;     // int32  [num_reqs][max_pages]    zero-copy mode: segment whose source page the entry still is, or -1
   size_t total;
 };
 WsLayout ws_layout(const sx_pool *pool, const sx_batch *batch);
@@ -37,6 +38,13 @@ sx_status check_launch(const char *what);
 // kernels (one launcher per translation unit)
 sx_status launch_realign(const sx_pool *pools, int num_layers, const sx_batch *b, float2 *table, int4 *page_desc,
                          cudaStream_t st);
+// zero-copy mode: rotation table + page_seg of the workspace (sx_realign.cu); run before a stage that rotates on the fly
+sx_status launch_zc_prepare(const sx_batch *b, float2 *table, int32_t *page_seg, cudaStream_t st);
+struct ZcArgs {  // what a rotating kernel needs; style < 0: not in zero-copy mode
+  int style = -1;
+  const float2 *table = nullptr;
+  const int32_t *page_seg = nullptr;
+};
 sx_status launch_scatter(const sx_pool *pool, const sx_batch *b, const void *k_fresh, const void *v_fresh,
                          const int32_t *rows, const int32_t *rows_off, int32_t max_rows, cudaStream_t st);
 sx_status launch_select(const sx_pool *pool, const sx_batch *b, const float *partial, const int32_t *sel_off,
@@ -47,21 +55,22 @@ size_t select_scratch_bytes(const sx_batch *b);
 // tcgen05 kernels. q_rows: bf16 [total_rows][Hq][128]; rows == nullptr => row n is position n - off[req].
 sx_status launch_attn(const sx_pool *pool, const sx_batch *b, const void *q, const int32_t *rows,
                       const int32_t *rows_off, int32_t total_rows, void *out, float *lse, int kv_splits,
-                      float *part, bool cta_pair, cudaStream_t st);
-int attn_pv_splits(const sx_pool *pool, const sx_batch *b, int32_t total_rows);
+                      float *part, bool cta_pair, const ZcArgs &zc, cudaStream_t st);
+int attn_pv_splits(const sx_pool *pool, const sx_batch *b, int32_t total_rows, int tiles_per_cta);
 size_t attn_part_bytes();
 unsigned long long *attn_tickets(float *part);  // rendezvous words of the key splits, behind the partial buffer
 // first sweep of stage (b) (sx_lse.cu): partial log-sum-exps [kv_splits][total_new][Hq] of the Sparse-Q rows
 int lse_splits(const sx_pool *pool, const sx_batch *b);
 sx_status launch_lse(const sx_pool *pool, const sx_batch *b, const void *q_new, float *lse_ws, int kv_splits,
-                     cudaStream_t st);
+                     const ZcArgs &zc, cudaStream_t st);
 // CUDA-core split-KV attention for fewer than 64 (row, head) pairs per KV head; part = ws.small_part
 sx_status launch_attn_small(const sx_pool *pool, const sx_batch *b, const void *q, const int32_t *rows,
                             const int32_t *rows_off, int32_t total_rows, void *out, float *lse, float *part,
                             cudaStream_t st);
 size_t small_ws_bytes(int num_reqs, int num_kv_heads, int group);
 sx_status launch_colsum(const sx_pool *pool, const sx_batch *b, const void *q_new, const float *lse_new,
-                        int lse_by_token, int lse_splits, float *partial, float2 *col_tab, cudaStream_t st);
+                        int lse_by_token, int lse_splits, float *partial, float2 *col_tab, const ZcArgs &zc,
+                        cudaStream_t st);
 size_t colsum_tab_bytes(const sx_pool *pool, const sx_batch *b);
 
 // descriptor validation (sx_check.cu): one kernel + one error word copied back; synchronises the stream

@@ -16,6 +16,7 @@
 
 #include "sx_internal.h"
 #include "sx_ptx.cuh"
+#include "sx_rotate.cuh"
 
 namespace sx {
 
@@ -40,15 +41,22 @@ struct LseParams {
   float *lse;              // [split][total_new][Hq] natural-log partial normalisers
   int num_reqs, max_pages, num_q_heads, num_kv_heads, group, rows_per_tile, total_new, kv_splits;
   float scale_log2, scale;
+  const float2 *zc_table;  // zero-copy mode: (cos, sin) per segment and the page classification (sx_rotate.cuh)
+  const int32_t *zc_page_seg;
 };
 
 struct LseBars {
   uint64_t q_full;
+  uint64_t k_rot[kLseStages];  // zero-copy mode: the consumers have rotated the K tile of the slot (256 arrivals)
   uint64_t k_full[kLseStages], k_empty[kLseStages];
   uint64_t s_full[2], s_free[2];
   uint32_t tmem_base;
 };
 
+// kZc: 0 = K is read as stored; 1 / 2 = zero-copy mode with half-split / interleaved RoPE pairs: before they turn to
+// S(t), the consumers rotate the rows of K tile t + 1 that still are cached source pages; the MMA of a tile waits for
+// its rotation instead of its TMA completion.
+template <int kZc>
 __global__ void __launch_bounds__(kLseThreads, 2)
 lse_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_constant__ CUtensorMap tm_k, const LseParams p) {
   extern __shared__ uint8_t smem_raw[];
@@ -68,6 +76,7 @@ lse_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_constant__ CUt
     for (int i = 0; i < kLseStages; ++i) {
       mbar_init(&bars->k_full[i], 1);
       mbar_init(&bars->k_empty[i], 1);
+      mbar_init(&bars->k_rot[i], 256);
     }
     for (int i = 0; i < 2; ++i) {
       mbar_init(&bars->s_full[i], 1);
@@ -161,7 +170,7 @@ lse_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_constant__ CUt
       mbar_wait(&bars->q_full, 0);
       for (int t = 0; t < n_tiles; ++t) {
         const int b = t & 1, s = t % kLseStages;
-        mbar_wait(&bars->k_full[s], (t / kLseStages) & 1);
+        mbar_wait(kZc ? &bars->k_rot[s] : &bars->k_full[s], (t / kLseStages) & 1);
         if (t >= 2) mbar_wait(&bars->s_free[b], ((t >> 1) + 1) & 1);
         tc_fence_after();
         const uint32_t kd = k_lo + (uint32_t)s * (kLseTileBytes >> 4);
@@ -184,8 +193,19 @@ lse_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_constant__ CUt
     const int pos = valid ? p.new_idx[row_base + n_local] : -1;
     const uint32_t lane_addr = (uint32_t)(quarter * 32) << 16;
     float m = -INFINITY, l = 0.f;  // running maximum (log2 domain) and sum of this thread's key columns
+    auto rotate_tile = [&](int t) {
+      const int s = t % kLseStages;
+      mbar_wait(&bars->k_full[s], (t / kLseStages) & 1);
+      rotate_k_tile<(kZc > 0 ? kZc - 1 : 0), 256>(smem + kLseOffK + s * kLseTileBytes, kLseHalf,
+                                                   p.zc_page_seg + (size_t)req * p.max_pages + (t0 + t) * 8,
+                                                   n_pages - (t0 + t) * 8, p.zc_table, (int)threadIdx.x);
+      fence_proxy_async_smem();
+      mbar_arrive(&bars->k_rot[s]);
+    };
+    if (kZc != 0 && n_tiles > 0) rotate_tile(0);
     for (int t = 0; t < n_tiles; ++t) {
       const int b = t & 1;
+      if (kZc != 0 && t + 1 < n_tiles) rotate_tile(t + 1);
       mbar_wait(&bars->s_full[b], (t >> 1) & 1);
       tc_fence_after();
       uint32_t sr[2][32];
@@ -267,7 +287,7 @@ int lse_splits(const sx_pool *pool, const sx_batch *b) {
 }
 
 sx_status launch_lse(const sx_pool *pool, const sx_batch *b, const void *q_new, float *lse_ws, int kv_splits,
-                     cudaStream_t st) {
+                     const ZcArgs &zc, cudaStream_t st) {
   const int g = pool->num_q_heads / pool->num_kv_heads;
   const int rpt = kTile / g;
   CUtensorMap tm_q, tm_k;
@@ -292,9 +312,12 @@ sx_status launch_lse(const sx_pool *pool, const sx_batch *b, const void *q_new, 
   p.scale = (float)(1.0 / sqrt((double)kHeadDim));
   p.scale_log2 = (float)(kLog2e / sqrt((double)kHeadDim));
   const int grid = (b->total_new / rpt + b->num_reqs) * pool->num_kv_heads;  // >= sum_r ceil(|I_nr(r)| / rpt) * Hkv
-  cudaError_t e = cudaFuncSetAttribute(lse_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, kLseSmemBytes);
+  p.zc_table = zc.table;
+  p.zc_page_seg = zc.page_seg;
+  auto kern = zc.style < 0 ? lse_kernel<0> : (zc.style == 0 ? lse_kernel<1> : lse_kernel<2>);
+  cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, kLseSmemBytes);
   if (e != cudaSuccess) return set_error(SX_ERR_CUDA, "lse smem attr: %s", cudaGetErrorString(e));
-  e = launch_pdl(lse_kernel, dim3(grid * p.kv_splits), dim3(kLseThreads), kLseSmemBytes, st, 1, tm_q, tm_k, p);
+  e = launch_pdl(kern, dim3(grid * p.kv_splits), dim3(kLseThreads), kLseSmemBytes, st, 1, tm_q, tm_k, p);
   if (e != cudaSuccess) return set_error(SX_ERR_CUDA, "lse launch: %s", cudaGetErrorString(e));
   return check_launch("lse_kernel");
 }

@@ -9,6 +9,7 @@
 // fp64 (an fp32 product Delta*theta_i loses ~3e-3 in the sine at Delta ~ 1.3e5), one RNE to bf16.
 #include "sx_internal.h"
 #include "sx_ptx.cuh"
+#include "sx_rotate.cuh"
 
 namespace sx {
 
@@ -23,11 +24,7 @@ __global__ void rope_table_kernel(const sx_segment *__restrict__ segs, int num_s
   int idx = blockIdx.x * blockDim.x + threadIdx.x;
   if (idx < num_segments * 64) {
     int m = idx >> 6, i = idx & 63;
-    double delta = (double)(segs[m].new_pos - segs[m].old_pos);
-    double inv_freq = pow(theta, -2.0 * (double)i / (double)kHeadDim);
-    double s, c;
-    sincos(delta * inv_freq, &s, &c);
-    table[idx] = make_float2((float)c, (float)s);
+    table[idx] = rope_cos_sin(theta, segs[m].new_pos - segs[m].old_pos, i);
   }
   if (idx < total_pages) {
     // segment m with src_off[m] <= page < src_off[m] + len/16 (src_off ascending: binary search)
@@ -54,36 +51,6 @@ __device__ __forceinline__ void st_stream(uint4 *p, const uint4 &v) {
   asm volatile("st.global.L1::no_allocate.v4.u32 [%0], {%1, %2, %3, %4};" ::"l"(p), "r"(v.x), "r"(v.y), "r"(v.z),
                "r"(v.w)
                : "memory");
-}
-
-__device__ __forceinline__ float bf_lo(uint32_t u) { return __uint_as_float(u << 16); }
-__device__ __forceinline__ float bf_hi(uint32_t u) { return __uint_as_float(u & 0xFFFF0000u); }
-
-// half-split pairing: element i of `a` (columns [8c, 8c+8)) pairs with element i of `b`
-// (columns [64+8c, 64+8c+8)); cs[e] = (cos, sin) of pair index 8c+e.
-__device__ __forceinline__ void rotate_split(uint4 &a, uint4 &b, const float2 *cs) {
-  uint32_t *pa = reinterpret_cast<uint32_t *>(&a);
-  uint32_t *pb = reinterpret_cast<uint32_t *>(&b);
-#pragma unroll
-  for (int w = 0; w < 4; ++w) {
-    float x0 = bf_lo(pa[w]), x1 = bf_hi(pa[w]);
-    float y0 = bf_lo(pb[w]), y1 = bf_hi(pb[w]);
-    float2 c0 = cs[2 * w], c1 = cs[2 * w + 1];
-    float xr0 = fmaf(x0, c0.x, -(y0 * c0.y)), yr0 = fmaf(x0, c0.y, y0 * c0.x);
-    float xr1 = fmaf(x1, c1.x, -(y1 * c1.y)), yr1 = fmaf(x1, c1.y, y1 * c1.x);
-    pa[w] = pack_bf16x2(xr0, xr1);
-    pb[w] = pack_bf16x2(yr0, yr1);
-  }
-}
-// interleaved pairing: the 4 pairs (2i, 2i+1) of one 16-byte chunk; cs[e] = pair 4c+e.
-__device__ __forceinline__ void rotate_inter(uint4 &a, const float2 *cs) {
-  uint32_t *pa = reinterpret_cast<uint32_t *>(&a);
-#pragma unroll
-  for (int w = 0; w < 4; ++w) {
-    float x = bf_lo(pa[w]), y = bf_hi(pa[w]);
-    float2 c = cs[w];
-    pa[w] = pack_bf16x2(fmaf(x, c.x, -(y * c.y)), fmaf(x, c.y, y * c.x));
-  }
 }
 
 constexpr int kRealignThreads = 128;
@@ -161,6 +128,40 @@ realign_kernel(const __grid_constant__ LayerPools pools, int num_kv_heads, const
       st_stream(vd + t + 128, v1);
     }
   }
+}
+
+// Zero-copy mode (sx_batch::zero_copy): nothing is copied; the stage kernels rotate cached K on the fly. They need,
+// per request and logical page, whether the page still IS the cached source page of a segment (then its keys are
+// stored at their old positions: rotate by that segment's Delta) or a private page (already at its position):
+//   page_seg[req][lp] = m if a segment m covers lp and k_block_table[req][lp] == the source page of m for lp, else -1
+// and the same per-segment (cos, sin) table as the copy kernel.
+__global__ void zc_prepare_kernel(const sx_segment *__restrict__ segs, int num_segments, double theta,
+                                  float2 *__restrict__ table, const int32_t *__restrict__ src_blocks,
+                                  const int32_t *__restrict__ k_table, int num_reqs, int max_pages,
+                                  const int32_t *__restrict__ seq_len, int32_t *__restrict__ page_seg) {
+  const int idx = blockIdx.x * blockDim.x + threadIdx.x;
+  if (idx < num_segments * 64) {
+    const int m = idx >> 6, i = idx & 63;
+    table[idx] = rope_cos_sin(theta, segs[m].new_pos - segs[m].old_pos, i);
+  }
+  if (idx < num_reqs * max_pages) {
+    const int req = idx / max_pages, lp = idx - req * max_pages;
+    int m = -1;
+    if (lp * kPage < seq_len[req]) {
+      m = find_segment(segs, num_segments, req, lp * kPage);
+      if (m >= 0 && k_table[idx] != src_blocks[segs[m].src_off + lp - segs[m].new_pos / kPage]) m = -1;
+    }
+    page_seg[idx] = m;
+  }
+}
+
+sx_status launch_zc_prepare(const sx_batch *b, float2 *table, int32_t *page_seg, cudaStream_t st) {
+  const int a = b->num_segments * 64, c = b->num_reqs * b->max_pages_per_req;
+  const int n = a > c ? a : c;
+  zc_prepare_kernel<<<(n + 127) / 128, 128, 0, st>>>(b->segments, b->num_segments, b->rope_theta, table, b->src_blocks,
+                                                    b->k_block_table, b->num_reqs, b->max_pages_per_req, b->seq_len,
+                                                    page_seg);
+  return check_launch("zc_prepare_kernel");
 }
 
 sx_status launch_realign(const sx_pool *pools, int num_layers, const sx_batch *b, float2 *table, int4 *page_desc,

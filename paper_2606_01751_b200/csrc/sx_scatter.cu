@@ -10,6 +10,7 @@
 // warp, no atomics, no second launch). The kernel is launched with programmatic dependent launch allowed.
 #include "sx_internal.h"
 #include "sx_ptx.cuh"
+#include "sx_rotate.cuh"
 
 namespace sx {
 
@@ -59,12 +60,52 @@ __device__ __forceinline__ void scatter_row(uint4 *pool_k, uint4 *pool_v, int nu
   }
 }
 
-template <bool kCow>
+// zero-copy mode (include/sparsex.h): what the copy-on-write of a K page needs to rotate a still-shared source page
+struct ScatterZc {
+  const sx_segment *segs;
+  const int32_t *src_blocks;
+  int num_segments;
+  int style;  // -1: not in zero-copy mode
+  double theta;
+};
+
+// copy-on-write of one K page in zero-copy mode: K[priv] = R_delta K[src], one warp (same arithmetic as realign_kernel)
+__device__ __forceinline__ void cow_rotate_page(const uint4 *__restrict__ s, uint4 *__restrict__ d, int num_kv_heads,
+                                                int style, double theta, int delta, int lane) {
+  if (style == 0) {
+    // items (head, row, c < 8): chunks c and c + 8 of the row; i = lane + 32 k keeps c = lane & 7
+    const int c = lane & 7;
+    float2 cs[8];
+#pragma unroll
+    for (int e = 0; e < 8; ++e) cs[e] = rope_cos_sin(theta, delta, 8 * c + e);
+    const int items = num_kv_heads * kPage * 8;
+    for (int i = lane; i < items; i += 32) {
+      const int o = (i >> 3) * 16 + c;
+      uint4 a = s[o], b = s[o + 8];
+      rotate_split(a, b, cs);
+      d[o] = a;
+      d[o + 8] = b;
+    }
+  } else {
+    const int c16 = lane & 15;
+    float2 cs[4];
+#pragma unroll
+    for (int e = 0; e < 4; ++e) cs[e] = rope_cos_sin(theta, delta, 4 * c16 + e);
+    const int items = num_kv_heads * kPage * 16;
+    for (int i = lane; i < items; i += 32) {
+      uint4 a = s[i];
+      rotate_inter(a, cs);
+      d[i] = a;
+    }
+  }
+}
+
+template <bool kCow, bool kZc = false>
 __global__ void __launch_bounds__(kScatterWarps * 32)
 scatter_kernel(uint4 *pool_k, uint4 *pool_v, int num_kv_heads, int num_reqs, int max_pages, int32_t *k_table,
                int32_t *v_table, const int32_t *__restrict__ cow_private, const uint4 *__restrict__ k_fresh,
                const uint4 *__restrict__ v_fresh, const int32_t *__restrict__ rows,
-               const int32_t *__restrict__ rows_off) {
+               const int32_t *__restrict__ rows_off, const ScatterZc zc) {
   griddep_launch();  // the next kernel's prologue may overlap this one
   griddep_wait();    // the row list / the pool may be outputs of the previous kernel
   const int n = blockIdx.x * kScatterWarps + (threadIdx.x >> 5);
@@ -89,7 +130,16 @@ scatter_kernel(uint4 *pool_k, uint4 *pool_v, int num_kv_heads, int num_reqs, int
     if (kb != priv) {
       const uint4 *s = pool_k + (size_t)kb * page_chunks;
       uint4 *d = pool_k + (size_t)priv * page_chunks;
-      for (int i = lane; i < page_chunks; i += 32) d[i] = s[i];
+      // zero-copy mode: a page that still is the cached source page of its segment holds keys at their OLD positions
+      int m = -1;
+      if (kZc) {
+        m = find_segment(zc.segs, zc.num_segments, req, pg * kPage);
+        if (m >= 0 && kb != zc.src_blocks[zc.segs[m].src_off + pg - zc.segs[m].new_pos / kPage]) m = -1;
+      }
+      if (kZc && m >= 0)
+        cow_rotate_page(s, d, num_kv_heads, zc.style, zc.theta, zc.segs[m].new_pos - zc.segs[m].old_pos, lane);
+      else
+        for (int i = lane; i < page_chunks; i += 32) d[i] = s[i];
     }
     if (vb != priv) {
       const uint4 *s = pool_v + (size_t)vb * page_chunks;
@@ -118,15 +168,25 @@ sx_status launch_scatter(const sx_pool *pool, const sx_batch *b, const void *k_f
   uint4 *pv = reinterpret_cast<uint4 *>(pool->v);
   const int grid = (max_rows + kScatterWarps - 1) / kScatterWarps;
   const uint4 *kf = reinterpret_cast<const uint4 *>(k_fresh), *vf = reinterpret_cast<const uint4 *>(v_fresh);
+  ScatterZc zc;
+  zc.segs = b->segments;
+  zc.src_blocks = b->src_blocks;
+  zc.num_segments = b->num_segments;
+  zc.style = (b->zero_copy && b->num_segments > 0) ? b->rope_style : -1;
+  zc.theta = b->rope_theta;
   cudaError_t e;
-  if (b->cow_private)
+  if (b->cow_private && zc.style >= 0)
+    e = launch_pdl(scatter_kernel<true, true>, dim3(grid), dim3(kScatterWarps * 32), 0, st, 1, pk, pv, pool->num_kv_heads,
+                   b->num_reqs, b->max_pages_per_req, b->k_block_table, b->v_block_table, b->cow_private, kf, vf, rows,
+                   rows_off, zc);
+  else if (b->cow_private)
     e = launch_pdl(scatter_kernel<true>, dim3(grid), dim3(kScatterWarps * 32), 0, st, 1, pk, pv, pool->num_kv_heads,
                    b->num_reqs, b->max_pages_per_req, b->k_block_table, b->v_block_table, b->cow_private, kf, vf, rows,
-                   rows_off);
+                   rows_off, zc);
   else
     e = launch_pdl(scatter_kernel<false>, dim3(grid), dim3(kScatterWarps * 32), 0, st, 1, pk, pv, pool->num_kv_heads,
                    b->num_reqs, b->max_pages_per_req, b->k_block_table, b->v_block_table, b->cow_private, kf, vf, rows,
-                   rows_off);
+                   rows_off, zc);
   if (e != cudaSuccess) return set_error(SX_ERR_CUDA, "scatter launch: %s", cudaGetErrorString(e));
   return check_launch("scatter_kernel");
 }

@@ -103,6 +103,7 @@ class Layout:
     salient_frac: float
     pool_salient: List[np.ndarray]     # bool [len] per pool segment
     cow: bool
+    zero_copy: bool = False            # K tables alias the cached source pages too (include/sparsex.h, zero-copy mode)
 
     @property
     def num_segments(self) -> int:
@@ -260,6 +261,19 @@ def build_layout(name: str, cfg_id: int, num_q_heads: int, num_kv_heads: int, ro
         new_idx=(np.concatenate(new_idx).astype(np.int32) if new_idx else np.zeros(0, np.int32)),
         k_per_req=k_per_req, pool_segments=pool_segments, pool_seg_pages=pool_seg_pages,
         salient_frac=salient_frac, pool_salient=pool_salient, cow=cow)
+
+
+def zero_copy_layout(lay: Layout) -> Layout:
+    """The same batch described for zero-copy mode (include/sparsex.h): the K and V table entries of every reused
+    page point at the shared source page, the request's own page becomes the reserved private page (cow_private)
+    that the first scatter into the page fills."""
+    kbt, cowp = lay.k_block_table.copy(), np.full_like(lay.k_block_table, -1)
+    for (r, ln, _old, new_pos, src_off) in (tuple(int(v) for v in s) for s in lay.segments):
+        p0, n = new_pos // PAGE, ln // PAGE
+        cowp[r, p0:p0 + n] = lay.k_block_table[r, p0:p0 + n]
+        kbt[r, p0:p0 + n] = lay.src_blocks[src_off:src_off + n]
+    return dataclasses.replace(lay, name=lay.name + "-zc", k_block_table=kbt, v_block_table=kbt.copy(),
+                               cow_private=cowp, cow=True, zero_copy=True)
 
 
 def build_layer(lay: Layout, layer: int = 0, threads: int = 8, need_q: bool = True) -> LayerTensors:

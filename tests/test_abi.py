@@ -32,9 +32,10 @@ def test_header_symbols_are_exported(lib):
 
 
 def test_struct_sizes_match_header():
-    # int32 x5 after two pointers; the batch struct has 7 int32, 9 pointers, a double and an int32
+    # int32 x5 after two pointers; the batch struct has 7 int32, 9 pointers, a double and two int32
     assert ctypes.sizeof(sx.SxPool) == 2 * 8 + 5 * 4 + 4
     assert ctypes.sizeof(sx.SxBatch) == 7 * 4 + 4 + 9 * 8 + 8 + 8
+    assert sx.SxBatch.zero_copy.offset == sx.SxBatch.rope_style.offset + 4
 
 
 def _host_structs(lay):
@@ -116,3 +117,38 @@ def test_check_calls_validate_host_arguments_first(lib):
     assert lib.sx_check_batch(ctypes.byref(pool), ctypes.byref(b), ws, 16, None) == -3
     assert lib.sx_check_rows(ctypes.byref(pool), ctypes.byref(b), ws, None, 4, ws, 1 << 30, None) == -1
     assert lib.sx_launch_count() >= 0
+
+
+def test_zero_copy_mode_host_rules(lib):
+    """include/sparsex.h, zero-copy mode: the re-alignment refuses the descriptor, the scatter needs reserved private
+    pages, CUDA-core kernels and CTA pairs are not available -- all decided on the host, before any launch."""
+    lay = wl.config_tiny()
+    pool, b = _host_structs(lay)
+    ws = ctypes.c_void_p(0x10000)
+    b.zero_copy = 2
+    assert lib.sx_check_batch(ctypes.byref(pool), ctypes.byref(b), ws, 1 << 30, None) == -1
+    b.zero_copy = 1
+    assert lib.sx_rope_realign(ctypes.byref(pool), ctypes.byref(b), ws, 1 << 30, None) == -1
+    assert b"zero-copy" in lib.sx_last_error()
+    assert lib.sx_scatter_kv(ctypes.byref(pool), ctypes.byref(b), ws, ws, ws, ws, 4, None) == -1
+    assert b"cow_private" in lib.sx_last_error()
+    for flag in (2, 4):
+        assert lib.sx_sparse_attn(ctypes.byref(pool), ctypes.byref(b), flag, ws, ws, ws, 4, ws, None, ws, 1 << 30,
+                                  None) == -2
+        assert b"zero-copy" in lib.sx_last_error()
+
+
+def test_zero_copy_layout_aliases_every_reused_page():
+    lay = wl.config_tiny(seed_id=10, tail=5)
+    z = wl.zero_copy_layout(lay)
+    assert z.zero_copy and z.cow and not lay.zero_copy
+    covered = np.zeros(lay.k_block_table.shape, dtype=bool)
+    for (req, ln, _old, new, so) in lay.segments.tolist():
+        p0, n = new // 16, ln // 16
+        covered[req, p0:p0 + n] = True
+        assert np.array_equal(z.k_block_table[req, p0:p0 + n], lay.src_blocks[so:so + n])
+        assert np.array_equal(z.cow_private[req, p0:p0 + n], lay.k_block_table[req, p0:p0 + n])
+    assert np.array_equal(z.k_block_table[~covered], lay.k_block_table[~covered])
+    assert np.all(z.cow_private[~covered] == -1)
+    assert np.array_equal(z.v_block_table, z.k_block_table)
+    assert np.array_equal(lay.k_block_table, wl.config_tiny(seed_id=10, tail=5).k_block_table)   # input untouched

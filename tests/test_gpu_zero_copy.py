@@ -1,0 +1,167 @@
+"""GPU parity of zero-copy mode (include/sparsex.h, sx_batch::zero_copy; S9 NEXT-3): the block tables
+of reused pages point at the shared cached pages, nothing is re-aligned up front, the stage kernels rotate K while
+they read it and the scatter copies-on-write (rotating) only the pages it writes.
+
+What must hold: the rotation done on the fly has the bits sx_rope_realign would have stored, so scores, S_key and R
+are those of the copy path (and of the fp64 oracle, bit-exact sets); attention within the same tolerance against
+fp64; every page written is a private page whose content equals the copy path's page bit for bit; every page not
+written still is the shared source page, unmodified; V is never rotated.
+"""
+import numpy as np
+import pytest
+import torch
+
+from oracle import sx_oracle as orc
+from paper_2606_01751_b200 import workloads as wl
+
+from helpers import check_close, oracle_layer
+from test_gpu_parity import SCORE_RTOL, _gpu, prepared
+
+pytestmark = pytest.mark.gpu
+
+ZC_CASES = ["tiny", "tiny-ragged", "tiny-interleaved", "tiny-g7", "tiny-g1", "tiny-prefix", "C1", "C2-quarter",
+            "C3-eighth", "C4-eighth", "C5-1/16"]
+
+
+def _seg_page_mask(lay):
+    """bool [num_reqs][max_pages]: logical page is covered by a reused segment."""
+    m = np.zeros(lay.k_block_table.shape, dtype=bool)
+    for (req, ln, _old, new, _so) in lay.segments.tolist():
+        m[req, new // 16:(new + ln) // 16] = True
+    return m
+
+
+@pytest.mark.parametrize("name", ZC_CASES)
+def test_zero_copy_sparse_layer(name):
+    GpuLayer, dev_to_bits = _gpu()
+    lay, lt, res, pk, pv, kt, vt = prepared(name)
+    g0 = GpuLayer(lay, lt)                    # copy path: realign, then the same stages
+    g0.step_sparse()
+    zlay = wl.zero_copy_layout(lay)
+    g = GpuLayer(zlay, lt)
+    g.step_sparse(do_realign=False)
+    torch.cuda.synchronize()
+    # scores: same kernels, same decomposition, K bits identical -> identical to the copy path
+    assert np.array_equal(g.scores.cpu().numpy(), g0.scores.cpu().numpy())
+    sc = g.scores.cpu().numpy().astype(np.float64)
+    sel, rows = g.sel_idx.cpu().numpy(), g.rows_R.cpu().numpy()
+    out = orc.bf16_to_f64(dev_to_bits(g.out))
+    lse = g.lse.cpu().numpy().astype(np.float64)
+    for r in range(lay.num_reqs):
+        o, t = int(lay.tok_off[r]), int(lay.seq_len[r])
+        rel = np.abs(sc[o:o + t] - res.scores[r]) / (np.abs(res.scores[r]) + 1e-2)
+        assert rel.max() < SCORE_RTOL
+        s0, s1 = g.sel_off_h[r], g.sel_off_h[r + 1]
+        r0, r1 = g.rows_off_h[r], g.rows_off_h[r + 1]
+        assert np.array_equal(sel[s0:s1], res.sel[r]), (name, r)
+        assert np.array_equal(rows[r0:r1], res.rows[r]), (name, r)
+        check_close("%s zero-copy req %d O" % (name, r), out[r0:r1], res.out[r])
+        assert np.max(np.abs(lse[r0:r1] - res.lse[r])) < 2e-3
+    # ---- pages and tables
+    gk, gv = dev_to_bits(g.pool_k), dev_to_bits(g.pool_v)
+    gk0 = dev_to_bits(g0.pool_k)
+    gkt, gvt = g.batch.k_block_table.cpu().numpy(), g.batch.v_block_table.cpu().numpy()
+    in_seg = _seg_page_mask(lay)
+    written = np.zeros_like(in_seg)
+    for r in range(lay.num_reqs):
+        written[r, np.unique(res.rows[r] // 16)] = True
+    priv = lay.k_block_table                  # the request's own pages = the reserved private pages
+    flipped = in_seg & written
+    assert np.array_equal(gkt[flipped], priv[flipped]) and np.array_equal(gvt[flipped], priv[flipped])
+    still = in_seg & ~written
+    assert np.array_equal(gkt[still], zlay.k_block_table[still]) and np.array_equal(gvt[still], zlay.v_block_table[still])
+    assert np.array_equal(gkt[~in_seg], priv[~in_seg])
+    # written pages: bit-identical to the copy path's pages (rotated copy + fresh rows); V to the oracle's
+    pages = priv[flipped | (~in_seg & written)]
+    assert np.array_equal(gk[pages], gk0[pages])
+    assert np.array_equal(gv[pages], pv[pages])
+    # shared source pages untouched; private pages of unwritten reused pages never filled (the memory not spent)
+    src = np.concatenate(lay.pool_seg_pages)
+    assert np.array_equal(gk[src], lt.pool_k[src]) and np.array_equal(gv[src], lt.pool_v[src])
+    assert not gk[priv[still]].any() and not gv[priv[still]].any()
+    # V through the final tables = the oracle's logical V everywhere
+    for r in range(lay.num_reqs):
+        t = int(lay.seq_len[r])
+        assert np.array_equal(orc.gather_tokens(gv, gvt[r], t), orc.gather_tokens(pv, vt[r], t))
+
+
+@pytest.mark.parametrize("name", ["tiny", "tiny-interleaved", "tiny-ragged", "C1"])
+def test_zero_copy_full_layer(name):
+    """Full-attention layer in zero-copy mode: every page is written, so every reused page goes through the rotating
+    copy-on-write before its rows are overwritten; attention then reads private pages only."""
+    GpuLayer, dev_to_bits = _gpu()
+    lay, lt = prepared(name)[:2]
+    res, pk, pv, kt, vt = oracle_layer(lay, lt, mode="full")
+    g = GpuLayer(wl.zero_copy_layout(lay), lt)
+    g.step_full(do_realign=False)
+    torch.cuda.synchronize()
+    out = orc.bf16_to_f64(dev_to_bits(g.out))
+    lse = g.lse.cpu().numpy().astype(np.float64)
+    for r in range(lay.num_reqs):
+        o, t = int(lay.tok_off[r]), int(lay.seq_len[r])
+        check_close("%s zero-copy full O" % name, out[o:o + t], res.out[r])
+        assert np.max(np.abs(lse[o:o + t] - res.lse[r])) < 2e-3
+    assert np.array_equal(g.batch.k_block_table.cpu().numpy(), lay.k_block_table)
+    gk = dev_to_bits(g.pool_k)
+    # rows of a ragged last page beyond seq_len keep the rotated copy; everything else is fresh: compare the tokens
+    for r in range(lay.num_reqs):
+        t = int(lay.seq_len[r])
+        assert np.array_equal(orc.gather_tokens(gk, lay.k_block_table[r], t), orc.gather_tokens(pk, kt[r], t))
+
+
+@pytest.mark.parametrize("name,nlast", [("C5-1/16", 16), ("C1", 40), ("C3-eighth", 24), ("tiny-interleaved", 8)])
+def test_zero_copy_attention_reads_rotated_pages(name, nlast):
+    """Attention over an arbitrary small row set on a pool where NOTHING has been made private yet (only the new
+    tokens are scattered): every reused key the rows see is rotated in shared memory, key splits included."""
+    GpuLayer, dev_to_bits = _gpu()
+    lay, lt = prepared(name)[:2]
+    # oracle state: realign + scatter(I_nr)
+    pk, pv = lt.pool_k.copy(), lt.pool_v.copy()
+    kt, vt = lay.k_block_table.copy(), lay.v_block_table.copy()
+    orc.realign(pk, pv, kt, vt, lay.segments, lay.src_blocks, lay.rope_theta, lay.rope_style)
+    g = GpuLayer(wl.zero_copy_layout(lay), lt)
+    g.scatter_new()
+    rows, off = [], [0]
+    for r in range(lay.num_reqs):
+        t, o = int(lay.seq_len[r]), int(lay.tok_off[r])
+        nidx = lay.new_idx[lay.new_off[r]:lay.new_off[r + 1]]
+        orc.scatter_kv(pk, pv, kt, vt, None, r, nidx, lt.k_fresh[o + nidx], lt.v_fresh[o + nidx])
+        rr = np.unique(np.concatenate([np.arange(max(t - nlast, 0), t), [3, t // 2]])).astype(np.int32)
+        rows.append(rr)
+        off.append(off[-1] + len(rr))
+    g.rows_off = torch.tensor(off, dtype=torch.int32, device=g.dev)
+    g.sel_off = torch.zeros(lay.num_reqs + 1, dtype=torch.int32, device=g.dev)
+    g.stage_rows(torch.zeros(0, dtype=torch.int32, device=g.dev), torch.from_numpy(np.concatenate(rows)).to(g.dev))
+    g.attend()
+    torch.cuda.synchronize()
+    out = orc.bf16_to_f64(dev_to_bits(g.out))
+    lse = g.lse.cpu().numpy().astype(np.float64)
+    for r in range(lay.num_reqs):
+        o, t = int(lay.tok_off[r]), int(lay.seq_len[r])
+        ref_o, ref_l = orc.attention(pk, pv, kt[r], vt[r], t, lt.q_full[o + rows[r]], rows[r], lay.num_q_heads,
+                                     want_lse=True)
+        check_close("%s zero-copy req %d O" % (name, r), out[off[r]:off[r + 1]], ref_o)
+        assert np.max(np.abs(lse[off[r]:off[r + 1]] - ref_l)) < 2e-3
+    # the tables still alias the source pages: attention wrote nothing
+    assert np.array_equal(g.batch.k_block_table.cpu().numpy(), wl.zero_copy_layout(lay).k_block_table)
+
+
+def test_zero_copy_refusals():
+    from paper_2606_01751_b200 import binding as sx
+    GpuLayer, _ = _gpu()
+    lay, lt = prepared("tiny")[:2]
+    g = GpuLayer(wl.zero_copy_layout(lay), lt)
+    with pytest.raises(sx.SparseXError, match="zero-copy"):
+        g.realign()
+    g.scatter_new()
+    g.select()
+    g.stage_rows(g.sel_idx, g.rows_R)
+    with pytest.raises(sx.SparseXError, match="zero-copy"):
+        g.attend(cuda_core=True)
+    g.cta_pair = True
+    with pytest.raises(sx.SparseXError, match="zero-copy"):
+        g.attend()
+    # scatter without reserved private pages would have to write the shared source pages
+    nocow = sx.DeviceBatch(wl.zero_copy_layout(lay), cow=False)
+    with pytest.raises(sx.SparseXError, match="cow_private"):
+        sx.scatter_kv(g.pool, nocow, g.kf_sel, g.vf_sel, g.sel_idx, g.sel_off, max_rows=int(g.sel_idx.numel()))
