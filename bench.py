@@ -477,6 +477,92 @@ def measure_s6(ctx, reps=10):
     return out
 
 
+def measure_zero_copy(ctx, reps=10):
+    """Zero-copy mode (include/sparsex.h; S9 NEXT-3) against the copy path, same inputs, same stages:
+      (i)  one sparse C4 layer (16 requests, two-sweep selection), every stage timed between events;
+      (ii) the S6 row sets (stage (c) alone over a 32K / 133K context where NOTHING has been made private: every
+           reused key is rotated in shared memory).
+    Block tables are restored before every repetition of the zero-copy arm (its scatter flips them), L2 is flushed
+    between repetitions. Memory: private pages a request holds for its reused segments after the layer."""
+    torch, sx, dev = ctx["torch"], ctx["sx"], ctx["dev"]
+    from paper_2606_01751_b200.layer import GpuLayer
+    flush = torch.empty(512 << 20, dtype=torch.uint8, device=dev)
+    out = {}
+
+    def timed(stages):
+        evs = [torch.cuda.Event(enable_timing=True) for _ in range(len(stages) + 1)]
+        evs[0].record()
+        for i, (_, fn) in enumerate(stages):
+            fn()
+            evs[i + 1].record()
+        torch.cuda.synchronize()
+        return [evs[i].elapsed_time(evs[i + 1]) for i in range(len(stages))]
+
+    # ---- (i) C4 sparse layer
+    lay = wl.CONFIGS["C4"]()
+    zlay = wl.zero_copy_layout(lay)
+    dl = DevLayer(lay, 0, dev, torch)
+    g0, g1 = GpuLayer(lay, dl, dev), GpuLayer(zlay, dl, dev)   # one pool: the arms run one after the other
+    kt1, vt1 = g1.batch.k_block_table.clone(), g1.batch.v_block_table.clone()
+    g0.step_sparse()                    # fixes S_key / R (identical in both arms: tests/test_gpu_zero_copy.py)
+    g1.stage_rows(g0.sel_idx, g0.rows_R)
+    for label, g in (("copy", g0), ("zero_copy", g1)):
+        stages = [("scatter_new", g.scatter_new), ("select", lambda g=g: g.select(want_scores=False)),
+                  ("scatter_sel", g.scatter_sel), ("attention", lambda g=g: g.attend(want_lse=False))]
+        if label == "copy":
+            stages.insert(0, ("realign", g.realign))
+        acc = []
+        for i in range(reps + 3):
+            if label == "zero_copy":
+                g.batch.k_block_table.copy_(kt1)
+                g.batch.v_block_table.copy_(vt1)
+            flush.zero_()
+            t = timed(stages)
+            if i >= 3:
+                acc.append(t)
+        med = np.median(np.asarray(acc), axis=0)
+        out.setdefault("C4_sparse_layer", {})[label] = {
+            "stage_ms": {n: round(float(v), 4) for (n, _), v in zip(stages, med)}, "ms": round(float(med.sum()), 4)}
+    torch.cuda.synchronize()
+    page_bytes = 2 * lay.num_kv_heads * 16 * 128 * 2    # K and V
+    flipped = int((g1.batch.k_block_table != kt1).sum().item())
+    out["C4_sparse_layer"]["private_pages"] = {
+        "copy": lay.total_seg_pages, "zero_copy": flipped, "page_bytes": page_bytes,
+        "copy_mb": round(lay.total_seg_pages * page_bytes / 1e6, 1), "zero_copy_mb": round(flipped * page_bytes / 1e6, 1)}
+    del g0, g1, dl
+    torch.cuda.empty_cache()
+
+    # ---- (ii) S6 row sets over untouched shared pages
+    for cfg, layer, lasts in (("C3", 4, (8,)), ("C5", 0, (16,))):
+        lay = wl.CONFIGS[cfg]()
+        zlay = wl.zero_copy_layout(lay)
+        dl = DevLayer(lay, layer, dev, torch)
+        g0, g1 = GpuLayer(lay, dl, dev), GpuLayer(zlay, dl, dev)
+        T, hq, hkv = lay.total_tokens, lay.num_q_heads, lay.num_kv_heads
+        g0.realign()
+        g0.scatter_new()    # (new tokens live in the request's own pages in both arms)
+        for n in lasts:
+            rows = torch.arange(T - n, T, dtype=torch.int32, device=dev)
+            off = torch.tensor([0, n], dtype=torch.int32, device=dev)
+            q = g0.q_full[T - n:T].contiguous()
+            o = torch.empty((n, hq, 128), dtype=torch.int16, device=dev)
+            res = {}
+            for label, g in (("copy", g0), ("zero_copy", g1)):
+                ms = []
+                for i in range(reps + 3):
+                    flush.zero_()
+                    ms.append(timed([("attention", lambda g=g: sx.sparse_attn(g.pool, g.batch, q, o, rows_R=rows,
+                                                                                 rows_off=off, total_rows=n))])[0])
+                t_ms = float(np.median(ms[3:]))
+                res[label] = {"ms": round(t_ms, 4), "hbm_gbs": round(4.0 * T * hkv * 128 / (t_ms * 1e-3) / 1e9, 1)}
+            out["%s_last%d_rows" % (cfg, n)] = res
+        del g0, g1, dl
+        torch.cuda.empty_cache()
+    del flush
+    torch.cuda.empty_cache()
+    return out
+
+
 def run_ours(args):
     import torch
     from paper_2606_01751_b200 import binding as sx
@@ -498,6 +584,12 @@ def run_ours(args):
             print(json.dumps({"metric": "small_row_attention_hbm", "unit": "GB/s", "n_gpus": 1, "dtype": "bf16",
                               "data": "synthetic", "config": {"workload": "S6: last rows of a 32K / 133K context"},
                               "cases": measure_s6(ctx, reps=max(args.steps, 3))}), flush=True)
+        return
+    if cfg == "ZC":   # supplementary: zero-copy mode against the copy path (S9)
+        if rank == 0:
+            print(json.dumps({"metric": "zero_copy_vs_copy", "unit": "ms", "n_gpus": 1, "dtype": "bf16",
+                              "data": "synthetic", "config": {"workload": "ZC: C4 sparse layer; S6 row sets"},
+                              "cases": measure_zero_copy(ctx, reps=max(args.steps, 3))}), flush=True)
         return
     m = measure(cfg, args.steps, args.warmup, ctx)
     # the other configs of BASELINE.json (north_star: throughput of all five at 1 GPU): short runs, same code path
@@ -531,6 +623,7 @@ def run_ours(args):
                 "stage_ms": {k: round(v, 4) for k, v in o["stage_ms"].items()},
                 "note": "one sparse C3 layer: realign, scatter(I_nr), two-sweep selection, scatter(S_key), attention"}
         others["S6"] = measure_s6(ctx)
+        others["zero_copy"] = measure_zero_copy(ctx)
     if rank != 0:
         return
     stack, n_layers, T = m["stack"], m["n_layers"], m["T"]
@@ -842,7 +935,7 @@ def main():
     ap.add_argument("--gpus", type=int, default=1)
     ap.add_argument("--steps", type=int, default=10)
     ap.add_argument("--warmup", type=int, default=3)
-    ap.add_argument("--config", default="C3", choices=list(wl.CONFIGS) + ["S6"])
+    ap.add_argument("--config", default="C3", choices=list(wl.CONFIGS) + ["S6", "ZC"])
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--no-cpu", action="store_true")
     ap.add_argument("--no-cpu-measured", action="store_true",

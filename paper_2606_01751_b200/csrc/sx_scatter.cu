@@ -69,33 +69,72 @@ struct ScatterZc {
   double theta;
 };
 
+// bit copy of one page by one warp: n (a multiple of 256) 16-byte chunks, eight loads in flight per lane (source and
+// destination never overlap: a shared source page / a reserved private page)
+__device__ __forceinline__ void copy_page(const uint4 *__restrict__ s, uint4 *__restrict__ d, int n, int lane) {
+  for (int i = lane; i < n; i += 256) {
+    uint4 t[8];
+#pragma unroll
+    for (int k = 0; k < 8; ++k) t[k] = s[i + 32 * k];
+#pragma unroll
+    for (int k = 0; k < 8; ++k) d[i + 32 * k] = t[k];
+  }
+}
+
 // copy-on-write of one K page in zero-copy mode: K[priv] = R_delta K[src], one warp (same arithmetic as realign_kernel)
 __device__ __forceinline__ void cow_rotate_page(const uint4 *__restrict__ s, uint4 *__restrict__ d, int num_kv_heads,
                                                 int style, double theta, int delta, int lane) {
   if (style == 0) {
     // items (head, row, c < 8): chunks c and c + 8 of the row; i = lane + 32 k keeps c = lane & 7
     const int c = lane & 7;
+    // the 64 (cos, sin) pairs of the segment: two per lane in fp64, handed round by shuffles (lane needs 8c .. 8c+7)
+    const float2 t0 = rope_cos_sin(theta, delta, 2 * lane), t1 = rope_cos_sin(theta, delta, 2 * lane + 1);
     float2 cs[8];
 #pragma unroll
-    for (int e = 0; e < 8; ++e) cs[e] = rope_cos_sin(theta, delta, 8 * c + e);
-    const int items = num_kv_heads * kPage * 8;
-    for (int i = lane; i < items; i += 32) {
-      const int o = (i >> 3) * 16 + c;
-      uint4 a = s[o], b = s[o + 8];
-      rotate_split(a, b, cs);
-      d[o] = a;
-      d[o + 8] = b;
+    for (int e = 0; e < 8; ++e) {
+      const int src = (8 * c + e) >> 1;
+      const float2 a = make_float2(__shfl_sync(0xffffffffu, t0.x, src), __shfl_sync(0xffffffffu, t0.y, src));
+      const float2 b = make_float2(__shfl_sync(0xffffffffu, t1.x, src), __shfl_sync(0xffffffffu, t1.y, src));
+      cs[e] = (e & 1) ? b : a;
+    }
+    const int items = num_kv_heads * kPage * 8;  // a multiple of 128: four items per lane and step, loads first
+    for (int i = lane; i < items; i += 128) {
+      uint4 a[4], b[4];
+#pragma unroll
+      for (int k = 0; k < 4; ++k) {
+        const int o = ((i + 32 * k) >> 3) * 16 + c;
+        a[k] = s[o];
+        b[k] = s[o + 8];
+      }
+#pragma unroll
+      for (int k = 0; k < 4; ++k) {
+        const int o = ((i + 32 * k) >> 3) * 16 + c;
+        rotate_split(a[k], b[k], cs);
+        d[o] = a[k];
+        d[o + 8] = b[k];
+      }
     }
   } else {
     const int c16 = lane & 15;
+    const float2 t0 = rope_cos_sin(theta, delta, 2 * lane), t1 = rope_cos_sin(theta, delta, 2 * lane + 1);
     float2 cs[4];
 #pragma unroll
-    for (int e = 0; e < 4; ++e) cs[e] = rope_cos_sin(theta, delta, 4 * c16 + e);
-    const int items = num_kv_heads * kPage * 16;
-    for (int i = lane; i < items; i += 32) {
-      uint4 a = s[i];
-      rotate_inter(a, cs);
-      d[i] = a;
+    for (int e = 0; e < 4; ++e) {
+      const int src = (4 * c16 + e) >> 1;
+      const float2 a = make_float2(__shfl_sync(0xffffffffu, t0.x, src), __shfl_sync(0xffffffffu, t0.y, src));
+      const float2 b = make_float2(__shfl_sync(0xffffffffu, t1.x, src), __shfl_sync(0xffffffffu, t1.y, src));
+      cs[e] = (e & 1) ? b : a;
+    }
+    const int items = num_kv_heads * kPage * 16;  // a multiple of 256
+    for (int i = lane; i < items; i += 256) {
+      uint4 a[8];
+#pragma unroll
+      for (int k = 0; k < 8; ++k) a[k] = s[i + 32 * k];
+#pragma unroll
+      for (int k = 0; k < 8; ++k) {
+        rotate_inter(a[k], cs);
+        d[i + 32 * k] = a[k];
+      }
     }
   }
 }
@@ -139,12 +178,10 @@ scatter_kernel(uint4 *pool_k, uint4 *pool_v, int num_kv_heads, int num_reqs, int
       if (kZc && m >= 0)
         cow_rotate_page(s, d, num_kv_heads, zc.style, zc.theta, zc.segs[m].new_pos - zc.segs[m].old_pos, lane);
       else
-        for (int i = lane; i < page_chunks; i += 32) d[i] = s[i];
+        copy_page(s, d, page_chunks, lane);
     }
     if (vb != priv) {
-      const uint4 *s = pool_v + (size_t)vb * page_chunks;
-      uint4 *d = pool_v + (size_t)priv * page_chunks;
-      for (int i = lane; i < page_chunks; i += 32) d[i] = s[i];
+      copy_page(pool_v + (size_t)vb * page_chunks, pool_v + (size_t)priv * page_chunks, page_chunks, lane);
     }
     __syncwarp();  // orders the page copy before the row writes of other lanes below
     if (lane == 0) {
