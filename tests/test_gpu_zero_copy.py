@@ -165,3 +165,60 @@ def test_zero_copy_refusals():
     nocow = sx.DeviceBatch(wl.zero_copy_layout(lay), cow=False)
     with pytest.raises(sx.SparseXError, match="cow_private"):
         sx.scatter_kv(g.pool, nocow, g.kf_sel, g.vf_sel, g.sel_idx, g.sel_off, max_rows=int(g.sel_idx.numel()))
+
+
+@pytest.mark.parametrize("name", ["C4", "C3"])
+def test_zero_copy_fullsize(name):
+    """Zero-copy mode at BASELINE.json's full sizes (C4: 16 requests, 208K context tokens; C3: one 32K request), on
+    the carved inputs of test_gpu_fullsize.py. Scores / S_key / R must equal the copy path's bit for bit (that path is
+    held against the oracle at full size in test_gpu_fullsize.py); attention is compared with the fp64 oracle on
+    the seam-aware row sample; written pages are bit-identical to the copy path's, unwritten ones still shared."""
+    import os
+    from helpers import apply_carve, edge_rows, load_carve
+    GpuLayer, dev_to_bits = _gpu()
+    gold = os.path.join(os.path.dirname(os.path.abspath(__file__)), "golden")
+    lay = wl.CONFIGS[name]()
+    lt = wl.build_layer(lay, 0)
+    apply_carve(lt, load_carve(os.path.join(gold, "carve_%s.txt" % name)))
+    hq, g_sz = lay.num_q_heads, lay.num_q_heads // lay.num_kv_heads
+    g0 = GpuLayer(lay, lt)
+    g0.step_sparse()
+    zlay = wl.zero_copy_layout(lay)
+    g = GpuLayer(zlay, lt)
+    g.step_sparse(do_realign=False)
+    torch.cuda.synchronize()
+    assert np.array_equal(g.scores.cpu().numpy(), g0.scores.cpu().numpy())
+    sel, rows = g.sel_idx.cpu().numpy(), g.rows_R.cpu().numpy()
+    assert np.array_equal(sel, g0.sel_idx.cpu().numpy()) and np.array_equal(rows, g0.rows_R.cpu().numpy())
+    # ---- oracle state after the layer's scatters, attention on sampled rows
+    pk, pv = lt.pool_k.copy(), lt.pool_v.copy()
+    kt, vt = lay.k_block_table.copy(), lay.v_block_table.copy()
+    orc.realign(pk, pv, kt, vt, lay.segments, lay.src_blocks, lay.rope_theta, lay.rope_style)
+    lse = g.lse.cpu().numpy().astype(np.float64)
+    written = np.zeros(lay.k_block_table.shape, dtype=bool)
+    for r in range(lay.num_reqs):
+        t, o = int(lay.seq_len[r]), int(lay.tok_off[r])
+        r0, r1 = g.rows_off_h[r], g.rows_off_h[r + 1]
+        rr = rows[r0:r1]
+        orc.scatter_kv(pk, pv, kt, vt, None, r, rr, lt.k_fresh[o + rr], lt.v_fresh[o + rr])
+        written[r, np.unique(rr // 16)] = True
+        n = 12 if name == "C4" else 256
+        pick = edge_rows(rr, n, 128 // g_sz) if len(rr) > n else np.arange(len(rr))   # a zero-copy CTA owns ONE tile
+        ref_o, ref_l = orc.attention(pk, pv, kt[r], vt[r], t, lt.q_full[o + rr[pick]], rr[pick], hq, want_lse=True)
+        got = orc.bf16_to_f64(dev_to_bits(g.out[r0:r1][torch.from_numpy(pick).to(g.dev)]))
+        check_close("%s zero-copy req %d O (sampled rows)" % (name, r), got, ref_o)
+        assert np.max(np.abs(lse[r0:r1][pick] - ref_l)) < 2e-3
+    # ---- pages and tables
+    gk, gv, gk0 = dev_to_bits(g.pool_k), dev_to_bits(g.pool_v), dev_to_bits(g0.pool_k)
+    gkt = g.batch.k_block_table.cpu().numpy()
+    in_seg = _seg_page_mask(lay)
+    priv = lay.k_block_table
+    assert np.array_equal(gkt[in_seg & written], priv[in_seg & written])
+    assert np.array_equal(gkt[in_seg & ~written], zlay.k_block_table[in_seg & ~written])
+    pages = priv[written]
+    assert np.array_equal(gk[pages], gk0[pages])
+    assert np.array_equal(gv[pages], pv[pages])
+    src = np.concatenate(lay.pool_seg_pages)
+    assert np.array_equal(gk[src], lt.pool_k[src])
+    saved = int((in_seg & ~written).sum())
+    assert saved > 0 and not gk[priv[in_seg & ~written]].any()
