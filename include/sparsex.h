@@ -115,8 +115,8 @@ typedef struct {
  *     for lp is read ROTATED by delta_m (same arithmetic, same bits as sx_rope_realign would have stored);
  *     every other page (fresh, prefix hit, or already made private) is read as stored;
  *   - sx_score_select[_ex] and sx_sparse_attn rotate each K tile in shared memory between its TMA load and the MMA
- *     (attention then works on ONE query tile per CTA, the second softmax warpgroup becomes the rotator; CTA pairs
- *     and the CUDA-core kernels are not available: SX_ERR_UNSUPPORTED);
+ *     (in attention the softmax warpgroups do it; CTA pairs and the CUDA-core kernels are not available:
+ *     SX_ERR_UNSUPPORTED);
  *   - sx_scatter_kv needs batch->cow_private: the first row written to a still-shared page copies it to its private
  *     page -- K rotated on the way, V bit-copied -- and flips the table entries; later calls see a private page;
  *   - sx_rope_realign[_layers] refuses the descriptor (SX_ERR_INVALID_ARG): its destination would be the shared

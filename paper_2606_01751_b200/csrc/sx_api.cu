@@ -384,7 +384,7 @@ sx_status sx_sparse_attn(const sx_pool *pool, const sx_batch *batch, int32_t mod
   const int g = pool->num_q_heads / pool->num_kv_heads;
   const bool allow_small = want_cuda_core;
   if (batch->zero_copy && batch->num_segments > 0) {
-    // K tiles are rotated in shared memory by the second softmax warpgroup: one query tile per CTA, no CTA pairs
+    // K tiles are rotated in shared memory by the softmax warpgroups of the single-CTA kernel: no CTA pairs
     if (want_cuda_core || (mode_flags & SX_ATTN_CTA_PAIR))
       return set_error(SX_ERR_UNSUPPORTED, "zero-copy mode: CUDA-core kernels / CTA pairs are not available");
     st = validate_ws(pool, batch, ws, ws_bytes);
@@ -392,7 +392,9 @@ sx_status sx_sparse_attn(const sx_pool *pool, const sx_batch *batch, int32_t mod
     ZcArgs zc;
     st = zc_prepare(pool, batch, ws, s, &zc);
     if (st != SX_OK) return st;
-    const int splits = attn_pv_splits(pool, batch, total_rows, 1);
+    // two query tiles per CTA fill the machine without key splits -> the shared-rotation form; else one tile per CTA
+    int splits = attn_pv_splits(pool, batch, total_rows, 2);
+    if (splits > 1) splits = attn_pv_splits(pool, batch, total_rows, 1);
     float *part = splits > 1 ? reinterpret_cast<float *>(static_cast<char *>(ws) + ws_layout(pool, batch).attn_part) : nullptr;
     return launch_attn(pool, batch, q, rows_R, rows_off, total_rows, out, lse, splits, part, false, zc, s);
   }
