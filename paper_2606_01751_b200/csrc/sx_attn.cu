@@ -292,9 +292,6 @@ attn_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_constant__ CU
         return (is_v ? p.v_table : p.k_table)[(size_t)req * p.max_pages + lp];
       };
       const uint32_t full0 = kPair ? mapa_u32(smem_u32(&bars->kv_full[0]), 0) : 0;
-#ifdef SX_KV_EVICT_LAST
-      const uint64_t kv_pol = l2_policy_evict_last();
-#endif
       int it = (warp == kWarpProd1) ? 1 : 0;
       int blk = (it < n_items && lane < n_boxes) ? table_entry(it) : 0;
       for (; it < n_items; it += 2) {
@@ -309,19 +306,10 @@ attn_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_constant__ CU
           if (kPair) {
             uint8_t *dst = smem + Cfg::kOffKV + s * kStageBytes +
                            (is_v ? pg_v * 2048 : half_k * (kHalfBytes / 2) + (lane >> 1) * 2048);
-#ifdef SX_KV_EVICT_LAST
-            tma_load_2d_pair_hint(dst, is_v ? &tm_v : &tm_k, full0 + s * 8, (is_v ? half_v : half_k) * 64, row0, kv_pol);
-#else
             tma_load_2d_pair(dst, is_v ? &tm_v : &tm_k, full0 + s * 8, (is_v ? half_v : half_k) * 64, row0);
-#endif
           } else {
-#ifdef SX_KV_EVICT_LAST
-            tma_load_2d_hint(smem + Cfg::kOffKV + s * kTileBytes + half_k * kHalfBytes + pg_k * 2048,
-                             is_v ? &tm_v : &tm_k, &bars->kv_full[s], half_k * 64, row0, kv_pol);
-#else
             tma_load_2d(smem + Cfg::kOffKV + s * kTileBytes + half_k * kHalfBytes + pg_k * 2048,
                         is_v ? &tm_v : &tm_k, &bars->kv_full[s], half_k * 64, row0);
-#endif
           }
         }
         blk = blk_next;
