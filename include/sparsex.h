@@ -245,7 +245,8 @@ sx_status sx_sparse_attn(const sx_pool *pool, const sx_batch *batch, int32_t mod
  * seq_len / tok_off / new_off consistent with the host counts; new_idx strictly ascending inside its request;
  * every segment's len / old_pos / new_pos a positive multiple of block_size, src_off the running
  * sum of len / block_size, segments sorted by (req, new_pos) and non-overlapping, inside the request's pages;
- * src_blocks, the block-table entries of used pages and cow_private inside the pool. One small kernel, one error
+ * src_blocks, the block-table entries of used pages and cow_private inside the pool; every table entry that still is
+ * its segment's shared source page (copy-on-write V, zero-copy K and V) has a reserved private page. One small kernel, one error
  * word copied back: this call SYNCHRONISES `stream`. Returns SX_OK or SX_ERR_INVALID_ARG with the failing check
  * and its index in sx_last_error(). A descriptor that fails here would corrupt pages in the stage calls. Uses ws. */
 sx_status sx_check_batch(const sx_pool *pool, const sx_batch *batch, void *ws, size_t ws_bytes, sx_stream stream);

@@ -11,7 +11,7 @@ namespace sx {
 // first failing check wins: the error word is min over (check id << 32 | index)
 enum CheckId : int {
   kChkSeqLen = 1, kChkTokOff, kChkNewOff, kChkNewIdx, kChkSegReq, kChkSegAlign, kChkSegRange, kChkSegSrcOff,
-  kChkSegOrder, kChkSegPages, kChkSrcBlock, kChkKTable, kChkVTable, kChkCow, kChkRowsOff, kChkRows
+  kChkSegOrder, kChkSegPages, kChkSrcBlock, kChkKTable, kChkVTable, kChkCow, kChkShared, kChkRowsOff, kChkRows
 };
 
 static const char *check_text(int id) {
@@ -30,6 +30,8 @@ static const char *check_text(int id) {
     case kChkKTable: return "k_block_table entry of a used page outside [0, num_blocks)";
     case kChkVTable: return "v_block_table entry of a used page outside [0, num_blocks)";
     case kChkCow: return "cow_private entry outside [-1, num_blocks)";
+    case kChkShared:
+      return "a table entry that still is its segment's shared source page has no reserved private page (cow_private)";
     case kChkRowsOff: return "rows_off not ascending from 0, or rows_off[num_reqs] > max_rows";
     case kChkRows: return "row list not strictly ascending inside [0, seq_len) of its request";
   }
@@ -89,6 +91,21 @@ check_batch_kernel(sx_batch b, int num_blocks, unsigned long long *err) {
   for (int i = tid; i < b.total_seg_pages; i += nth) {
     const int blk = b.src_blocks[i];
     if (blk < 0 || blk >= num_blocks) fail(err, kChkSrcBlock, i);
+    // copy-on-write / zero-copy: an entry that still aliases the shared page must have somewhere to go when written
+    int lo = 0, hi = b.num_segments - 1;
+    while (lo < hi) {
+      const int mid = (lo + hi + 1) >> 1;
+      if (b.segments[mid].src_off <= i) lo = mid; else hi = mid - 1;
+    }
+    const sx_segment s = b.segments[lo];
+    const int lp = s.new_pos / kPage + (i - s.src_off);
+    if (s.req >= 0 && s.req < b.num_reqs && s.new_pos >= 0 && i >= s.src_off && lp < b.max_pages_per_req) {
+      const size_t e = (size_t)s.req * b.max_pages_per_req + lp;
+      if (b.k_block_table[e] == blk || b.v_block_table[e] == blk) {
+        const int cp = b.cow_private ? b.cow_private[e] : -1;
+        if (cp < 0 || cp == blk) fail(err, kChkShared, i);
+      }
+    }
   }
   const int entries = b.num_reqs * b.max_pages_per_req;
   for (int i = tid; i < entries; i += nth) {

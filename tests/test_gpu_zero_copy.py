@@ -222,3 +222,30 @@ def test_zero_copy_fullsize(name):
     assert np.array_equal(gk[src], lt.pool_k[src])
     saved = int((in_seg & ~written).sum())
     assert saved > 0 and not gk[priv[in_seg & ~written]].any()
+
+
+def test_check_batch_wants_a_private_page_behind_every_shared_entry():
+    """sx_check_batch: a table entry that still is its segment's shared source page (zero-copy K / V, copy-on-write V)
+    must have a reserved private page, or the first scatter into it would write the shared cache."""
+    import dataclasses
+    from paper_2606_01751_b200 import binding as sx
+    GpuLayer, _ = _gpu()
+    lay, lt = prepared("tiny")[:2]
+    z = wl.zero_copy_layout(lay)
+    g = GpuLayer(z, lt)
+    sx.check_batch(g.pool, g.batch)                       # a good zero-copy descriptor passes
+    _req, _ln, _old, new, so = (int(v) for v in lay.segments[1])
+    cowp = z.cow_private.copy()
+    cowp[_req, new // 16 + 1] = -1                        # no private page behind a shared entry
+    gb = GpuLayer(dataclasses.replace(z, cow_private=cowp), lt)
+    with pytest.raises(sx.SparseXError, match="reserved private page"):
+        sx.check_batch(gb.pool, gb.batch)
+    cowp = z.cow_private.copy()
+    cowp[_req, new // 16] = int(lay.src_blocks[so])       # "private" page IS the shared page
+    gb = GpuLayer(dataclasses.replace(z, cow_private=cowp), lt)
+    with pytest.raises(sx.SparseXError, match="reserved private page"):
+        sx.check_batch(gb.pool, gb.batch)
+    # the copy-on-write layout of round 1 (V aliases, K private) and the plain layout still pass
+    for other in (wl.config_tiny(seed_id=14, cow=True), lay):
+        go = GpuLayer(other, wl.build_layer(other, 0))
+        sx.check_batch(go.pool, go.batch)
