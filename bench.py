@@ -369,6 +369,13 @@ def measure(cfg, steps, warmup, ctx, want_e2e=True, want_clocks=True):
     if "select" in stage_ms:
         sel_fl = select_flops(lay, hq, 1 if stack else 2)
         hbm["select_tflops"] = round(sel_fl / (stage_ms["select"] * 1e-3) / 1e12, 1)
+        # stage (b) is bound by the exponentials (one per 256 flop), not by the tensor pipe: hold it against the
+        # measured rate of its own MUFU / FMA-pipe mix (sx_probe_pipe), whole stage time (top-k included)
+        pr = ctx.get("pipe_rates")
+        if pr:
+            exps = sel_fl / 256.0
+            hbm["select_gexp_per_s"] = round(exps / (stage_ms["select"] * 1e-3) / 1e9, 1)
+            hbm["select_alu_frac"] = round(exps / (stage_ms["select"] * 1e-3) / (pr["sweep_mix_gexp_per_s"] * 1e9), 4)
 
     # launch-bound single-layer configs: the same step replayed from a CUDA graph (no host launch gaps)
     graph_ms = None
@@ -477,6 +484,30 @@ def measure_s6(ctx, reps=10):
     return out
 
 
+def measure_pipes(ctx):
+    """Instruction-pipe rates of this GPU (sx_probe_pipe): lane-operations per clock and SM and, with the clock the
+    probe itself ran at, per second for the whole GPU. `sweep_mix` = the scoring sweeps' exponential mix (6 of 8 on
+    MUFU.EX2, 2 of 8 by the FMA-pipe polynomial): the roofline of stage (b) (`select_alu_frac`)."""
+    torch, sx, dev = ctx["torch"], ctx["sx"], ctx["dev"]
+    n_sm = torch.cuda.get_device_properties(dev).multi_processor_count
+    out = {"sms": n_sm}
+    iters = 8192
+    for name, pipe in (("mufu_ex2", 0), ("ffma", 1), ("ffma2", 2), ("sweep_mix", 3)):
+        per_clk = sx.probe_pipe(pipe, iters=iters, device=dev)
+        cyc = torch.zeros(n_sm + 1, dtype=torch.int64, device=dev)
+        a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        a.record()
+        sx.load().sx_probe_pipe(pipe, iters, cyc.data_ptr(), n_sm, None)
+        b.record()
+        torch.cuda.synchronize()
+        ms = a.elapsed_time(b)
+        out[name + "_per_clk_sm"] = round(per_clk, 2)
+        out[name + "_gexp_per_s" if pipe in (0, 3) else name + "_gops_per_s"] = round(
+            1024.0 * 8 * iters * n_sm / (ms * 1e-3) / 1e9, 1)
+        out[name + "_sm_mhz"] = round(float(cyc[:n_sm].median().item()) / (ms * 1e-3) / 1e6, 0)
+    return out
+
+
 def measure_zero_copy(ctx, reps=10):
     """Zero-copy mode (include/sparsex.h; S9 NEXT-3) against the copy path, same inputs, same stages:
       (i)  one sparse C4 layer (16 requests, two-sweep selection), every stage timed between events;
@@ -579,6 +610,8 @@ def run_ours(args):
     ctx = {"torch": torch, "sx": sx, "du": du, "dev": dev, "local": local, "rank": rank, "world": world,
            "peaks": load_peaks(), "args": args}
     cfg = args.config
+    if world == 1:
+        ctx["pipe_rates"] = measure_pipes(ctx)
     if cfg == "S6":   # supplementary: stage (c) alone on small row sets (HBM regime); not the headline metric
         if rank == 0:
             print(json.dumps({"metric": "small_row_attention_hbm", "unit": "GB/s", "n_gpus": 1, "dtype": "bf16",
@@ -645,6 +678,8 @@ def run_ours(args):
                    "recomputed_tokens_per_s": round(world * m["rows_R"] * m["n_sparse"] / (m["ms_per_step"] * 1e-3), 1)},
         "clocks": m["clocks"], "e2e": m["e2e"], "gpu_launches": m["launches"], "roofline": m["roofline"],
     }
+    if "pipe_rates" in ctx:
+        line["config"]["pipe_rates"] = ctx["pipe_rates"]
     if others:
         line["config"]["other_configs"] = others
     if world == 1 and not args.no_cpu:

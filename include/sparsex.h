@@ -260,6 +260,15 @@ sx_status sx_check_rows(const sx_pool *pool, const sx_batch *batch, const int32_
 /* Number of kernels this library has launched in the process so far (diagnostic; monotone, thread safe). */
 uint64_t sx_launch_count(void);
 
+/* Diagnostic, not part of the method: instruction-pipe rate probe, the denominator of the roofline of the scoring
+ * sweeps (one exponential per 256 flop: bound by the special-function pipe). Launches num_ctas CTAs of 1024 threads,
+ * each running 8 * iters dependent-chain operations per thread on ONE pipe, and writes the clock64() cycles of every
+ * CTA's loop to cycles[0 .. num_ctas) (device, uint64; one more word behind them is scratch):
+ *   pipe 0 = MUFU.EX2, 1 = FFMA, 2 = FFMA2 (two fused multiply-adds per lane), 3 = the sweeps' mix (of every 8
+ *   exponentials 6 on MUFU.EX2 and 2 by the FMA-pipe polynomial).
+ * Lane-operations per clock and SM = 1024 * 8 * iters / cycles with one CTA per SM. Asynchronous on `stream`. */
+sx_status sx_probe_pipe(int32_t pipe, int32_t iters, uint64_t *cycles, int32_t num_ctas, sx_stream stream);
+
 /* Thread-local text of the last error returned on this thread ("" if none). Static storage. */
 const char *sx_last_error(void);
 

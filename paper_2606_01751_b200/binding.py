@@ -25,7 +25,7 @@ _lib = None
 SX_OK = 0
 EXPORTS = ["sx_workspace_size", "sx_rope_realign", "sx_rope_realign_layers", "sx_scatter_kv", "sx_score_select",
            "sx_score_select_ex", "sx_sparse_attn", "sx_check_batch", "sx_check_rows", "sx_launch_count",
-           "sx_last_error", "sx_version"]
+           "sx_probe_pipe", "sx_last_error", "sx_version"]
 
 
 class SxPool(ctypes.Structure):
@@ -84,6 +84,8 @@ def load():
         lib.sx_check_rows.argtypes = [PP, PB, vp, vp, i32, vp, sz, vp]
         lib.sx_launch_count.restype = ctypes.c_uint64
         lib.sx_launch_count.argtypes = []
+        lib.sx_probe_pipe.restype = ctypes.c_int
+        lib.sx_probe_pipe.argtypes = [i32, i32, vp, i32, vp]
         lib.sx_last_error.restype = ctypes.c_char_p
         lib.sx_version.restype = ctypes.c_char_p
         _lib = lib
@@ -97,6 +99,18 @@ def version() -> str:
 def launch_count() -> int:
     """Kernels the library has launched in this process so far (counted inside libsparsex.so)."""
     return int(load().sx_launch_count())
+
+
+def probe_pipe(pipe: int, iters: int = 4096, num_ctas: Optional[int] = None, device="cuda", stream=None) -> float:
+    """sx_probe_pipe: lane-operations per clock and SM of one instruction pipe (0 MUFU.EX2, 1 FFMA, 2 FFMA2,
+    3 the scoring sweeps' 6:2 MUFU / polynomial mix); median over one CTA per SM."""
+    dev = torch.device(device)
+    n = int(num_ctas) if num_ctas else torch.cuda.get_device_properties(dev).multi_processor_count
+    cyc = torch.zeros(n + 1, dtype=torch.int64, device=dev)
+    for _ in range(2):   # the first launch warms the clocks up
+        _check(load().sx_probe_pipe(int(pipe), int(iters), _ptr(cyc), n, _stream(stream)), "sx_probe_pipe")
+    torch.cuda.synchronize(dev)
+    return 1024.0 * 8.0 * iters / float(cyc[:n].median().item())
 
 
 def _check(rc: int, what: str):

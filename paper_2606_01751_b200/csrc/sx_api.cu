@@ -224,6 +224,12 @@ const char *sx_version(void) { return "sparsex-b200 0.3 (sm_100a; tcgen05/TMEM/T
 
 uint64_t sx_launch_count(void) { return g_launches.load(std::memory_order_relaxed); }
 
+sx_status sx_probe_pipe(int32_t pipe, int32_t iters, uint64_t *cycles, int32_t num_ctas, sx_stream stream) {
+  if (!cycles || iters <= 0 || num_ctas <= 0) return set_error(SX_ERR_INVALID_ARG, "probe: bad arguments");
+  return launch_probe(pipe, iters, reinterpret_cast<unsigned long long *>(cycles), num_ctas,
+                      reinterpret_cast<cudaStream_t>(stream));
+}
+
 sx_status sx_check_batch(const sx_pool *pool, const sx_batch *batch, void *ws, size_t ws_bytes, sx_stream stream) {
   sx_status st = validate(pool, batch);
   if (st != SX_OK) return st;

@@ -78,6 +78,9 @@ sx_status run_check_batch(const sx_pool *pool, const sx_batch *b, void *ws, cuda
 sx_status run_check_rows(const sx_batch *b, const int32_t *rows, const int32_t *rows_off, int32_t max_rows, void *ws,
                          cudaStream_t st);
 
+// instruction-pipe rate probe (sx_probe.cu)
+sx_status launch_probe(int pipe, int iters, unsigned long long *cycles, int num_ctas, cudaStream_t st);
+
 // TMA descriptor construction (driver entry point fetched through the runtime; no libcuda link)
 sx_status make_tmap_pool(CUtensorMap *out, const void *base, int num_blocks, int num_kv_heads);
 sx_status make_tmap_q(CUtensorMap *out, const void *base, int total_rows, int num_q_heads, int group,

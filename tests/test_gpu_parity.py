@@ -621,3 +621,17 @@ def test_key_split_path_under_cuda_graph_replay():
     sx.sparse_attn(g.pool, g.batch, q, out, rows_R=rows, rows_off=off, total_rows=6)   # and eager again afterwards
     torch.cuda.synchronize()
     assert torch.equal(out, eager)
+
+
+def test_pipe_probe_reports_plausible_rates():
+    """sx_probe_pipe (diagnostic; the denominator of stage (b)'s roofline in bench.py): MUFU.EX2 retires 16 lane-ops
+    per clock and SM on sm_100, FFMA about 128; the probe must land near both on any healthy B200."""
+    from paper_2606_01751_b200 import binding as sx
+    mufu = sx.probe_pipe(0, iters=2048)
+    ffma = sx.probe_pipe(1, iters=2048)
+    mix = sx.probe_pipe(3, iters=2048)
+    assert 14.0 < mufu < 16.5, mufu
+    assert 100.0 < ffma < 130.0, ffma
+    assert mufu < mix < 2.0 * mufu, (mufu, mix)          # the polynomial share adds to what MUFU alone retires
+    with pytest.raises(sx.SparseXError):
+        sx.probe_pipe(9)
