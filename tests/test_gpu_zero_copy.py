@@ -249,3 +249,77 @@ def test_check_batch_wants_a_private_page_behind_every_shared_entry():
     for other in (wl.config_tiny(seed_id=14, cow=True), lay):
         go = GpuLayer(other, wl.build_layer(other, 0))
         sx.check_batch(go.pool, go.batch)
+
+
+@pytest.mark.parametrize("ov,tail,prefix", [(1, 64, 0), (2, 16, 16)])
+def test_zero_copy_extended_selection_and_cuda_graph(ov, tail, prefix):
+    """sx_score_select_ex (overflow + tail fallback: a data-dependent row list whose rows sit on page boundaries of
+    reused segments) and the stages after it in zero-copy mode, against the copy path on the same inputs: same
+    S_key and R bit for bit, same written pages, outputs within a few bf16 ulps of each other (the two modes cut the
+    attention into different CTAs). Then the whole zero-copy layer once more from a CUDA graph: same results."""
+    from helpers import carve_margins
+    from paper_2606_01751_b200 import binding as sx
+    GpuLayer, dev_to_bits = _gpu()
+    lay = wl.config_tail(prefix=prefix)
+    lt = wl.build_layer(lay, 0)
+    carve_margins(lay, lt)
+
+    def layer(g, realign):
+        if realign:
+            g.realign()
+        g.scatter_new()
+        g.select_ex(overflow_blocks=ov, tail_tokens=tail)
+        g.stage_rows(g.sel_idx, g.rows_R)
+        sx.scatter_kv(g.pool, g.batch, g.kf_R, g.vf_R, g.rows_R, g.rows_off, max_rows=g.rows_cap)
+        g.attend()
+        torch.cuda.synchronize()
+    g0 = GpuLayer(lay, lt)
+    layer(g0, True)
+    zlay = wl.zero_copy_layout(lay)
+    g = GpuLayer(zlay, lt)
+    layer(g, False)
+    assert np.array_equal(g.scores.cpu().numpy(), g0.scores.cpu().numpy())
+    assert np.array_equal(g.sel_idx.cpu().numpy(), g0.sel_idx.cpu().numpy())
+    assert np.array_equal(g.rows_R.cpu().numpy(), g0.rows_R.cpu().numpy())
+    a, b = orc.bf16_to_f64(dev_to_bits(g.out)), orc.bf16_to_f64(dev_to_bits(g0.out))
+    assert np.max(np.abs(a - b)) < 2e-2 and np.mean(np.abs(a - b)) < 5e-4
+    rows, off = g.rows_R.cpu().numpy(), g.rows_off_h
+    gk, gk0 = dev_to_bits(g.pool_k), dev_to_bits(g0.pool_k)
+    for r in range(lay.num_reqs):
+        pages = lay.k_block_table[r, np.unique(rows[off[r]:off[r + 1]] // 16)]
+        assert np.array_equal(gk[pages], gk0[pages])
+    # ---- the same zero-copy stages replayed from a CUDA graph (tables reset first: the scatter flips them)
+    out_eager, lse_eager = g.out.clone(), g.lse.clone()
+    kt0 = torch.from_numpy(zlay.k_block_table).to(g.dev)
+    g.batch.k_block_table.copy_(kt0)
+    g.batch.v_block_table.copy_(kt0)
+    g.pool_k.copy_(torch.from_numpy(lt.pool_k.view(np.int16)))
+    g.pool_v.copy_(torch.from_numpy(lt.pool_v.view(np.int16)))
+    g.scatter_new()
+    cap = torch.from_numpy(sx.rows_capacity(lay, ov, tail)).to(g.dev)
+    sel = torch.full_like(g.sel_idx, -1)
+    rows_d = torch.full((g.rows_cap,), -1, dtype=torch.int32, device=g.dev)
+    off_out = torch.zeros(lay.num_reqs + 1, dtype=torch.int32, device=g.dev)
+    torch.cuda.synchronize()
+
+    def stages():
+        sx.score_select_ex(g.pool, g.batch, g.q_new, g.sel_off, cap, sel, rows_d, off_out, overflow_blocks=ov,
+                           tail_tokens=tail)
+        sx.scatter_kv(g.pool, g.batch, g.kf_R, g.vf_R, rows_d, off_out, max_rows=g.rows_cap)
+        sx.sparse_attn(g.pool, g.batch, g.q_R, g.out, rows_R=rows_d, rows_off=off_out, total_rows=int(g.out.shape[0]),
+                       lse=g.lse)
+
+    def reset():
+        g.batch.k_block_table.copy_(kt0)
+        g.batch.v_block_table.copy_(kt0)
+        g.out.zero_()
+        torch.cuda.synchronize()
+    graph = torch.cuda.CUDAGraph()
+    with torch.cuda.graph(graph):
+        stages()
+    for _ in range(2):
+        reset()
+        graph.replay()
+        torch.cuda.synchronize()
+        assert torch.equal(g.out, out_eager) and torch.equal(g.lse, lse_eager)
+        assert np.array_equal(rows_d[:len(rows)].cpu().numpy(), rows)
