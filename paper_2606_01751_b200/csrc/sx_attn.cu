@@ -431,7 +431,10 @@ attn_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_constant__ CU
     const int n_local = row / g, hh = row - n_local * g;
     const bool valid = n_local < (qt ? nrows[1] : nrows[0]);
     const int grow = row_base + qt * rpt + n_local;  // batch-wide row index
-    const int pos = valid ? (p.rows ? p.rows[grow] : grow - p.rows_off[req]) : 0;
+    // rows without a query (pad rows when g does not divide 128, the tail of a request's last tile) are treated as
+    // seeing every key: their S is finite and their O is never stored, but with position 0 they would drag their
+    // whole warp through the masking path on every tile after the first
+    const int pos = valid ? (p.rows ? p.rows[grow] : grow - p.rows_off[req]) : 0x3fffffff;
     const uint32_t lane_addr = (uint32_t)(quarter * 32) << 16;
     const uint32_t tmem_s = tmem + lane_addr + qt * 128;
     const uint32_t tmem_o = tmem + lane_addr + 256 + qt * 128;

@@ -190,7 +190,10 @@ lse_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_constant__ CUt
     const int row = quarter * 32 + lane;  // (query, head) row = TMEM lane
     const int n_local = row / g, hh = row - n_local * g;
     const bool valid = n_local < n_rows;
-    const int pos = valid ? p.new_idx[row_base + n_local] : -1;
+    // rows without a query (pad rows when g does not divide 128, the tail of a request's last tile) are treated as
+    // seeing every key: their S is finite (zero or another request's Q rows) and their result is never stored, but
+    // with position -1 they would drag their whole warp through the masking path on every tile
+    const int pos = valid ? p.new_idx[row_base + n_local] : 0x3fffffff;
     const uint32_t lane_addr = (uint32_t)(quarter * 32) << 16;
     float m = -INFINITY, l = 0.f;  // running maximum (log2 domain) and sum of this thread's key columns
     auto rotate_tile = [&](int t) {
