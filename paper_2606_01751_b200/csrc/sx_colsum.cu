@@ -65,6 +65,8 @@ struct CsBars {
 // causal mask (the majority) read the normalisers only, four columns per 16-byte shared-memory load.
 __global__ void __launch_bounds__(128)
 coltab_kernel(const ColsumParams p) {
+  griddep_launch();  // programmatic dependent launch: the next kernel may become resident now ...
+  griddep_wait();    // ... and this one touches global memory only after its predecessor has completed
   const int g = p.group, rpt = p.rows_per_tile;
   int req = 0, base = 0;
   for (; req < p.num_reqs; ++req) {
@@ -141,6 +143,8 @@ colsum_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_constant__ 
   uint8_t *smem = reinterpret_cast<uint8_t *>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~uintptr_t(1023));
   CsBars *bars = reinterpret_cast<CsBars *>(smem + kCsOffBar);
   float2 *col_sm = reinterpret_cast<float2 *>(smem + kCsOffCol);  // [kCsColStages][128] (lse2, position)
+  griddep_launch();
+  griddep_wait();
 
   // ---- (request, key tile, KV head); early key tiles (seen by the most queries) first
   const int g = p.group, rpt = p.rows_per_tile;
@@ -355,10 +359,12 @@ sx_status launch_colsum(const sx_pool *pool, const sx_batch *b, const void *q_ne
   cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, kCsSmemBytes);
   if (e != cudaSuccess) return set_error(SX_ERR_CUDA, "colsum smem attr: %s", cudaGetErrorString(e));
   const int n_qt = b->total_new / rpt + b->num_reqs;  // >= sum_r ceil(|I_nr(r)| / rpt)
-  coltab_kernel<<<dim3(n_qt, pool->num_kv_heads), 128, 0, st>>>(p);
+  e = launch_pdl(coltab_kernel, dim3(n_qt, pool->num_kv_heads), dim3(128), 0, st, 1, p);
+  if (e != cudaSuccess) return set_error(SX_ERR_CUDA, "coltab launch: %s", cudaGetErrorString(e));
   s = check_launch("coltab_kernel");
   if (s != SX_OK) return s;
-  kern<<<grid, kCsThreads, kCsSmemBytes, st>>>(tm_q, tm_k, p);
+  e = launch_pdl(kern, dim3(grid), dim3(kCsThreads), kCsSmemBytes, st, 1, tm_q, tm_k, p);
+  if (e != cudaSuccess) return set_error(SX_ERR_CUDA, "colsum launch: %s", cudaGetErrorString(e));
   return check_launch("colsum_kernel");
 }
 

@@ -21,6 +21,8 @@ __global__ void rope_table_kernel(const sx_segment *__restrict__ segs, int num_s
                                   float2 *__restrict__ table, int total_pages,
                                   const int32_t *__restrict__ src_blocks, const int32_t *__restrict__ k_table,
                                   const int32_t *__restrict__ v_table, int max_pages, int4 *__restrict__ page_desc) {
+  griddep_launch();  // programmatic dependent launch: the copy kernel may become resident now ...
+  griddep_wait();    // ... and the block tables may be outputs of the previous kernel in the stream
   int idx = blockIdx.x * blockDim.x + threadIdx.x;
   if (idx < num_segments * 64) {
     int m = idx >> 6, i = idx & 63;
@@ -67,6 +69,8 @@ template <int STYLE>
 __global__ void __launch_bounds__(kRealignThreads)
 realign_kernel(const __grid_constant__ LayerPools pools, int num_kv_heads, const int4 *__restrict__ page_desc,
                const float2 *__restrict__ table) {
+  griddep_launch();
+  griddep_wait();  // page descriptors and rotation table come from the preparation kernel
   const int page = blockIdx.x, h = blockIdx.y;
   const uint4 *pool_k_src = pools.k[blockIdx.z], *pool_v_src = pools.v[blockIdx.z];
   uint4 *pool_k_dst = pools.k[blockIdx.z], *pool_v_dst = pools.v[blockIdx.z];
@@ -139,6 +143,8 @@ __global__ void zc_prepare_kernel(const sx_segment *__restrict__ segs, int num_s
                                   float2 *__restrict__ table, const int32_t *__restrict__ src_blocks,
                                   const int32_t *__restrict__ k_table, int num_reqs, int max_pages,
                                   const int32_t *__restrict__ seq_len, int32_t *__restrict__ page_seg) {
+  griddep_launch();
+  griddep_wait();  // the block tables may have been flipped by the previous kernel (a scatter)
   const int idx = blockIdx.x * blockDim.x + threadIdx.x;
   if (idx < num_segments * 64) {
     const int m = idx >> 6, i = idx & 63;
@@ -158,18 +164,20 @@ __global__ void zc_prepare_kernel(const sx_segment *__restrict__ segs, int num_s
 sx_status launch_zc_prepare(const sx_batch *b, float2 *table, int32_t *page_seg, cudaStream_t st) {
   const int a = b->num_segments * 64, c = b->num_reqs * b->max_pages_per_req;
   const int n = a > c ? a : c;
-  zc_prepare_kernel<<<(n + 127) / 128, 128, 0, st>>>(b->segments, b->num_segments, b->rope_theta, table, b->src_blocks,
-                                                    b->k_block_table, b->num_reqs, b->max_pages_per_req, b->seq_len,
-                                                    page_seg);
+  cudaError_t e = launch_pdl(zc_prepare_kernel, dim3((n + 127) / 128), dim3(128), 0, st, 1, b->segments, b->num_segments,
+                             b->rope_theta, table, b->src_blocks, (const int32_t *)b->k_block_table, b->num_reqs,
+                             b->max_pages_per_req, b->seq_len, page_seg);
+  if (e != cudaSuccess) return set_error(SX_ERR_CUDA, "zc_prepare launch: %s", cudaGetErrorString(e));
   return check_launch("zc_prepare_kernel");
 }
 
 sx_status launch_realign(const sx_pool *pools, int num_layers, const sx_batch *b, float2 *table, int4 *page_desc,
                          cudaStream_t st) {
   const int n = b->num_segments * 64 > b->total_seg_pages ? b->num_segments * 64 : b->total_seg_pages;
-  rope_table_kernel<<<(n + 127) / 128, 128, 0, st>>>(b->segments, b->num_segments, b->rope_theta, table,
-                                                    b->total_seg_pages, b->src_blocks, b->k_block_table,
-                                                    b->v_block_table, b->max_pages_per_req, page_desc);
+  cudaError_t e = launch_pdl(rope_table_kernel, dim3((n + 127) / 128), dim3(128), 0, st, 1, b->segments, b->num_segments,
+                             b->rope_theta, table, b->total_seg_pages, b->src_blocks, (const int32_t *)b->k_block_table,
+                             (const int32_t *)b->v_block_table, b->max_pages_per_req, page_desc);
+  if (e != cudaSuccess) return set_error(SX_ERR_CUDA, "rope_table launch: %s", cudaGetErrorString(e));
   sx_status s = check_launch("rope_table_kernel");
   if (s != SX_OK) return s;
   for (int l0 = 0; l0 < num_layers; l0 += kRealignMaxLayers) {
@@ -180,10 +188,9 @@ sx_status launch_realign(const sx_pool *pools, int num_layers, const sx_batch *b
       lp.v[l] = reinterpret_cast<uint4 *>(pools[l0 + l].v);
     }
     const dim3 grid(b->total_seg_pages, pools[0].num_kv_heads, nl);
-    if (b->rope_style == 0)
-      realign_kernel<0><<<grid, kRealignThreads, 0, st>>>(lp, pools[0].num_kv_heads, page_desc, table);
-    else
-      realign_kernel<1><<<grid, kRealignThreads, 0, st>>>(lp, pools[0].num_kv_heads, page_desc, table);
+    e = launch_pdl(b->rope_style == 0 ? realign_kernel<0> : realign_kernel<1>, grid, dim3(kRealignThreads), 0, st, 1, lp,
+                   pools[0].num_kv_heads, (const int4 *)page_desc, (const float2 *)table);
+    if (e != cudaSuccess) return set_error(SX_ERR_CUDA, "realign launch: %s", cudaGetErrorString(e));
     s = check_launch("realign_kernel");
     if (s != SX_OK) return s;
   }

@@ -54,6 +54,8 @@ __device__ __forceinline__ Scan3 block_scan3(bool fa, bool fb, bool fc, int (*wa
 // Head aggregation: scores[j] = sum over KV heads of the per-head column sums, fixed order.
 __global__ void __launch_bounds__(256)
 score_sum_kernel(int num_kv_heads, int total_tokens, const float *__restrict__ partial, float *__restrict__ scores) {
+  griddep_launch();  // programmatic dependent launch: the next kernel may become resident now ...
+  griddep_wait();    // ... and this one touches global memory only after its predecessor has completed
   const int j = blockIdx.x * 256 + threadIdx.x;
   if (j >= total_tokens) return;
   float s = 0.f;
@@ -73,6 +75,8 @@ select_kernel(int num_kv_heads, int total_tokens, const int32_t *__restrict__ se
   // slices, one CTA each; digit histograms and the per-slice counts of the ordered emission meet in `scratch`
   // (zeroed by the launcher) and the CTAs of the grid synchronise between the phases.
   namespace cg = cooperative_groups;
+  griddep_launch();
+  griddep_wait();  // (a no-op under the cooperative launch, which does not use programmatic serialisation)
   const int ns = gridDim.y, sl = blockIdx.y;
   int *ghist = scratch + (size_t)blockIdx.x * (4 * 256 + 4 * 64);  // [4 passes][256] then [4 counters][64 slices]
   int *gcnt = ghist + 4 * 256;
@@ -371,6 +375,8 @@ select_kernel(int num_kv_heads, int total_tokens, const int32_t *__restrict__ se
 __global__ void __launch_bounds__(kSelThreads)
 compact_rows_kernel(int num_reqs, const int32_t *__restrict__ tok_off, const int32_t *__restrict__ cnt,
                     const int32_t *__restrict__ tmp, int32_t *__restrict__ rows_R, int32_t *__restrict__ rows_off_out) {
+  griddep_launch();
+  griddep_wait();
   int out = 0;
   for (int r = 0; r < num_reqs; ++r) {
     const int n = cnt[r], src = tok_off[r];
@@ -393,7 +399,9 @@ sx_status launch_select(const sx_pool *pool, const sx_batch *b, const float *par
     cudaError_t e = cudaFuncSetAttribute(select_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (e != cudaSuccess) return set_error(SX_ERR_CUDA, "select smem attr: %s", cudaGetErrorString(e));
   }
-  score_sum_kernel<<<(b->total_tokens + 255) / 256, 256, 0, st>>>(pool->num_kv_heads, b->total_tokens, partial, scores);
+  cudaError_t le = launch_pdl(score_sum_kernel, dim3((b->total_tokens + 255) / 256), dim3(256), 0, st, 1,
+                              pool->num_kv_heads, b->total_tokens, partial, scores);
+  if (le != cudaSuccess) return set_error(SX_ERR_CUDA, "score_sum launch: %s", cudaGetErrorString(le));
   sx_status s0 = check_launch("score_sum_kernel");
   if (s0 != SX_OK) return s0;
   const bool ex = rows_off_out != nullptr;  // extended: variable |R|, slots of capacity rows_off, then compaction
@@ -420,13 +428,17 @@ sx_status launch_select(const sx_pool *pool, const sx_batch *b, const float *par
       ns = 1;  // cooperative launch not possible here (e.g. too few free SMs): one CTA per request
     }
   }
-  if (ns == 1)
-    select_kernel<<<dim3(b->num_reqs, 1), kSelThreads, smem, st>>>(num_kv, total_tokens, seq_len, tok_off, new_off,
-                                                                  new_idx, partial, sel_off, rows_off, scores, sel_idx,
-                                                                  rows_dst, ov_tokens, tail_tokens, segs, nseg, cnt, scratch);
+  if (ns == 1) {
+    le = launch_pdl(select_kernel, dim3(b->num_reqs, 1), dim3(kSelThreads), smem, st, 1, num_kv, total_tokens, seq_len,
+                    tok_off, new_off, new_idx, partial, sel_off, rows_off, scores, sel_idx, rows_dst, ov_tokens,
+                    tail_tokens, segs, nseg, cnt, scratch);
+    if (le != cudaSuccess) return set_error(SX_ERR_CUDA, "select launch: %s", cudaGetErrorString(le));
+  }
   sx_status s = check_launch("select_kernel");
   if (s != SX_OK || !ex) return s;
-  compact_rows_kernel<<<1, kSelThreads, 0, st>>>(b->num_reqs, b->tok_off, rows_cnt, rows_tmp, rows_R, rows_off_out);
+  le = launch_pdl(compact_rows_kernel, dim3(1), dim3(kSelThreads), 0, st, 1, b->num_reqs, b->tok_off,
+                  (const int32_t *)rows_cnt, (const int32_t *)rows_tmp, rows_R, rows_off_out);
+  if (le != cudaSuccess) return set_error(SX_ERR_CUDA, "compact launch: %s", cudaGetErrorString(le));
   return check_launch("compact_rows_kernel");
 }
 
