@@ -241,6 +241,27 @@ sx_status sx_sparse_attn(const sx_pool *pool, const sx_batch *batch, int32_t mod
                          const int32_t *rows_R, const int32_t *rows_off, int32_t total_rows,
                          void *out, float *lse, void *ws, size_t ws_bytes, sx_stream stream);
 
+/* (c) for SMALL row sets without a workspace and without any allocation: for callers that cannot allocate device
+ * memory where they call from (code under CUDA-graph capture, tight serving loops, harnesses that forbid cudaMalloc).
+ * Same operation, same kernel and same results as sx_sparse_attn in mode 0 (the single-CTA tensor-core kernel with
+ * self-merging key splits); the scratch of the key splits lives in a file-scope device array of
+ * SX_NOALLOC_SCRATCH_BYTES (9.1 MiB) that every GPU which loads the library holds until the process exits.
+ *   Limit: total_rows * num_q_heads <= SX_NOALLOC_MAX_PAIRS (row, query head) pairs (e.g. 32 rows x 32 heads);
+ *          beyond it SX_ERR_UNSUPPORTED with the sizes in sx_last_error(), nothing launched. The number of key
+ *          splits is reduced until its partials fit the array (18 at the limit), so a row set near the limit may be
+ *          cut differently from sx_sparse_attn (same tolerance, different rounding); equal cuts give equal bits.
+ *   Not available for batches in zero-copy mode (their page classification needs the workspace).
+ *   The call makes no cudaMalloc / cudaFree and uses no allocating library routine; the first call on a device looks
+ *   the array's device address up once (make that call outside a graph capture).
+ *   SHARED STATE: every call on a device uses the same array. Calls ordered on one stream (or by events / graph
+ *   edges) are safe, and nothing has to be cleared between them; calls that OVERLAP on the GPU race on the array
+ *   (wrong results or a hang): concurrent callers use sx_sparse_attn with a workspace each. */
+#define SX_NOALLOC_MAX_PAIRS 1024
+#define SX_NOALLOC_SCRATCH_BYTES 9512096
+sx_status sx_sparse_attn_noalloc(const sx_pool *pool, const sx_batch *batch, const void *q, const int32_t *rows_R,
+                                 const int32_t *rows_off, int32_t total_rows, void *out, float *lse,
+                                 sx_stream stream);
+
 /* Validation of the DEVICE-resident descriptor arrays, which the stage calls cannot see from the host mirrors:
  * seq_len / tok_off / new_off consistent with the host counts; new_idx strictly ascending inside its request;
  * every segment's len / old_pos / new_pos a positive multiple of block_size, src_off the running

@@ -25,7 +25,8 @@ _lib = None
 SX_OK = 0
 EXPORTS = ["sx_workspace_size", "sx_rope_realign", "sx_rope_realign_layers", "sx_scatter_kv", "sx_score_select",
            "sx_score_select_ex", "sx_sparse_attn", "sx_check_batch", "sx_check_rows", "sx_launch_count",
-           "sx_probe_pipe", "sx_last_error", "sx_version"]
+           "sx_probe_pipe", "sx_sparse_attn_noalloc", "sx_last_error", "sx_version"]
+NOALLOC_MAX_PAIRS = 1024          # SX_NOALLOC_MAX_PAIRS of include/sparsex.h
 
 
 class SxPool(ctypes.Structure):
@@ -84,6 +85,8 @@ def load():
         lib.sx_check_rows.argtypes = [PP, PB, vp, vp, i32, vp, sz, vp]
         lib.sx_launch_count.restype = ctypes.c_uint64
         lib.sx_launch_count.argtypes = []
+        lib.sx_sparse_attn_noalloc.restype = ctypes.c_int
+        lib.sx_sparse_attn_noalloc.argtypes = [PP, PB, vp, vp, vp, i32, vp, vp, vp]
         lib.sx_probe_pipe.restype = ctypes.c_int
         lib.sx_probe_pipe.argtypes = [i32, i32, vp, i32, vp]
         lib.sx_last_error.restype = ctypes.c_char_p
@@ -281,6 +284,18 @@ def sparse_attn(pool: DevicePool, batch: DeviceBatch, q: torch.Tensor, out: torc
     _check(load().sx_sparse_attn(ctypes.byref(pool.c), ctypes.byref(batch.c), (1 if full else 0) | (2 if cuda_core else 0) | (0 if cta_pair is None else (4 if cta_pair else 8)), _ptr(q),
                                  _ptr(rows_R), _ptr(rows_off), n, _ptr(out), _ptr(lse), _ptr(ws), ws.numel(),
                                  _stream(stream)), "sx_sparse_attn")
+
+
+def sparse_attn_noalloc(pool: DevicePool, batch: DeviceBatch, q: torch.Tensor, out: torch.Tensor,
+                        rows_R: torch.Tensor, rows_off: torch.Tensor, total_rows: Optional[int] = None,
+                        lse: Optional[torch.Tensor] = None, stream=None):
+    """Stage (c) for small row sets with the library's built-in scratch: no workspace, no allocation
+    (sx_sparse_attn_noalloc; total_rows * Hq <= NOALLOC_MAX_PAIRS). Calls that overlap on the GPU race on that scratch."""
+    n = int(q.shape[0]) if total_rows is None else int(total_rows)
+    assert q.is_contiguous() and out.is_contiguous()
+    _check(load().sx_sparse_attn_noalloc(ctypes.byref(pool.c), ctypes.byref(batch.c), _ptr(q), _ptr(rows_R),
+                                         _ptr(rows_off), n, _ptr(out), _ptr(lse), _stream(stream)),
+           "sx_sparse_attn_noalloc")
 
 
 def selection_offsets(lay) -> tuple:

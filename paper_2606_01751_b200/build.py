@@ -13,7 +13,7 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 OBJ = os.path.join(HERE, "build")
 LIB = os.path.join(HERE, "libsparsex.so")
-SOURCES = ["sx_api.cu", "sx_realign.cu", "sx_scatter.cu", "sx_select.cu", "sx_attn.cu", "sx_attn_small.cu", "sx_colsum.cu", "sx_lse.cu", "sx_index.cu", "sx_check.cu", "sx_probe.cu"]
+SOURCES = ["sx_api.cu", "sx_realign.cu", "sx_scatter.cu", "sx_select.cu", "sx_attn.cu", "sx_attn_small.cu", "sx_colsum.cu", "sx_lse.cu", "sx_index.cu", "sx_check.cu", "sx_probe.cu", "sx_attn_noalloc.cu"]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",
               "-Xcompiler", "-fPIC", "-Xptxas", "-v"]
 

@@ -421,4 +421,19 @@ sx_status sx_sparse_attn(const sx_pool *pool, const sx_batch *batch, int32_t mod
   return launch_attn(pool, batch, q, rows_R, rows_off, total_rows, out, lse, splits, part, want_cta_pair, ZcArgs(), s);
 }
 
+sx_status sx_sparse_attn_noalloc(const sx_pool *pool, const sx_batch *batch, const void *q, const int32_t *rows_R,
+                                 const int32_t *rows_off, int32_t total_rows, void *out, float *lse,
+                                 sx_stream stream) {
+  sx_status st = validate(pool, batch);
+  if (st != SX_OK) return st;
+  if (total_rows < 0) return set_error(SX_ERR_INVALID_ARG, "total_rows < 0");
+  if (total_rows == 0) return SX_OK;
+  if (!q || !out || !rows_R || !rows_off) return set_error(SX_ERR_INVALID_ARG, "q / out / rows_R / rows_off is NULL");
+  if (misaligned(q) || misaligned(out)) return set_error(SX_ERR_MISALIGNED, "q / out not 16-B aligned");
+  if (batch->zero_copy && batch->num_segments > 0)
+    return set_error(SX_ERR_UNSUPPORTED, "sx_sparse_attn_noalloc: zero-copy batches need the workspace (sx_sparse_attn)");
+  return launch_attn_noalloc(pool, batch, q, rows_R, rows_off, total_rows, out, lse,
+                             reinterpret_cast<cudaStream_t>(stream));
+}
+
 }  // extern "C"

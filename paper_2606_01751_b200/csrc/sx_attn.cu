@@ -734,7 +734,7 @@ int attn_pv_splits(const sx_pool *pool, const sx_batch *b, int32_t total_rows, i
 
 sx_status launch_attn(const sx_pool *pool, const sx_batch *b, const void *q, const int32_t *rows,
                       const int32_t *rows_off, int32_t total_rows, void *out, float *lse, int kv_splits,
-                      float *part, bool cta_pair, const ZcArgs &zc, cudaStream_t st) {
+                      float *part, bool cta_pair, const ZcArgs &zc, cudaStream_t st, unsigned long long *tickets) {
   const int g = pool->num_q_heads / pool->num_kv_heads;
   const int rpt = kTile / g;
   CUtensorMap tm_q, tm_k, tm_v;
@@ -762,7 +762,7 @@ sx_status launch_attn(const sx_pool *pool, const sx_batch *b, const void *q, con
   p.kv_splits = kv_splits < 1 ? 1 : kv_splits;
   p.part_o = part;
   p.part_lse = part ? part + (size_t)p.kv_splits * total_rows * pool->num_q_heads * kHeadDim : nullptr;
-  p.tickets = part ? attn_tickets(part) : nullptr;
+  p.tickets = part ? (tickets ? tickets : attn_tickets(part)) : nullptr;
   p.scale = (float)(1.0 / sqrt((double)kHeadDim));
   p.scale_log2 = (float)(kLog2e / sqrt((double)kHeadDim));
   p.zc_table = zc.table;

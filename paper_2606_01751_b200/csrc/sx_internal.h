@@ -55,7 +55,11 @@ size_t select_scratch_bytes(const sx_batch *b);
 // tcgen05 kernels. q_rows: bf16 [total_rows][Hq][128]; rows == nullptr => row n is position n - off[req].
 sx_status launch_attn(const sx_pool *pool, const sx_batch *b, const void *q, const int32_t *rows,
                       const int32_t *rows_off, int32_t total_rows, void *out, float *lse, int kv_splits,
-                      float *part, bool cta_pair, const ZcArgs &zc, cudaStream_t st);
+                      float *part, bool cta_pair, const ZcArgs &zc, cudaStream_t st,
+                      unsigned long long *tickets = nullptr);  // tickets == nullptr: the words behind `part` (attn_tickets)
+// the same kernel with its key-split scratch in a file-scope device array (sx_attn_noalloc.cu): no workspace argument
+sx_status launch_attn_noalloc(const sx_pool *pool, const sx_batch *b, const void *q, const int32_t *rows,
+                              const int32_t *rows_off, int32_t total_rows, void *out, float *lse, cudaStream_t st);
 int attn_pv_splits(const sx_pool *pool, const sx_batch *b, int32_t total_rows, int tiles_per_cta);
 size_t attn_part_bytes();
 unsigned long long *attn_tickets(float *part);  // rendezvous words of the key splits, behind the partial buffer
