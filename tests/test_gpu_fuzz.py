@@ -1,0 +1,302 @@
+"""Randomised layouts through the whole layer on the GPU against the fp64 oracle.
+
+The named parity cases (test_gpu_parity.py) have hand-made shapes; this file draws the shape itself from a seed:
+number of requests, head counts (g = 1 ... 8, 7 included), pool segments of 1 ... 12 pages with arbitrary old
+positions (deltas of either sign and zero), requests that start with new tokens, a reused segment or prefix-cache
+hits, requests without any reused segment, ragged tails, both RoPE pairings, copy-on-write, budgets from 0 to "all
+cached tokens". Every case runs a sparse layer with its own two-sweep selection (bit-exact S_key / R / tables /
+scattered rows, attention within tolerance), the same layer in zero-copy mode (scores and sets equal to the copy
+path's bit for bit), and a full-attention layer.
+"""
+import numpy as np
+import pytest
+import torch
+
+from oracle import sx_oracle as orc
+from paper_2606_01751_b200 import workloads as wl
+
+from helpers import carve_margins, check_close, oracle_layer
+
+pytestmark = pytest.mark.gpu
+
+SEEDS = list(range(96))
+
+
+def random_layout(seed: int) -> wl.Layout:
+    rng = np.random.default_rng(1000 + seed)
+    hkv = int(rng.choice([1, 2, 4, 8]))
+    g = int(rng.choice([1, 2, 4, 7, 8]))
+    n_pool = int(rng.integers(2, 7))
+    pool = [wl.PoolSegment(16 * int(rng.integers(1, 13)), 16 * int(rng.integers(0, 40))) for _ in range(n_pool)]
+    num_reqs = int(rng.choice([1, 2, 3, 5, 9]))
+    reqs, ratios = [], []
+    for r in range(num_reqs):
+        spec = []
+        if rng.random() < 0.25:
+            spec.append(("prefix", 16 * int(rng.integers(1, 4))))
+        n_items = int(rng.integers(1, 7))
+        for _ in range(n_items):
+            if rng.random() < 0.55 and not (r == 1 and num_reqs > 2):      # request 1 of larger batches: no reuse at all
+                spec.append(("seg", int(rng.integers(0, n_pool))))
+            else:
+                spec.append(("new", 16 * int(rng.integers(1, 4))))
+        # every request ends with new tokens (cached tokens behind the last new one score exactly 0: a pure tie),
+        # the last run possibly ragged
+        spec.append(("new", 16 * int(rng.integers(1, 3)) + (int(rng.integers(0, 16)) if rng.random() < 0.5 else 0)))
+        reqs.append(spec)
+        ratios.append(float(rng.choice([0.0, 0.1, 0.25, 0.5, 1.0])))
+    return wl.build_layout("fuzz%d" % seed, 100 + seed, g * hkv, hkv, float(rng.choice([1e4, 5e5])), pool, reqs, ratios,
+                           0.1, cow=bool(rng.random() < 0.3), rope_style=int(rng.integers(0, 2)))
+
+
+def _prepare(seed):
+    lay = random_layout(seed)
+    lt = wl.build_layer(lay, 0)
+    try:
+        carve_margins(lay, lt, max_iter=20)
+    except RuntimeError as e:          # a draw whose cut cannot be made unambiguous says nothing about the kernels
+        pytest.skip("margin carving: %s" % e)
+    return lay, lt
+
+
+# LSE tolerance when the GPU reads its OWN re-rotated keys (chained): the fp32 rotation rounds a few elements in a
+# thousand to the other bf16 neighbour than the fp64 oracle does (reading A12: <= 1 ulp); on a salient (x4) key that is
+# 4 * 2^-8 on one element, i.e. up to |q_i| * 0.0156 / sqrt(128) ~ 4e-3 on the logit of a row that key dominates.
+# With identical key bits (stage-isolated protocol) the bar is 2e-3 (measured < 1e-4).
+LSE_TOL, LSE_TOL_CHAINED = 2e-3, 1e-2
+
+
+@pytest.mark.parametrize("seed", SEEDS)
+def test_random_layout_sparse_layer_copy_and_zero_copy(seed):
+    from paper_2606_01751_b200.layer import GpuLayer, dev_to_bits
+    lay, lt = _prepare(seed)
+    res, pk, pv, kt, vt = oracle_layer(lay, lt, mode="sparse")
+    # the oracle's pool right after stage (a)
+    pk_a, pv_a = lt.pool_k.copy(), lt.pool_v.copy()
+    kt_a, vt_a = lay.k_block_table.copy(), lay.v_block_table.copy()
+    orc.realign(pk_a, pv_a, kt_a, vt_a, lay.segments, lay.src_blocks, lay.rope_theta, lay.rope_style)
+
+    # ---- (A) stage-isolated: stage (a) checked on its own, then every later stage reads the ORACLE's key bits
+    g = GpuLayer(lay, lt)
+    g.cta_pair = bool(seed & 1)
+    g.realign()
+    torch.cuda.synchronize()
+    gk_a = dev_to_bits(g.pool_k)
+    a64, b64 = orc.bf16_to_f64(gk_a), orc.bf16_to_f64(pk_a)
+    assert np.all(np.abs(a64 - b64) <= 2.0 ** -7 * np.abs(b64) + 1e-5)          # <= 1 bf16 ulp everywhere
+    assert np.mean(gk_a == pk_a) > 0.99
+    assert np.array_equal(dev_to_bits(g.pool_v), pv_a)
+    g.pool_k.copy_(torch.from_numpy(pk_a.view(np.int16)))
+    g.step_sparse(do_realign=False)
+    torch.cuda.synchronize()
+    sel, rows = g.sel_idx.cpu().numpy(), g.rows_R.cpu().numpy()
+    out = orc.bf16_to_f64(dev_to_bits(g.out))
+    lse = g.lse.cpu().numpy().astype(np.float64)
+    sc = g.scores.cpu().numpy().astype(np.float64)
+    for r in range(lay.num_reqs):
+        o, t = int(lay.tok_off[r]), int(lay.seq_len[r])
+        s0, s1 = g.sel_off_h[r], g.sel_off_h[r + 1]
+        r0, r1 = g.rows_off_h[r], g.rows_off_h[r + 1]
+        rel = np.abs(sc[o:o + t] - res.scores[r]) / (np.abs(res.scores[r]) + 1e-2)
+        assert rel.max() < 5e-3, (seed, r, rel.max())
+        assert np.array_equal(sel[s0:s1], res.sel[r]), (seed, r)
+        assert np.array_equal(rows[r0:r1], res.rows[r]), (seed, r)
+        if r1 > r0:
+            check_close("fuzz %d req %d O" % (seed, r), out[r0:r1], res.out[r])
+            assert np.max(np.abs(lse[r0:r1] - res.lse[r])) < LSE_TOL
+    # identical inputs to every write: the pool and the tables after the layer equal the oracle's bit for bit
+    assert np.array_equal(g.batch.k_block_table.cpu().numpy(), kt)
+    assert np.array_equal(g.batch.v_block_table.cpu().numpy(), vt)
+    assert np.array_equal(dev_to_bits(g.pool_k), pk) and np.array_equal(dev_to_bits(g.pool_v), pv)
+
+    # ---- (B) chained: the GPU reads its own re-rotated keys; the carved margin keeps the sets identical
+    c = GpuLayer(lay, lt)
+    c.cta_pair = bool(seed & 1)
+    c.step_sparse()
+    # ---- (C) the same layer in zero-copy mode: keys rotated on the fly = the bits of (B)
+    z = GpuLayer(wl.zero_copy_layout(lay), lt)
+    z.step_sparse(do_realign=False)
+    torch.cuda.synchronize()
+    assert np.array_equal(z.scores.cpu().numpy(), c.scores.cpu().numpy())
+    ck = dev_to_bits(c.pool_k)
+    zk = dev_to_bits(z.pool_k)
+    for name, x in (("chained", c), ("zero-copy", z)):
+        assert np.array_equal(x.sel_idx.cpu().numpy(), sel) and np.array_equal(x.rows_R.cpu().numpy(), rows), (seed, name)
+        xo = orc.bf16_to_f64(dev_to_bits(x.out))
+        xl = x.lse.cpu().numpy().astype(np.float64)
+        for r in range(lay.num_reqs):
+            r0, r1 = g.rows_off_h[r], g.rows_off_h[r + 1]
+            if r1 > r0:
+                check_close("fuzz %d %s req %d O" % (seed, name, r), xo[r0:r1], res.out[r])
+                assert np.max(np.abs(xl[r0:r1] - res.lse[r])) < LSE_TOL_CHAINED
+    assert np.max(np.abs(z.lse.cpu().numpy() - c.lse.cpu().numpy()), initial=0.0) < LSE_TOL   # same key bits again
+    for r in range(lay.num_reqs):
+        pages = lay.k_block_table[r, np.unique(res.rows[r] // 16)]
+        assert np.array_equal(zk[pages], ck[pages]), (seed, r)
+    src = np.concatenate(lay.pool_seg_pages)
+    assert np.array_equal(zk[src], lt.pool_k[src]) and np.array_equal(ck[src], lt.pool_k[src])
+
+
+@pytest.mark.parametrize("seed", SEEDS[::3])
+def test_random_layout_full_layer(seed):
+    from paper_2606_01751_b200.layer import GpuLayer, dev_to_bits
+    lay, lt = _prepare(seed)
+    has_prefix = any(bool(lay.prefix_mask(r).any()) for r in range(lay.num_reqs))
+    if has_prefix:
+        pytest.skip("with prefix-cache hits full layers run in mode 0 (covered by tiny-prefix)")
+    res, pk, pv, kt, vt = oracle_layer(lay, lt, mode="full")
+    g = GpuLayer(lay, lt)
+    g.cta_pair = bool(seed & 1)
+    g.step_full()
+    torch.cuda.synchronize()
+    out = orc.bf16_to_f64(dev_to_bits(g.out))
+    lse = g.lse.cpu().numpy().astype(np.float64)
+    for r in range(lay.num_reqs):
+        o, t = int(lay.tok_off[r]), int(lay.seq_len[r])
+        check_close("fuzz %d full O" % seed, out[o:o + t], res.out[r])
+        assert np.max(np.abs(lse[o:o + t] - res.lse[r])) < LSE_TOL      # every key is fresh: identical bits
+    assert np.array_equal(dev_to_bits(g.pool_v), pv)
+
+
+@pytest.mark.parametrize("seed", SEEDS[::2])
+def test_random_row_sets_attention_all_dispatch_choices(seed):
+    """Stage (c) alone on random row lists (0 ... 40 rows per request, some requests empty) over the oracle's own
+    pool bits: the default dispatch (tensor-core tile, key splits when the grid is small), the CUDA-core kernels
+    (SX_ATTN_CUDA_CORE, when the row set qualifies) and the no-allocation entry point, each against orc.attention."""
+    from paper_2606_01751_b200 import binding as sx
+    from paper_2606_01751_b200.layer import GpuLayer, dev_to_bits
+    lay = random_layout(seed)
+    lt = wl.build_layer(lay, 0)
+    rng = np.random.default_rng(5000 + seed)
+    # oracle pool: realign, then every position that is new or reused gets its fresh row (prefix hits keep theirs)
+    pk, pv = lt.pool_k.copy(), lt.pool_v.copy()
+    kt, vt = lay.k_block_table.copy(), lay.v_block_table.copy()
+    cow = lay.cow_private if lay.cow else None
+    orc.realign(pk, pv, kt, vt, lay.segments, lay.src_blocks, lay.rope_theta, lay.rope_style)
+    picks = []
+    for r in range(lay.num_reqs):
+        t, o = int(lay.seq_len[r]), int(lay.tok_off[r])
+        nidx = lay.new_idx[lay.new_off[r]:lay.new_off[r + 1]]
+        orc.scatter_kv(pk, pv, kt, vt, cow, r, nidx, lt.k_fresh[o + nidx], lt.v_fresh[o + nidx])
+        n = 0 if (lay.num_reqs > 1 and rng.random() < 0.25) else int(rng.integers(1, min(t, 40) + 1))
+        cand = np.nonzero(~lay.prefix_mask(r))[0]
+        picks.append(np.sort(rng.choice(cand, size=min(n, len(cand)), replace=False)).astype(np.int32))
+    if sum(len(p) for p in picks) == 0:
+        picks[0] = np.asarray([int(lay.seq_len[0]) - 1], dtype=np.int32)
+    g = GpuLayer(lay, lt)
+    g.pool_k.copy_(torch.from_numpy(pk.view(np.int16)))
+    g.pool_v.copy_(torch.from_numpy(pv.view(np.int16)))
+    g.batch.k_block_table.copy_(torch.from_numpy(kt).to(g.dev))
+    g.batch.v_block_table.copy_(torch.from_numpy(vt).to(g.dev))
+    off = np.concatenate([[0], np.cumsum([len(p) for p in picks])]).astype(np.int32)
+    rows = torch.from_numpy(np.concatenate(picks)).to(g.dev)
+    rows_off = torch.from_numpy(off).to(g.dev)
+    tok = np.concatenate([int(lay.tok_off[r]) + p.astype(np.int64) for r, p in enumerate(picks)])
+    q = g.q_full[torch.from_numpy(tok).to(g.dev)].contiguous()
+    n, hq = int(rows.numel()), lay.num_q_heads
+    ref = [orc.attention(pk, pv, kt[r], vt[r], int(lay.seq_len[r]), lt.q_full[int(lay.tok_off[r]) + picks[r]], picks[r],
+                         hq, want_lse=True) if len(picks[r]) else None for r in range(lay.num_reqs)]
+    choices = [("default", lambda o, l: sx.sparse_attn(g.pool, g.batch, q, o, rows_R=rows, rows_off=rows_off,
+                                                        total_rows=n, lse=l))]
+    if hq // lay.num_kv_heads <= 32:
+        choices.append(("cuda-core", lambda o, l: sx.sparse_attn(g.pool, g.batch, q, o, rows_R=rows, rows_off=rows_off,
+                                                                  total_rows=n, lse=l, cuda_core=True)))
+    if n * hq <= sx.NOALLOC_MAX_PAIRS:
+        choices.append(("noalloc", lambda o, l: sx.sparse_attn_noalloc(g.pool, g.batch, q, o, rows, rows_off,
+                                                                        total_rows=n, lse=l)))
+    for name, call in choices:
+        o = torch.full((n, hq, 128), 0x7fc0, dtype=torch.int16, device=g.dev)
+        l = torch.full((n, hq), float("nan"), dtype=torch.float32, device=g.dev)
+        call(o, l)
+        torch.cuda.synchronize()
+        got_o, got_l = orc.bf16_to_f64(dev_to_bits(o)), l.cpu().numpy().astype(np.float64)
+        for r in range(lay.num_reqs):
+            if ref[r] is not None:
+                check_close("fuzz %d %s req %d O" % (seed, name, r), got_o[off[r]:off[r + 1]], ref[r][0])
+                assert np.max(np.abs(got_l[off[r]:off[r + 1]] - ref[r][1])) < LSE_TOL, (seed, name, r)
+
+
+def random_layout_ending_anywhere(seed: int) -> wl.Layout:
+    """Like random_layout, but a request may END inside a reused segment (tail fallback). Budgets count
+    only the cached tokens in front of the last new token: the ones behind it score exactly 0 on both sides, and a
+    cut among them would be a pure position tie that no margin can be carved into."""
+    rng = np.random.default_rng(9000 + seed)
+    hkv = int(rng.choice([1, 2, 4]))
+    g = int(rng.choice([1, 2, 4, 7]))
+    n_pool = int(rng.integers(2, 6))
+    pool = [wl.PoolSegment(16 * int(rng.integers(1, 10)), 16 * int(rng.integers(0, 40))) for _ in range(n_pool)]
+    num_reqs = int(rng.choice([1, 2, 3, 4]))
+    reqs, ratios = [], []
+    for r in range(num_reqs):
+        spec = [("prefix", 16 * int(rng.integers(1, 3)))] if rng.random() < 0.3 else []
+        spec.append(("new", 16 * int(rng.integers(1, 3))) if rng.random() < 0.5 else ("seg", int(rng.integers(0, n_pool))))
+        for _ in range(int(rng.integers(1, 5))):
+            spec.append(("seg", int(rng.integers(0, n_pool))) if rng.random() < 0.6 else ("new", 16 * int(rng.integers(1, 3))))
+        if not any(k == "new" for k, _ in spec):
+            spec.insert(len(spec) // 2 + 1, ("new", 16))
+        reqs.append(spec)
+        ratios.append(float(rng.choice([0.1, 0.25, 0.5])))
+    args = ("fuzz-tail%d" % seed, 300 + seed, g * hkv, hkv, 1e4, pool, reqs, ratios, 0.1)
+    lay0 = wl.build_layout(*args, rope_style=int(seed & 1))
+    k = []
+    for r in range(num_reqs):
+        last_new = int(lay0.new_idx[lay0.new_off[r + 1] - 1])
+        k.append(int(np.floor(ratios[r] * int(lay0.cached_mask(r)[:last_new].sum()))))
+    trim = [int(rng.integers(0, 16)) if spec[-1][0] == "seg" and rng.random() < 0.4 else 0 for spec in reqs]
+    return wl.build_layout(*args, rope_style=int(seed & 1), k_override=k, trim=trim)
+
+
+@pytest.mark.parametrize("seed", SEEDS[::2])
+def test_random_layout_extended_selection(seed):
+    """sx_score_select_ex on random layouts whose requests may end inside a reused segment, with random overflow /
+    tail settings: R = I_nr U S_key U S_ov U S_tail bit-exact against the oracle, then scatter + attention on that
+    data-dependent row list; the same in zero-copy mode (same sets)."""
+    from paper_2606_01751_b200 import binding as sx
+    from paper_2606_01751_b200.layer import GpuLayer, dev_to_bits
+    rng = np.random.default_rng(7000 + seed)
+    ov, tail = int(rng.choice([0, 1, 2])), int(rng.choice([0, 16, 64]))
+    lay = random_layout_ending_anywhere(seed)
+    lt = wl.build_layer(lay, 0)
+    try:
+        carve_margins(lay, lt, max_iter=20)
+    except RuntimeError as e:
+        pytest.skip("margin carving: %s" % e)
+    pk, pv = lt.pool_k.copy(), lt.pool_v.copy()
+    kt, vt = lay.k_block_table.copy(), lay.v_block_table.copy()
+    orc.realign(pk, pv, kt, vt, lay.segments, lay.src_blocks, lay.rope_theta, lay.rope_style)
+    layers = []
+    for zc in (False, True):
+        g = GpuLayer(wl.zero_copy_layout(lay) if zc else lay, lt)
+        if not zc:
+            g.realign()
+            g.pool_k.copy_(torch.from_numpy(pk.view(np.int16)))      # stage-isolated: the oracle's key bits
+        g.scatter_new()
+        g.select_ex(overflow_blocks=ov, tail_tokens=tail)
+        g.stage_rows(g.sel_idx, g.rows_R)
+        sx.scatter_kv(g.pool, g.batch, g.kf_R, g.vf_R, g.rows_R, g.rows_off, max_rows=g.rows_cap)
+        g.attend()
+        torch.cuda.synchronize()
+        layers.append(g)
+    g, z = layers
+    sel_g, rows_g = g.sel_idx.cpu().numpy(), g.rows_R.cpu().numpy()
+    assert np.array_equal(z.sel_idx.cpu().numpy(), sel_g) and np.array_equal(z.rows_R.cpu().numpy(), rows_g)
+    assert np.array_equal(z.rows_off_h, g.rows_off_h)
+    out = orc.bf16_to_f64(dev_to_bits(g.out))
+    zout = orc.bf16_to_f64(dev_to_bits(z.out))
+    for r in range(lay.num_reqs):
+        t, o = int(lay.seq_len[r]), int(lay.tok_off[r])
+        nidx = lay.new_idx[lay.new_off[r]:lay.new_off[r + 1]]
+        orc.scatter_kv(pk, pv, kt, vt, None, r, nidx, lt.k_fresh[o + nidx], lt.v_fresh[o + nidx])
+        s = orc.scores(pk, kt[r], t, lt.q_full[o + nidx], nidx, lay.num_q_heads)
+        is_new, cand = lay.is_new_mask(r), lay.cached_mask(r)
+        sel, _ = orc.select_topk(s, is_new, int(lay.k_per_req[r]), cand)
+        segr = [(int(n), int(n + ln)) for (rq, ln, _, n, _) in lay.segments.tolist() if rq == r]
+        rows = orc.recompute_set(is_new, sel, segr, ov, tail, cand_mask=cand)
+        r0, r1 = int(g.rows_off_h[r]), int(g.rows_off_h[r + 1])
+        assert np.array_equal(sel_g[g.sel_off_h[r]:g.sel_off_h[r + 1]], sel), (seed, r, ov, tail)
+        assert np.array_equal(rows_g[r0:r1], rows), (seed, r, ov, tail)
+        orc.scatter_kv(pk, pv, kt, vt, None, r, rows, lt.k_fresh[o + rows], lt.v_fresh[o + rows])
+        ref = orc.attention(pk, pv, kt[r], vt[r], t, lt.q_full[o + rows], rows, lay.num_q_heads)
+        check_close("fuzz %d ex req %d O" % (seed, r), out[r0:r1], ref)
+        check_close("fuzz %d ex zero-copy req %d O" % (seed, r), zout[r0:r1], ref)
+    assert np.array_equal(dev_to_bits(g.pool_k), pk) and np.array_equal(dev_to_bits(g.pool_v), pv)
