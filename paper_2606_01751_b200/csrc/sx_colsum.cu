@@ -24,12 +24,25 @@ constexpr int kCsThreads = 320;  // warps 0-7 consumers, warp 8 TMA producer, wa
 constexpr int kCsTileBytes = kTile * kHeadDim * 2;
 constexpr int kCsHalf = kCsTileBytes / 2;
 constexpr int kCsStages = 2;
+#ifndef SX_COLSUM_KSLOT
+#define SX_COLSUM_KSLOT 1  // 1: the normaliser rides through the MMA as a ninth K step (see colsum_kernel); 0: added per element
+#endif
+constexpr bool kCsKslot = SX_COLSUM_KSLOT != 0;
+// extra operand blocks of the ninth K step: 128 rows x 16 bf16 (32 B), K-major, NO swizzle: core matrices of
+// 8 rows x 16 B; (row group, K chunk) at group * 256 + chunk * 128, i.e. LBO = 128 B, SBO = 256 B
+constexpr int kCsExtBytes = kCsKslot ? kTile * 32 : 0;
 constexpr int kCsOffK = 0;
-constexpr int kCsOffQ = kCsOffK + kCsTileBytes;
-constexpr int kCsColStages = 8;  // (lse, position) rows of 128 columns: 1 KB each, own ring (see producer)
-constexpr int kCsOffCol = kCsOffQ + kCsStages * kCsTileBytes;  // float2 [kCsColStages][128]
-constexpr int kCsOffBar = kCsOffCol + kCsColStages * 1024;
-constexpr int kCsSmemBytes = kCsOffBar + 256 + 1024;  // 2 CTAs per SM
+constexpr int kCsOffAext = kCsOffK + kCsTileBytes;              // A side: [1, 1, 1, 0 ...] for every key row
+constexpr int kCsOffQ = kCsOffAext + kCsExtBytes;
+constexpr int kCsQStage = kCsTileBytes + kCsExtBytes;           // a Q stage = the tile, then its extra block
+constexpr int kCsColStages = kCsKslot ? 6 : 8;                  // ring of column rows (see producer)
+constexpr int kCsColRow = kCsKslot ? 512 : 1024;                // K-slot form: positions only (mask tiles only)
+constexpr int kCsOffCol = kCsOffQ + kCsStages * kCsQStage;
+constexpr int kCsOffBar = kCsOffCol + kCsColStages * kCsColRow;
+constexpr int kCsSmemBytes = kCsOffBar + 256 + 1024;  // 2 CTAs per SM: 2 x (this + 1 KB) <= 228 KB
+static_assert(2 * (kCsSmemBytes + 1024) <= 233472, "two CTAs per SM");
+static_assert(kCsQStage % 1024 == 0, "128-B swizzle atoms need 1024-B aligned tiles");
+constexpr int kCsTabEntry = 1024 + (kCsKslot ? 4096 : 0);       // bytes per (query tile, KV head) in the workspace
 #ifndef SX_COLSUM_POLY
 #define SX_COLSUM_POLY 2  // of every 8 pairs of exponentials, this many pairs go to the FMA pipe (0..8);
                           // measured on C2 / C4 / C5 (MUFU pipe 77 % busy at 1): 2 and 3 are 1-2 % faster than 1, 4 slower
@@ -41,7 +54,8 @@ struct ColsumParams {
   int lse_by_token;
   int lse_splits;     // > 1: lse holds that many partial normalisers [split][total_new][Hq] (key splits)
   size_t lse_stride;  // total_new * Hq
-  float2 *col_tab;   // [query tiles of the batch][Hkv] rows of 1 KB: float lse * log2 e [128], then int position [128]
+  float2 *col_tab;   // [query tiles of the batch][Hkv] entries of kCsTabEntry bytes: float lse * log2 e [128], int position
+                     // [128], then (K-slot form) the 4-KB extra B block of the tile in its shared-memory layout
   float *partial;    // [Hkv][total_tokens]
   int num_reqs, max_pages, num_q_heads, num_kv_heads, group, rows_per_tile, total_tokens;
   float scale_log2;
@@ -94,9 +108,25 @@ coltab_kernel(const ColsumParams p) {
     }
     lse2 = l * (float)kLog2e;
   }
-  float *row = reinterpret_cast<float *>(p.col_tab + ((size_t)blockIdx.x * p.num_kv_heads + kvh) * 128);
+  uint8_t *entry = reinterpret_cast<uint8_t *>(p.col_tab) + ((size_t)blockIdx.x * p.num_kv_heads + kvh) * kCsTabEntry;
+  float *row = reinterpret_cast<float *>(entry);
   row[ct] = lse2;
   row[128 + ct] = __int_as_float(qpos);
+  if (kCsKslot) {
+    // -lse2 / scale_log2 = -lse * sqrt(d), split into three bf16 (hi + mid + lo carries 24 bits): the MMA adds it to
+    // the raw score of every key of the column. Pad columns: -inf (their exponential is 0), mid = lo = 0.
+    const float v = (lse2 == INFINITY) ? -INFINITY : -lse2 / p.scale_log2;
+    const __nv_bfloat16 h = __float2bfloat16_rn(v);
+    float rem = (lse2 == INFINITY) ? 0.f : v - __bfloat162float(h);
+    const __nv_bfloat16 m = __float2bfloat16_rn(rem);
+    rem -= __bfloat162float(m);
+    const __nv_bfloat16 l = __float2bfloat16_rn(rem);
+    const uint32_t w0 = (uint32_t)__bfloat16_as_ushort(h) | ((uint32_t)__bfloat16_as_ushort(m) << 16);
+    const uint32_t w1 = (uint32_t)__bfloat16_as_ushort(l);
+    uint4 *ext = reinterpret_cast<uint4 *>(entry + 1024);
+    ext[(ct >> 3) * 16 + (ct & 7)] = make_uint4(w0, w1, 0, 0);   // K chunk 0 of column ct
+    ext[(ct >> 3) * 16 + 8 + (ct & 7)] = make_uint4(0, 0, 0, 0);  // K chunk 1
+  }
 }
 
 // One consumer thread, one D tile: sum of exp2(s * c - lse_col) over its 64 columns (d[2][32] = raw scores of its key
@@ -107,15 +137,16 @@ __device__ __forceinline__ float2 cs_consume(const uint32_t (&d)[2][32], uint32_
   for (int c = 0; c < 2; ++c)
 #pragma unroll
     for (int i = 0; i < 32; i += 4) {
-      const float4 l4 = lds_f4(col + (c * 32 + i) * 4);  // lse of four columns
+      float4 l4 = make_float4(0.f, 0.f, 0.f, 0.f);
+      if (!kCsKslot) l4 = lds_f4(col + (c * 32 + i) * 4);  // lse of four columns (K-slot form: already inside d)
       float4 p4 = make_float4(0.f, 0.f, 0.f, 0.f);
-      if (kMask) p4 = lds_f4(col + 512 + (c * 32 + i) * 4);  // their positions (int bits)
+      if (kMask) p4 = lds_f4(col + (kCsKslot ? 0 : 512) + (c * 32 + i) * 4);  // their positions (int bits)
 #pragma unroll
       for (int h2 = 0; h2 < 2; ++h2) {
         const int ii = i + 2 * h2;
         const float la = h2 ? l4.z : l4.x, lb = h2 ? l4.w : l4.y;
-        float2 x = __ffma2_rn(make_float2(__uint_as_float(d[c][ii]), __uint_as_float(d[c][ii + 1])), sc2,
-                              make_float2(-la, -lb));
+        const float2 dv = make_float2(__uint_as_float(d[c][ii]), __uint_as_float(d[c][ii + 1]));
+        const float2 x = kCsKslot ? __fmul2_rn(dv, sc2) : __ffma2_rn(dv, sc2, make_float2(-la, -lb));
         float2 e;
         if ((ii & 15) < 2 * SX_COLSUM_POLY) {
           e = ex2_poly2(x);
@@ -142,7 +173,7 @@ colsum_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_constant__ 
   extern __shared__ uint8_t smem_raw[];
   uint8_t *smem = reinterpret_cast<uint8_t *>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~uintptr_t(1023));
   CsBars *bars = reinterpret_cast<CsBars *>(smem + kCsOffBar);
-  float2 *col_sm = reinterpret_cast<float2 *>(smem + kCsOffCol);  // [kCsColStages][128] (lse2, position)
+  uint8_t *col_sm = smem + kCsOffCol;  // [kCsColStages] rows of kCsColRow bytes: (lse2[128],) position[128]
   griddep_launch();
   griddep_wait();
 
@@ -172,6 +203,14 @@ colsum_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_constant__ 
   const int qt0 = lo / rpt;                          // first query tile with a visible query
   const int n_qt = (nn + rpt - 1) / rpt;
   const int n_it = (lo < nn) ? n_qt - qt0 : 0;
+  // queries are sorted by position: only the leading tiles, whose first query sits below the tile's last key, need a
+  // causal mask. n_mask = tiles it < n_mask (first query index (qt0 + it) * rpt below lower_bound(new_idx, j0 + 127))
+  int lo2 = lo, hi2 = nn;
+  while (lo2 < hi2) {
+    int mid = (lo2 + hi2) >> 1;
+    if (p.new_idx[nq0 + mid] < j0 + kTile - 1) lo2 = mid + 1; else hi2 = mid;
+  }
+  const int n_mask = max(0, (lo2 + rpt - 1) / rpt - qt0);
 
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
   constexpr int kWarpProd = 8, kWarpMma = 9;
@@ -200,8 +239,17 @@ colsum_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_constant__ 
     const int pad = kTile - rpt * g;
     for (int i = threadIdx.x; i < kCsStages * 2 * pad * 8; i += kCsThreads) {
       int c16 = i & 7, r = (i >> 3) % pad, hs = (i >> 3) / pad;  // hs = stage*2 + half
-      *reinterpret_cast<uint4 *>(smem + kCsOffQ + hs * kCsHalf + (rpt * g + r) * 128 + c16 * 16) =
-          make_uint4(0, 0, 0, 0);
+      *reinterpret_cast<uint4 *>(smem + kCsOffQ + (hs >> 1) * kCsQStage + (hs & 1) * kCsHalf + (rpt * g + r) * 128 +
+                                 c16 * 16) = make_uint4(0, 0, 0, 0);
+    }
+    fence_proxy_async_smem();
+  }
+  if (kCsKslot) {
+    // A side of the ninth K step: every key row is [1, 1, 1, 0 ...] (bf16 1.0 = 0x3F80); 256 chunks of 16 B
+    if (threadIdx.x < 256) {
+      const int ch = threadIdx.x;  // chunk (row group, K chunk, row): K chunk = bit 3
+      reinterpret_cast<uint4 *>(smem + kCsOffAext)[ch] =
+          ((ch >> 3) & 1) ? make_uint4(0, 0, 0, 0) : make_uint4(0x3F803F80u, 0x00003F80u, 0, 0);
     }
     fence_proxy_async_smem();
   }
@@ -228,16 +276,28 @@ colsum_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_constant__ 
         int s = 0, ph = 1;
         for (int it = 0; it < n_it; ++it) {
           mbar_wait(&bars->q_empty[s], ph);
-          mbar_expect_tx(&bars->q_full[s], (uint32_t)(2 * rpt * g * 128));
+          mbar_expect_tx(&bars->q_full[s], (uint32_t)(2 * rpt * g * 128 + kCsExtBytes));
           const int r0 = nq0 + (qt0 + it) * rpt;
-          tma_load_3d(smem + kCsOffQ + s * kCsTileBytes, &tm_q, &bars->q_full[s], 0, kvh * g, r0);
-          tma_load_3d(smem + kCsOffQ + s * kCsTileBytes + kCsHalf, &tm_q, &bars->q_full[s], 64, kvh * g, r0);
-          // column table row of this query tile. Ring of 8: this thread is at most 2 tiles ahead of the MMA
-          // issuer, which is at most 2 tiles ahead of the consumers' D loads, so stage it & 7 is free.
-          mbar_expect_tx(&bars->c_full[it & (kCsColStages - 1)], 1024);
-          bulk_load_1d(col_sm + (it & (kCsColStages - 1)) * 128,
-                       p.col_tab + ((size_t)(qt_base + qt0 + it) * p.num_kv_heads + kvh) * 128, 1024,
-                       &bars->c_full[it & (kCsColStages - 1)]);
+          uint8_t *qs = smem + kCsOffQ + s * kCsQStage;
+          tma_load_3d(qs, &tm_q, &bars->q_full[s], 0, kvh * g, r0);
+          tma_load_3d(qs + kCsHalf, &tm_q, &bars->q_full[s], 64, kvh * g, r0);
+          const uint8_t *entry = reinterpret_cast<const uint8_t *>(p.col_tab) +
+                                 ((size_t)(qt_base + qt0 + it) * p.num_kv_heads + kvh) * kCsTabEntry;
+          // Column row of this query tile, own ring: this thread is at most 2 tiles ahead of the MMA issuer, which is
+          // at most 2 tiles ahead of the consumers' D loads, so 5 slots suffice.
+          const int cs = it % kCsColStages;
+          if (kCsKslot) {
+            // the tile's extra B block (normalisers) lands behind the tile on the same barrier; positions are needed by
+            // the leading mask tiles only
+            bulk_load_1d(qs + kCsTileBytes, entry + 1024, kCsExtBytes, &bars->q_full[s]);
+            if (it < n_mask) {
+              mbar_expect_tx(&bars->c_full[cs], 512);
+              bulk_load_1d(col_sm + cs * kCsColRow, entry + 512, 512, &bars->c_full[cs]);
+            }
+          } else {
+            mbar_expect_tx(&bars->c_full[cs], 1024);
+            bulk_load_1d(col_sm + cs * kCsColRow, entry, 1024, &bars->c_full[cs]);
+          }
           if (++s == kCsStages) { s = 0; ph ^= 1; }
         }
       }
@@ -256,11 +316,19 @@ colsum_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_constant__ 
         mbar_wait(&bars->q_full[s], ph);
         if (it >= 2) mbar_wait(&bars->d_empty[b], ((it >> 1) + 1) & 1);
         tc_fence_after();
-        const uint32_t qd = q_lo + (uint32_t)s * (kCsTileBytes >> 4);
+        const uint32_t qd = q_lo + (uint32_t)s * (kCsQStage >> 4);
 #pragma unroll
         for (int kk = 0; kk < 8; ++kk) {
           const uint32_t o = ((kk >> 2) * kCsHalf + (kk & 3) * 32) >> 4;
           umma_ss2(tmem + b * 128, k_lo + o, hi32, qd + o, hi32, idesc, kk > 0);
+        }
+        if (kCsKslot) {
+          // ninth K step: D += [1 1 1 0 ...] x [hi mid lo 0 ...]^T = -lse * sqrt(d) of every column, added to every
+          // key row. Unswizzled K-major blocks: LBO = 128 B (K chunks), SBO = 256 B (8-row groups), layout type 0.
+          constexpr uint32_t ext_hi = (256u >> 4) | (1u << 14);
+          const uint32_t a_ext = ((smem_u32(smem + kCsOffAext) & 0x3FFFF) >> 4) | ((128u >> 4) << 16);
+          const uint32_t b_ext = ((smem_u32(smem + kCsOffQ + s * kCsQStage + kCsTileBytes) & 0x3FFFF) >> 4) | ((128u >> 4) << 16);
+          umma_ss2(tmem + b * 128, a_ext, ext_hi, b_ext, ext_hi, idesc, 1);
         }
         umma_commit(&bars->d_full[b]);
         umma_commit(&bars->q_empty[s]);
@@ -284,11 +352,12 @@ colsum_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_constant__ 
       mbar_arrive(&bars->k_rot);
     }
     for (int it = 0; it < n_it; ++it) {
-      const int b = it & 1, cs = it & (kCsColStages - 1);
-      mbar_wait(&bars->c_full[cs], (it / kCsColStages) & 1);
-      const uint32_t col = smem_u32(col_sm + cs * 128) + hf * 256;   // lse of this thread's 64 columns; +512: positions
-      // queries are sorted by position: only tiles whose first query is below the tile's last key need a mask
-      const bool need_mask = __float_as_int(lds_f1(smem_u32(col_sm + cs * 128) + 512)) < j0 + kTile - 1;
+      const int b = it & 1, cs = it % kCsColStages;
+      const bool need_mask = it < n_mask;  // (the leading tiles, see n_mask)
+      // K-slot form: the row holds positions only and exists for mask tiles only
+      if (!kCsKslot || need_mask) mbar_wait(&bars->c_full[cs], (it / kCsColStages) & 1);
+      const uint32_t col = smem_u32(col_sm + cs * kCsColRow) + hf * 256;  // this thread's 64 columns: lse (+512:
+                                                                          // positions), or positions alone
       mbar_wait(&bars->d_full[b], (it >> 1) & 1);
       tc_fence_after();
       uint32_t d[2][32];
@@ -319,7 +388,7 @@ colsum_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_constant__ 
 size_t colsum_tab_bytes(const sx_pool *pool, const sx_batch *b) {
   const int g = pool->num_q_heads / pool->num_kv_heads;
   const int rpt = kTile / (g > 0 ? g : 1) > 0 ? kTile / (g > 0 ? g : 1) : 1;
-  return (size_t)(b->total_new / rpt + b->num_reqs) * pool->num_kv_heads * 128 * sizeof(float2);
+  return (size_t)(b->total_new / rpt + b->num_reqs) * pool->num_kv_heads * kCsTabEntry;
 }
 
 sx_status launch_colsum(const sx_pool *pool, const sx_batch *b, const void *q_new, const float *lse_new,
