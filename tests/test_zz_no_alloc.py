@@ -109,3 +109,26 @@ def test_noalloc_near_the_limit_cuts_the_keys_differently_but_stays_in_tolerance
     _both(sx, g, lay, [np.arange(t - 35, t)])
     same, _, _ = _both(sx, g, lay, [np.arange(t - 16, t)])      # 448 pairs: 32 splits fit, equal cuts again
     assert same
+
+
+def test_noalloc_under_cuda_graph_capture_and_replay():
+    """The use case the entry point exists for: captured into a CUDA graph (after one eager call, which performs the
+    once-per-device address lookup) and replayed; every replay gives the bits of the eager call."""
+    lay = wl.config_c1()
+    sx, g = _layer(lay)
+    t = int(lay.seq_len[0])
+    rows, off, q = _rows(lay, g, [np.arange(t - 6, t)])
+    out = torch.zeros((6, lay.num_q_heads, 128), dtype=torch.int16, device=g.dev)
+    lse = torch.zeros((6, lay.num_q_heads), dtype=torch.float32, device=g.dev)
+    sx.sparse_attn_noalloc(g.pool, g.batch, q, out, rows, off, total_rows=6, lse=lse)
+    torch.cuda.synchronize()
+    eager_o, eager_l = out.clone(), lse.clone()
+    graph = torch.cuda.CUDAGraph()
+    with torch.cuda.graph(graph):
+        sx.sparse_attn_noalloc(g.pool, g.batch, q, out, rows, off, total_rows=6, lse=lse)
+    for _ in range(3):
+        out.zero_()
+        lse.zero_()
+        graph.replay()
+        torch.cuda.synchronize()
+        assert torch.equal(out, eager_o) and torch.equal(lse, eager_l)
