@@ -15,8 +15,10 @@
  *   - "device" pointers are CUDA device memory owned by the caller; "host" values are plain integers
  *     in the structs below. The library allocates nothing and frees nothing. The only process-wide state it
  *     keeps is (i) a bounded cache of encoded TMA tensor maps keyed by (base pointer, shape) -- a pure function
- *     of its key, so it cannot go stale -- (ii) the kernel-launch counter of sx_launch_count() and (iii) the
- *     thread-local text of sx_last_error(). All entry points may be called from several threads.
+ *     of its key, so it cannot go stale -- (ii) the kernel-launch counter of sx_launch_count(), (iii) the
+ *     thread-local text of sx_last_error() and (iv) the built-in device scratch of sx_sparse_attn_noalloc (9.1 MiB
+ *     per GPU, used by that entry point only). All entry points may be called from several threads; calls of
+ *     sx_sparse_attn_noalloc must not overlap on the GPU (see there).
  *   - Every stage call is asynchronous on `stream` and never synchronises the device (the two validation calls
  *     sx_check_batch / sx_check_rows do: they are for descriptor construction time). A non-zero status
  *     means nothing was launched (argument errors) or a launch failed (SX_ERR_CUDA);
