@@ -148,6 +148,10 @@ attn_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_constant__ CU
     mbar_init(&bars->v_landed, 1);
     fence_mbar_init();
   }
+  // kPair: the TMA loads of rank 1 complete on rank 0's barriers, which must exist by then: both CTAs meet once,
+  // split in two halves so that the lookups below run in between (the producer warps wait before their first load,
+  // everyone else just before the block-wide sync)
+  if (kPair) cluster_arrive();
   if (warp == kWarpMma) {
     if (kPair) {
       tmem_alloc_pair(&bars->tmem_base, 512);
@@ -200,6 +204,86 @@ attn_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_constant__ CU
   const int row_base = pair >= 0 ? p.rows_off[req] + pair * rpc : p.total_rows;  // first row of query tile 0
   const int T = p.seq_len[req];
   const int n_pages = (T + kPage - 1) / kPage;
+  // ---- TMA producers' addressing. Single CTA: lane = (page of the tile, 64-column half), 16 boxes per item.
+  // kPair: 8 boxes per item: K item = this CTA's 64 keys (4 pages) x both halves -> [half][64 keys][128 B],
+  //        the keys being 32 of each 64-key half of the tile: pages {2r, 2r+1, 4+2r, 5+2r} for rank r;
+  //        V item = all 8 pages x the CTA's own 64-column half -> [128 keys][128 B].
+  const int pgi = lane >> 1;
+  const int pg_k = kPair ? 2 * rank + (pgi & 1) + 4 * (pgi >> 1) : pgi, half_k = lane & 1;
+  const int pg_v = kPair ? lane : (lane >> 1), half_v = kPair ? rank : (lane & 1);
+  const int n_boxes = kPair ? 8 : 16;
+  const uint32_t full0 = kPair ? mapa_u32(smem_u32(&bars->kv_full[0]), 0) : 0;
+  auto table_entry = [&](int it, int first_tile) -> int {   // ring item it = K (even) / V (odd) of key tile first_tile + it / 2
+    const int t = first_tile + (it >> 1);
+    const bool is_v = it & 1;
+    int lp = t * 8 + (is_v ? pg_v : pg_k);
+    if (lp > n_pages - 1) lp = n_pages - 1;  // pages past the sequence: any valid page (keys are masked)
+    return (is_v ? p.v_table : p.k_table)[(size_t)req * p.max_pages + lp];
+  };
+  auto issue_item = [&](int it, int blk) {                  // the boxes of ring item `it` (its slot must be free)
+    const bool is_v = it & 1;
+    const int s = it % kStages;
+    if (lane == 0 && rank == 0) mbar_expect_tx(&bars->kv_full[s], kTileBytes);  // both CTAs' bytes
+    __syncwarp();
+    if (lane < n_boxes) {
+      const int row0 = (blk * p.num_kv_heads + kvh) * kPage;
+      if (kPair) {
+        uint8_t *dst = smem + Cfg::kOffKV + s * kStageBytes +
+                       (is_v ? pg_v * 2048 : half_k * (kHalfBytes / 2) + (lane >> 1) * 2048);
+        tma_load_2d_pair(dst, is_v ? &tm_v : &tm_k, full0 + s * 8, (is_v ? half_v : half_k) * 64, row0);
+      } else {
+        tma_load_2d(smem + Cfg::kOffKV + s * kTileBytes + half_k * kHalfBytes + pg_k * 2048,
+                    is_v ? &tm_v : &tm_k, &bars->kv_full[s], half_k * 64, row0);
+      }
+    }
+  };
+  auto issue_q = [&](int nq) {  // one thread
+    if (kPair) {
+      // both CTAs always load both query tiles (rows past the batch read as zeros; rows of another request
+      // are never stored), so rank 0's barrier expects a fixed byte count
+      const uint32_t qbar = mapa_u32(smem_u32(&bars->q_full), 0);
+      if (rank == 0) mbar_expect_tx(&bars->q_full, (uint32_t)(2 * 2 * 2 * rpt * g * 128));
+      for (int i = 0; i < 2; ++i) {
+        tma_load_3d_pair(smem + Cfg::kOffQ + i * kTileBytes, &tm_q, qbar, 0, kvh * g, row_base + i * rpt);
+        tma_load_3d_pair(smem + Cfg::kOffQ + i * kTileBytes + kHalfBytes, &tm_q, qbar, 64, kvh * g, row_base + i * rpt);
+      }
+    } else {
+      mbar_expect_tx(&bars->q_full, (uint32_t)(nq * 2 * rpt * g * 128));
+      for (int i = 0; i < nq; ++i) {
+        tma_load_3d(smem + Cfg::kOffQ + i * kTileBytes, &tm_q, &bars->q_full, 0, kvh * g, row_base + i * rpt);
+        tma_load_3d(smem + Cfg::kOffQ + i * kTileBytes + kHalfBytes, &tm_q, &bars->q_full, 64, kvh * g,
+                    row_base + i * rpt);
+      }
+    }
+  };
+  // ---- early issue. Q and the K / V tiles of key tile 0 depend on the row offsets only: not on the tile counts (two
+  // more dependent global loads below), nor on TMEM or the block-wide sync. Issued here they land ~2 000 clk sooner
+  // (clock64 trace of the prologue: CTA entry -> first S tile 7 500 clk before). Not with key splits, whose first key
+  // tile depends on the tile counts. Every CTA that owns rows has at least one key tile.
+  // Warp 8 alone does it (it initialised the barriers: no ordering with another warp needed), and it does not make
+  // the others wait for it: it ARRIVES at the block-wide meeting before it starts issuing (36 TMA operations take
+  // ~2 000 clk) and never waits there itself in the single-CTA form (it needs neither TMEM nor anything another warp
+  // writes before the meeting); in a cluster it picks the second half of the meeting up after the issue.
+  // (Zero-copy variants: warp 8 initialises the rotation barriers after the tile counts are known, so it meets the
+  // others the ordinary way.)
+  const bool early = active && p.kv_splits == 1;
+  int blk_ahead = 0;  // warp 8: block-table entry of its next ring item (K of key tile 1), in flight
+  if (warp == kWarpProd0) {
+    if (kPair) {
+      cluster_wait();    // first meeting (barrier init) complete
+      cluster_arrive();  // second meeting, first half
+    } else if (kZc == 0) {
+      named_bar_arrive(3, kAttnThreads);
+    }
+    if (early) {
+      const int cta_rows = pair >= 0 ? min(rpc, n_r - pair * rpc) : 0;
+      if (lane == 0) issue_q(cta_rows > rpt ? 2 : 1);
+      const int blk_k = lane < n_boxes ? table_entry(0, 0) : 0, blk_v = lane < n_boxes ? table_entry(1, 0) : 0;
+      issue_item(0, blk_k);
+      issue_item(1, blk_v);
+      blk_ahead = lane < n_boxes ? table_entry(2, 0) : 0;  // (clamped to a valid page if there is no key tile 1)
+    }
+  }
   // valid rows and number of key tiles of each query tile of row pair `pr`
   auto tile_info = [&](int pr, int (&nr)[2], int (&nt)[2]) {
     const int cta_rows = pr >= 0 ? min(rpc, n_r - pr * rpc) : 0;
@@ -241,7 +325,17 @@ attn_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_constant__ CU
   }
 
   tc_fence_before();
-  if (kPair) cluster_sync(); else __syncthreads();
+  if (kPair) {
+    if (warp != kWarpProd0) {
+      cluster_wait();  // (second half of the meeting after the barrier init)
+      cluster_arrive();
+    }
+    cluster_wait();
+  } else if (kZc != 0) {
+    __syncthreads();
+  } else if (warp != kWarpProd0) {
+    named_bar_sync(3, kAttnThreads);  // warp 8 has arrived already (before its early issue) and goes on
+  }
   tc_fence_after();
   const uint32_t tmem = bars->tmem_base;
 
@@ -252,67 +346,24 @@ attn_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_constant__ CU
     setmaxnreg_dec<56>();
     if (warp == kWarpProd0 || warp == kWarpProd1) {
       // ================================================================ TMA producers
-      // warp 0 loads Q and the even ring items, warp 2 the odd ones (PV variant: K tiles / V tiles);
-      // the block-table entries of a warp's next item are fetched before it waits for the free slot.
-      if (warp == kWarpProd0 && lane == 0) {
-        if (kPair) {
-          // both CTAs always load both query tiles (rows past the batch read as zeros; rows of another request
-          // are never stored), so rank 0's barrier expects a fixed byte count
-          const uint32_t qbar = mapa_u32(smem_u32(&bars->q_full), 0);
-          if (rank == 0) mbar_expect_tx(&bars->q_full, (uint32_t)(2 * 2 * 2 * rpt * g * 128));
-          for (int i = 0; i < 2; ++i) {
-            tma_load_3d_pair(smem + Cfg::kOffQ + i * kTileBytes, &tm_q, qbar, 0, kvh * g, row_base + i * rpt);
-            tma_load_3d_pair(smem + Cfg::kOffQ + i * kTileBytes + kHalfBytes, &tm_q, qbar, 64, kvh * g,
-                             row_base + i * rpt);
-          }
-        } else {
-          const int nq = nrows[1] > 0 ? 2 : 1;
-          mbar_expect_tx(&bars->q_full, (uint32_t)(nq * 2 * rpt * g * 128));
-          for (int i = 0; i < nq; ++i) {
-            tma_load_3d(smem + Cfg::kOffQ + i * kTileBytes, &tm_q, &bars->q_full, 0, kvh * g, row_base + i * rpt);
-            tma_load_3d(smem + Cfg::kOffQ + i * kTileBytes + kHalfBytes, &tm_q, &bars->q_full, 64, kvh * g,
-                        row_base + i * rpt);
-          }
-        }
-      }
-      // single CTA: lane = (page of the tile, 64-column half), 16 boxes per item.
-      // kPair: 8 boxes per item: K item = this CTA's 64 keys (4 pages) x both halves -> [half][64 keys][128 B],
-      //        the keys being 32 of each 64-key half of the tile: pages {2r, 2r+1, 4+2r, 5+2r} for rank r;
-      //        V item = all 8 pages x the CTA's own 64-column half -> [128 keys][128 B].
+      // warp 8 loads Q and the even ring items (K tiles), warp 10 the odd ones (V tiles); the block-table entries of a
+      // warp's next item are fetched right after it has issued the current one, so their latency hides behind the
+      // wait for the next free slot (fetched BEFORE the issue, the second fetch delayed the first issue by 1 300 clk).
       const int n_items = 2 * n_tiles;
-      const int pgi = lane >> 1;
-      const int pg_k = kPair ? 2 * rank + (pgi & 1) + 4 * (pgi >> 1) : pgi, half_k = lane & 1;
-      const int pg_v = kPair ? lane : (lane >> 1), half_v = kPair ? rank : (lane & 1);
-      const int n_boxes = kPair ? 8 : 16;
-      auto table_entry = [&](int it) -> int {
-        const int t = t0 + (it >> 1);
-        const bool is_v = it & 1;
-        int lp = t * 8 + (is_v ? pg_v : pg_k);
-        if (lp > n_pages - 1) lp = n_pages - 1;  // pages past the sequence: any valid page (keys are masked)
-        return (is_v ? p.v_table : p.k_table)[(size_t)req * p.max_pages + lp];
-      };
-      const uint32_t full0 = kPair ? mapa_u32(smem_u32(&bars->kv_full[0]), 0) : 0;
       int it = (warp == kWarpProd1) ? 1 : 0;
-      int blk = (it < n_items && lane < n_boxes) ? table_entry(it) : 0;
+      int blk = blk_ahead;
+      if (early) {
+        it += 2;  // items 0 and 1 are in flight (warp 8 holds the entry of item 2 already)
+        if (warp == kWarpProd1) blk = (it < n_items && lane < n_boxes) ? table_entry(it, t0) : 0;
+      } else {
+        if (warp == kWarpProd0 && lane == 0) issue_q(nrows[1] > 0 ? 2 : 1);
+        blk = (it < n_items && lane < n_boxes) ? table_entry(it, t0) : 0;
+      }
       for (; it < n_items; it += 2) {
-        const int blk_next = (it + 2 < n_items && lane < n_boxes) ? table_entry(it + 2) : 0;
-        const bool is_v = it & 1;
         const int s = it % kStages, u = it / kStages;
         mbar_wait_relaxed(&bars->kv_empty[s], (u & 1) ^ 1);   // the ring is several tiles deep: no hurry
-        if (lane == 0 && rank == 0) mbar_expect_tx(&bars->kv_full[s], kTileBytes);  // both CTAs' bytes
-        __syncwarp();
-        if (lane < n_boxes) {
-          const int row0 = (blk * p.num_kv_heads + kvh) * kPage;
-          if (kPair) {
-            uint8_t *dst = smem + Cfg::kOffKV + s * kStageBytes +
-                           (is_v ? pg_v * 2048 : half_k * (kHalfBytes / 2) + (lane >> 1) * 2048);
-            tma_load_2d_pair(dst, is_v ? &tm_v : &tm_k, full0 + s * 8, (is_v ? half_v : half_k) * 64, row0);
-          } else {
-            tma_load_2d(smem + Cfg::kOffKV + s * kTileBytes + half_k * kHalfBytes + pg_k * 2048,
-                        is_v ? &tm_v : &tm_k, &bars->kv_full[s], half_k * 64, row0);
-          }
-        }
-        blk = blk_next;
+        issue_item(it, blk);
+        blk = (it + 2 < n_items && lane < n_boxes) ? table_entry(it + 2, t0) : 0;
       }
     } else if (warp == kWarpMma) {
       // ================================================================ MMA issuer
@@ -670,26 +721,41 @@ attn_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_constant__ CU
       if (threadIdx.x == 0) split_depart(p.tickets + bid, p.kv_splits);
     } else if (my_tiles > 0) {
       {
+        // The CTA ends with this epilogue (the second query tile's, about a tile later than the first's), and the
+        // next CTA of the SM starts only then: all four TMEM loads in flight at once, and 32-byte stores -- a thread
+        // owns one output row of 256 B, so 16-byte stores of a warp hit 32 sectors each and fill only half of them
+        // (clock64 trace: 3 500 clk per warpgroup before).
         mbar_wait(&bars->o_full[qt], 0);
         tc_fence_after();
         const float inv = 1.f / (l + l_fix);
+        uint32_t o[4][32];
 #pragma unroll
-        for (int c = 0; c < 4; ++c) {
-          uint32_t o[32];
-          tmem_ld32(tmem_o + c * 32, o);
-          tmem_wait_ld();
-          if (valid) {
-            uint4 *dst = reinterpret_cast<uint4 *>(p.out + out_row * kHeadDim + c * 32);
+        for (int c = 0; c < 4; ++c) tmem_ld32(tmem_o + c * 32, o[c]);
+        tmem_wait_ld();
+        if (valid) {
+          uint8_t *dst = reinterpret_cast<uint8_t *>(p.out + out_row * kHeadDim);
+          const bool wide = (reinterpret_cast<uintptr_t>(p.out) & 31) == 0;  // (the ABI asks for 16-byte alignment only)
 #pragma unroll
-            for (int v4 = 0; v4 < 4; ++v4) {
-              uint4 v;
-              v.x = pack_bf16x2(__uint_as_float(o[v4 * 8 + 0]) * inv, __uint_as_float(o[v4 * 8 + 1]) * inv);
-              v.y = pack_bf16x2(__uint_as_float(o[v4 * 8 + 2]) * inv, __uint_as_float(o[v4 * 8 + 3]) * inv);
-              v.z = pack_bf16x2(__uint_as_float(o[v4 * 8 + 4]) * inv, __uint_as_float(o[v4 * 8 + 5]) * inv);
-              v.w = pack_bf16x2(__uint_as_float(o[v4 * 8 + 6]) * inv, __uint_as_float(o[v4 * 8 + 7]) * inv);
-              dst[v4] = v;
+          for (int c = 0; c < 4; ++c)
+#pragma unroll
+            for (int h8 = 0; h8 < 2; ++h8) {
+              uint4 v[2];
+#pragma unroll
+              for (int k = 0; k < 2; ++k) {
+                const int b = h8 * 16 + k * 8;
+                v[k].x = pack_bf16x2(__uint_as_float(o[c][b + 0]) * inv, __uint_as_float(o[c][b + 1]) * inv);
+                v[k].y = pack_bf16x2(__uint_as_float(o[c][b + 2]) * inv, __uint_as_float(o[c][b + 3]) * inv);
+                v[k].z = pack_bf16x2(__uint_as_float(o[c][b + 4]) * inv, __uint_as_float(o[c][b + 5]) * inv);
+                v[k].w = pack_bf16x2(__uint_as_float(o[c][b + 6]) * inv, __uint_as_float(o[c][b + 7]) * inv);
+              }
+              uint8_t *d32 = dst + c * 64 + h8 * 32;
+              if (wide) {
+                stg_256(d32, v[0], v[1]);
+              } else {
+                reinterpret_cast<uint4 *>(d32)[0] = v[0];
+                reinterpret_cast<uint4 *>(d32)[1] = v[1];
+              }
             }
-          }
         }
       }
       if (p.lse && valid) p.lse[out_row] = m_used * p.scale + logf(l);
