@@ -635,3 +635,24 @@ def test_pipe_probe_reports_plausible_rates():
     assert mufu < mix < 2.0 * mufu, (mufu, mix)          # the polynomial share adds to what MUFU alone retires
     with pytest.raises(sx.SparseXError):
         sx.probe_pipe(9)
+
+
+def test_attention_output_pointer_aligned_to_16_bytes_only():
+    """The ABI asks for 16-byte alignment of `out`; the epilogue of the tensor-core kernel stores 32 bytes per lane
+    when the pointer allows it and falls back to 16-byte stores otherwise: same bits either way."""
+    GpuLayer, dev_to_bits = _gpu()
+    from paper_2606_01751_b200 import binding as sx
+    lay, lt, res, pk, pv, kt, vt = prepared("C2-quarter")
+    g = GpuLayer(lay, lt)
+    g.step_sparse()
+    n, hq = int(g.rows_R.numel()), lay.num_q_heads
+    buf = torch.zeros(n * hq * 128 + 8, dtype=torch.int16, device=g.dev)
+    shifted = buf[8:].view(n, hq, 128)
+    assert shifted.data_ptr() % 32 == 16 and shifted.is_contiguous()
+    for pair in (False, True):
+        buf.zero_()
+        sx.sparse_attn(g.pool, g.batch, g.q_R, shifted, rows_R=g.rows_R, rows_off=g.rows_off, total_rows=n, cta_pair=pair)
+        ref = torch.zeros((n, hq, 128), dtype=torch.int16, device=g.dev)
+        sx.sparse_attn(g.pool, g.batch, g.q_R, ref, rows_R=g.rows_R, rows_off=g.rows_off, total_rows=n, cta_pair=pair)
+        torch.cuda.synchronize()
+        assert torch.equal(shifted, ref) and int(buf[:8].abs().sum()) == 0
