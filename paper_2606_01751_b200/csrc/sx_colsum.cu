@@ -61,6 +61,8 @@ struct ColsumParams {
   float scale_log2;
   const float2 *zc_table;     // zero-copy mode: (cos, sin) per segment and the page classification (sx_rotate.cuh)
   const int32_t *zc_page_seg;
+  int4 *plan;                 // [colsum grid][2] work record of every colsum CTA, written by coltab_kernel (see there)
+  int n_qt_blocks, cs_grid;   // coltab grid: blockIdx.x < n_qt_blocks build column rows, the rest build the plan
 };
 
 struct CsBars {
@@ -82,6 +84,47 @@ coltab_kernel(const ColsumParams p) {
   griddep_launch();  // programmatic dependent launch: the next kernel may become resident now ...
   griddep_wait();    // ... and this one touches global memory only after its predecessor has completed
   const int g = p.group, rpt = p.rows_per_tile;
+  if ((int)blockIdx.x >= p.n_qt_blocks) {
+    // ---- work records of the colsum CTAs: which (request, key tile, KV head) a CTA owns and which query tiles can
+    // see its keys is a serial walk over the requests plus two binary searches over new_idx -- a dozen DEPENDENT
+    // global loads (clock64 trace: 6 300 clk per CTA, a quarter of a C4 CTA's life). One thread per CTA does them
+    // here, once; the CTA then starts from a single 32-byte load.
+    const int cta = (((int)blockIdx.x - p.n_qt_blocks) * (int)gridDim.y + (int)blockIdx.y) * 128 + (int)threadIdx.x;
+    if (cta >= p.cs_grid) return;
+    int req = 0, base = 0, ktiles = 0, qt_base = 0;  // qt_base: query tiles of the requests before this one
+    for (; req < p.num_reqs; ++req) {
+      ktiles = (p.seq_len[req] + kTile - 1) / kTile;
+      if (cta < base + ktiles * p.num_kv_heads) break;
+      base += ktiles * p.num_kv_heads;
+      qt_base += (p.new_off[req + 1] - p.new_off[req] + rpt - 1) / rpt;
+    }
+    int4 r0 = make_int4(-1, 0, 0, 0), r1 = make_int4(0, 0, 0, 0);
+    if (req < p.num_reqs) {
+      const int local = cta - base;
+      const int kvh = local % p.num_kv_heads, kt = local / p.num_kv_heads;  // early key tiles (seen by the most queries) first
+      const int j0 = kt * kTile;
+      const int nq0 = p.new_off[req], nn = p.new_off[req + 1] - nq0;
+      int lo = 0, hi = nn;  // first Sparse-Q query that can see key j0: lower_bound(new_idx, j0)
+      while (lo < hi) {
+        const int mid = (lo + hi) >> 1;
+        if (p.new_idx[nq0 + mid] < j0) lo = mid + 1; else hi = mid;
+      }
+      const int qt0 = lo / rpt;  // first query tile with a visible query
+      const int n_it = (lo < nn) ? (nn + rpt - 1) / rpt - qt0 : 0;
+      // queries are sorted by position: only the leading tiles, whose first query sits below the tile's last key,
+      // need a causal mask: tiles it < n_mask (first query index (qt0 + it) * rpt below lower_bound(new_idx, j0 + 127))
+      int lo2 = lo, hi2 = nn;
+      while (lo2 < hi2) {
+        const int mid = (lo2 + hi2) >> 1;
+        if (p.new_idx[nq0 + mid] < j0 + kTile - 1) lo2 = mid + 1; else hi2 = mid;
+      }
+      r0 = make_int4(req, kt | (kvh << 24), p.seq_len[req], nq0 + qt0 * rpt);
+      r1 = make_int4(n_it, max(0, (lo2 + rpt - 1) / rpt - qt0), qt_base + qt0, p.tok_off[req]);
+    }
+    p.plan[2 * cta] = r0;
+    p.plan[2 * cta + 1] = r1;
+    return;
+  }
   int req = 0, base = 0;
   for (; req < p.num_reqs; ++req) {
     const int nq = (p.new_off[req + 1] - p.new_off[req] + rpt - 1) / rpt;
@@ -174,46 +217,12 @@ colsum_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_constant__ 
   uint8_t *smem = reinterpret_cast<uint8_t *>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~uintptr_t(1023));
   CsBars *bars = reinterpret_cast<CsBars *>(smem + kCsOffBar);
   uint8_t *col_sm = smem + kCsOffCol;  // [kCsColStages] rows of kCsColRow bytes: (lse2[128],) position[128]
-  griddep_launch();
-  griddep_wait();
-
-  // ---- (request, key tile, KV head); early key tiles (seen by the most queries) first
   const int g = p.group, rpt = p.rows_per_tile;
-  int req = 0, base = 0, ktiles = 0, qt_base = 0;  // qt_base: query tiles of the requests before this one
-  for (; req < p.num_reqs; ++req) {
-    ktiles = (p.seq_len[req] + kTile - 1) / kTile;
-    if ((int)blockIdx.x < base + ktiles * p.num_kv_heads) break;
-    base += ktiles * p.num_kv_heads;
-    qt_base += (p.new_off[req + 1] - p.new_off[req] + rpt - 1) / rpt;
-  }
-  if (req >= p.num_reqs) return;
-  const int local = blockIdx.x - base;
-  const int kvh = local % p.num_kv_heads;
-  const int kt = local / p.num_kv_heads;
-  const int T = p.seq_len[req];
-  const int j0 = kt * kTile;
-  const int n_pages = (T + kPage - 1) / kPage;
-  const int nq0 = p.new_off[req], nn = p.new_off[req + 1] - nq0;
-  // first Sparse-Q query that can see key j0: lower_bound(new_idx, j0)
-  int lo = 0, hi = nn;
-  while (lo < hi) {
-    int mid = (lo + hi) >> 1;
-    if (p.new_idx[nq0 + mid] < j0) lo = mid + 1; else hi = mid;
-  }
-  const int qt0 = lo / rpt;                          // first query tile with a visible query
-  const int n_qt = (nn + rpt - 1) / rpt;
-  const int n_it = (lo < nn) ? n_qt - qt0 : 0;
-  // queries are sorted by position: only the leading tiles, whose first query sits below the tile's last key, need a
-  // causal mask. n_mask = tiles it < n_mask (first query index (qt0 + it) * rpt below lower_bound(new_idx, j0 + 127))
-  int lo2 = lo, hi2 = nn;
-  while (lo2 < hi2) {
-    int mid = (lo2 + hi2) >> 1;
-    if (p.new_idx[nq0 + mid] < j0 + kTile - 1) lo2 = mid + 1; else hi2 = mid;
-  }
-  const int n_mask = max(0, (lo2 + rpt - 1) / rpt - qt0);
-
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
   constexpr int kWarpProd = 8, kWarpMma = 9;
+
+  // ---- prologue without global memory (may overlap the previous kernel: programmatic dependent launch)
+  griddep_launch();
   if (warp == kWarpProd && lane == 0) {
     tma_prefetch_desc(&tm_q);
     tma_prefetch_desc(&tm_k);
@@ -253,10 +262,26 @@ colsum_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_constant__ 
     }
     fence_proxy_async_smem();
   }
-  tc_fence_before();
-  __syncthreads();
-  tc_fence_after();
-  const uint32_t tmem = bars->tmem_base;
+  griddep_wait();
+
+  // ---- this CTA's work record (coltab_kernel): (request, key tile, KV head), the query tiles that see its keys
+  // (plain loads: the record is an OUTPUT of the preceding kernel, and under programmatic dependent launch this CTA
+  // may have become resident before that kernel wrote it -- the read-only (.nc) path must not be used for it)
+  const int4 w0 = p.plan[2 * blockIdx.x], w1 = p.plan[2 * blockIdx.x + 1];
+  const int req = w0.x, kt = w0.y & 0xFFFFFF, kvh = w0.y >> 24, T = w0.z, r_first = w0.w;
+  const int n_it = req >= 0 ? w1.x : 0, n_mask = w1.y, qt_first = w1.z, tok0 = w1.w;
+  const int j0 = kt * kTile;
+  const int n_pages = (T + kPage - 1) / kPage;
+
+  // The producer warp does not wait for the others: it initialised the barriers itself and needs neither TMEM nor
+  // the operand rows the others zero, so it ARRIVES at the block-wide meeting and starts loading at once.
+  if (warp == kWarpProd) named_bar_arrive(2, kCsThreads);
+  else {
+    tc_fence_before();
+    named_bar_sync(2, kCsThreads);
+    tc_fence_after();
+  }
+  const uint32_t tmem = bars->tmem_base;  // (not used by the producer warp)
 
   if (warp == kWarpProd) {
     // ================================================================ TMA producer
@@ -277,12 +302,12 @@ colsum_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_constant__ 
         for (int it = 0; it < n_it; ++it) {
           mbar_wait(&bars->q_empty[s], ph);
           mbar_expect_tx(&bars->q_full[s], (uint32_t)(2 * rpt * g * 128 + kCsExtBytes));
-          const int r0 = nq0 + (qt0 + it) * rpt;
+          const int r0 = r_first + it * rpt;
           uint8_t *qs = smem + kCsOffQ + s * kCsQStage;
           tma_load_3d(qs, &tm_q, &bars->q_full[s], 0, kvh * g, r0);
           tma_load_3d(qs + kCsHalf, &tm_q, &bars->q_full[s], 64, kvh * g, r0);
           const uint8_t *entry = reinterpret_cast<const uint8_t *>(p.col_tab) +
-                                 ((size_t)(qt_base + qt0 + it) * p.num_kv_heads + kvh) * kCsTabEntry;
+                                 ((size_t)(qt_first + it) * p.num_kv_heads + kvh) * kCsTabEntry;
           // Column row of this query tile, own ring: this thread is at most 2 tiles ahead of the MMA issuer, which is
           // at most 2 tiles ahead of the consumers' D loads, so 5 slots suffice.
           const int cs = it % kCsColStages;
@@ -377,7 +402,7 @@ colsum_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_constant__ 
     const float acc = acc2.x + acc2.y;
     if (hf == 1) xch[row] = acc;
     named_bar_sync(1, 256);
-    if (hf == 0 && j < T) p.partial[(size_t)kvh * p.total_tokens + p.tok_off[req] + j] = acc + xch[row];
+    if (hf == 0 && j < T) p.partial[(size_t)kvh * p.total_tokens + tok0 + j] = acc + xch[row];
   }
 
   tc_fence_before();
@@ -388,7 +413,9 @@ colsum_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_constant__ 
 size_t colsum_tab_bytes(const sx_pool *pool, const sx_batch *b) {
   const int g = pool->num_q_heads / pool->num_kv_heads;
   const int rpt = kTile / (g > 0 ? g : 1) > 0 ? kTile / (g > 0 ? g : 1) : 1;
-  return (size_t)(b->total_new / rpt + b->num_reqs) * pool->num_kv_heads * kCsTabEntry;
+  const size_t entries = (size_t)(b->total_new / rpt + b->num_reqs) * pool->num_kv_heads * kCsTabEntry;
+  const size_t plan = (size_t)(b->total_tokens / kTile + b->num_reqs) * pool->num_kv_heads * 2 * sizeof(int4);
+  return entries + plan;  // column entries, then one 32-byte work record per colsum CTA
 }
 
 sx_status launch_colsum(const sx_pool *pool, const sx_batch *b, const void *q_new, const float *lse_new,
@@ -428,7 +455,11 @@ sx_status launch_colsum(const sx_pool *pool, const sx_batch *b, const void *q_ne
   cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, kCsSmemBytes);
   if (e != cudaSuccess) return set_error(SX_ERR_CUDA, "colsum smem attr: %s", cudaGetErrorString(e));
   const int n_qt = b->total_new / rpt + b->num_reqs;  // >= sum_r ceil(|I_nr(r)| / rpt)
-  e = launch_pdl(coltab_kernel, dim3(n_qt, pool->num_kv_heads), dim3(128), 0, st, 1, p);
+  p.plan = reinterpret_cast<int4 *>(reinterpret_cast<uint8_t *>(col_tab) + (size_t)n_qt * pool->num_kv_heads * kCsTabEntry);
+  p.n_qt_blocks = n_qt;
+  p.cs_grid = grid;
+  const int plan_blocks = (grid + 128 * pool->num_kv_heads - 1) / (128 * pool->num_kv_heads);
+  e = launch_pdl(coltab_kernel, dim3(n_qt + plan_blocks, pool->num_kv_heads), dim3(128), 0, st, 1, p);
   if (e != cudaSuccess) return set_error(SX_ERR_CUDA, "coltab launch: %s", cudaGetErrorString(e));
   s = check_launch("coltab_kernel");
   if (s != SX_OK) return s;

@@ -366,6 +366,32 @@ __device__ __forceinline__ float lds_f1(uint32_t saddr) {
 // its writes are visible); everything before the wait (barrier init, TMEM allocation, tensor-map prefetch) overlaps
 // the predecessor's tail. Without the launch attribute both are no-ops.
 __device__ __forceinline__ void griddep_wait() { asm volatile("griddepcontrol.wait;" ::: "memory"); }
+// Loads of data that a PRECEDING KERNEL of the stream may have written (workspace intermediates, block tables, row
+// lists, normalisers): they must not take the read-only path (ld.global.nc: what `__ldg` and `const __restrict__`
+// pointers compile to). Under programmatic dependent launch a CTA of this kernel can be resident before the
+// predecessor has written the data, and the read-only cache of its SM may then serve a line from BEFORE that write
+// (seen: a colsum CTA read a stale work record that coltab_kernel had just rewritten at the same workspace address).
+// These are plain, coherent loads, and being `asm volatile` they also stay behind griddep_wait().
+__device__ __forceinline__ int ld_dep(const int *p) {
+  int v;
+  asm volatile("ld.global.b32 %0, [%1];" : "=r"(v) : "l"(p) : "memory");
+  return v;
+}
+__device__ __forceinline__ float ld_dep(const float *p) {
+  float v;
+  asm volatile("ld.global.f32 %0, [%1];" : "=f"(v) : "l"(p) : "memory");
+  return v;
+}
+__device__ __forceinline__ int4 ld_dep(const int4 *p) {
+  int4 v;
+  asm volatile("ld.global.v4.b32 {%0, %1, %2, %3}, [%4];" : "=r"(v.x), "=r"(v.y), "=r"(v.z), "=r"(v.w) : "l"(p) : "memory");
+  return v;
+}
+__device__ __forceinline__ float4 ld_dep(const float4 *p) {
+  float4 v;
+  asm volatile("ld.global.v4.f32 {%0, %1, %2, %3}, [%4];" : "=f"(v.x), "=f"(v.y), "=f"(v.z), "=f"(v.w) : "l"(p) : "memory");
+  return v;
+}
 __device__ __forceinline__ void griddep_launch() { asm volatile("griddepcontrol.launch_dependents;" ::: "memory"); }
 
 // ------------------------------------------------------------------------------------ misc math

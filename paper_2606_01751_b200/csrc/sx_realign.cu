@@ -37,14 +37,14 @@ __global__ void rope_table_kernel(const sx_segment *__restrict__ segs, int num_s
     }
     const sx_segment sg = segs[lo];
     const int lpage = sg.new_pos / kPage + (idx - sg.src_off);
-    page_desc[idx] = make_int4(lo, src_blocks[idx], k_table[(size_t)sg.req * max_pages + lpage],
-                               v_table[(size_t)sg.req * max_pages + lpage]);
+    page_desc[idx] = make_int4(lo, src_blocks[idx], ld_dep(k_table + (size_t)sg.req * max_pages + lpage),
+                               ld_dep(v_table + (size_t)sg.req * max_pages + lpage));  // (tables: a scatter may just have flipped them)
   }
 }
 
 __device__ __forceinline__ uint4 ld_stream(const uint4 *p) {
   uint4 r;
-  asm volatile("ld.global.nc.L1::no_allocate.v4.u32 {%0, %1, %2, %3}, [%4];"
+  asm volatile("ld.global.L1::no_allocate.v4.u32 {%0, %1, %2, %3}, [%4];"
                : "=r"(r.x), "=r"(r.y), "=r"(r.z), "=r"(r.w)
                : "l"(p));
   return r;
@@ -74,7 +74,7 @@ realign_kernel(const __grid_constant__ LayerPools pools, int num_kv_heads, const
   const int page = blockIdx.x, h = blockIdx.y;
   const uint4 *pool_k_src = pools.k[blockIdx.z], *pool_v_src = pools.v[blockIdx.z];
   uint4 *pool_k_dst = pools.k[blockIdx.z], *pool_v_dst = pools.v[blockIdx.z];
-  const int4 d = __ldg(page_desc + page);  // (segment, source page, destination K page, destination V page)
+  const int4 d = ld_dep(page_desc + page);  // (segment, source page, destination K page, destination V page)
   const size_t tile = (size_t)kPage * 16;  // 16-byte chunks of one (page, head) tile
   const uint4 *ks = pool_k_src + ((size_t)d.y * num_kv_heads + h) * tile;
   uint4 *kd = pool_k_dst + ((size_t)d.z * num_kv_heads + h) * tile;
@@ -96,7 +96,7 @@ realign_kernel(const __grid_constant__ LayerPools pools, int num_kv_heads, const
     const float4 *tp = reinterpret_cast<const float4 *>(table + d.x * 64 + c * 8);
 #pragma unroll
     for (int i = 0; i < 4; ++i) {
-      const float4 f = __ldg(tp + i);
+      const float4 f = ld_dep(tp + i);
       cs[2 * i] = make_float2(f.x, f.y);
       cs[2 * i + 1] = make_float2(f.z, f.w);
     }
@@ -119,7 +119,7 @@ realign_kernel(const __grid_constant__ LayerPools pools, int num_kv_heads, const
     const float4 *tp = reinterpret_cast<const float4 *>(table + d.x * 64 + (t & 15) * 4);
 #pragma unroll
     for (int i = 0; i < 2; ++i) {
-      const float4 f = __ldg(tp + i);
+      const float4 f = ld_dep(tp + i);
       cs[2 * i] = make_float2(f.x, f.y);
       cs[2 * i + 1] = make_float2(f.z, f.w);
     }
@@ -155,7 +155,7 @@ __global__ void zc_prepare_kernel(const sx_segment *__restrict__ segs, int num_s
     int m = -1;
     if (lp * kPage < seq_len[req]) {
       m = find_segment(segs, num_segments, req, lp * kPage);
-      if (m >= 0 && k_table[idx] != src_blocks[segs[m].src_off + lp - segs[m].new_pos / kPage]) m = -1;
+      if (m >= 0 && ld_dep(k_table + idx) != src_blocks[segs[m].src_off + lp - segs[m].new_pos / kPage]) m = -1;
     }
     page_seg[idx] = m;
   }

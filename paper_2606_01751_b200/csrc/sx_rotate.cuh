@@ -78,13 +78,13 @@ __device__ __forceinline__ void rotate_k_tile(uint8_t *tile, int half_bytes, con
     float2 cs[8];
     for (int r = tid >> 3; r < kTile; r += NTHREADS / 8) {
       const int pg = r >> 4;
-      const int m = pg < n_valid ? __ldg(page_seg8 + pg) : -1;
+      const int m = pg < n_valid ? ld_dep(page_seg8 + pg) : -1;
       if (m < 0) continue;
       if (m != m_prev) {
         const float4 *tp = reinterpret_cast<const float4 *>(table + m * 64 + c * 8);
 #pragma unroll
         for (int i = 0; i < 4; ++i) {
-          const float4 f = __ldg(tp + i);
+          const float4 f = ld_dep(tp + i);
           cs[2 * i] = make_float2(f.x, f.y);
           cs[2 * i + 1] = make_float2(f.z, f.w);
         }
@@ -102,13 +102,13 @@ __device__ __forceinline__ void rotate_k_tile(uint8_t *tile, int half_bytes, con
     float2 cs[4];
     for (int r = tid >> 4; r < kTile; r += NTHREADS / 16) {
       const int pg = r >> 4;
-      const int m = pg < n_valid ? __ldg(page_seg8 + pg) : -1;
+      const int m = pg < n_valid ? ld_dep(page_seg8 + pg) : -1;
       if (m < 0) continue;
       if (m != m_prev) {
         const float4 *tp = reinterpret_cast<const float4 *>(table + m * 64 + c16 * 4);
 #pragma unroll
         for (int i = 0; i < 2; ++i) {
-          const float4 f = __ldg(tp + i);
+          const float4 f = ld_dep(tp + i);
           cs[2 * i] = make_float2(f.x, f.y);
           cs[2 * i + 1] = make_float2(f.z, f.w);
         }

@@ -19,7 +19,7 @@ __device__ __forceinline__ int find_req(const int32_t *__restrict__ off, int num
   int lo = 0, hi = num_reqs - 1;
   while (lo < hi) {
     const int mid = (lo + hi + 1) >> 1;
-    if (__ldg(off + mid) <= n) lo = mid; else hi = mid - 1;
+    if (ld_dep(off + mid) <= n) lo = mid; else hi = mid - 1;
   }
   return lo;
 }
@@ -37,7 +37,7 @@ __device__ __forceinline__ void scatter_row(uint4 *pool_k, uint4 *pool_v, int nu
     for (int i = 0; i < kScatterMaxChunks; ++i) {
       const int c = lane + 32 * i;
       if (c < row_chunks) {
-        a[i] = __ldg(ks + c);
+        a[i] = __ldg(ks + c);  // (read-only path: the fresh rows are inputs of the call, never written by this library)
         b[i] = __ldg(vs + c);
       }
     }
@@ -149,9 +149,9 @@ scatter_kernel(uint4 *pool_k, uint4 *pool_v, int num_kv_heads, int num_reqs, int
   griddep_wait();    // the row list / the pool may be outputs of the previous kernel
   const int n = blockIdx.x * kScatterWarps + (threadIdx.x >> 5);
   const int lane = threadIdx.x & 31;
-  if (n >= __ldg(rows_off + num_reqs)) return;
+  if (n >= ld_dep(rows_off + num_reqs)) return;
   const int req = find_req(rows_off, num_reqs, n);
-  const int p = __ldg(rows + n);
+  const int p = ld_dep(rows + n);
   const int pg = p / kPage;
   const size_t e = (size_t)req * max_pages + pg;
   const int row_chunks = num_kv_heads * 16;
@@ -161,7 +161,7 @@ scatter_kernel(uint4 *pool_k, uint4 *pool_v, int num_kv_heads, int num_reqs, int
     return;
   }
   // copy-on-write: the warp of the FIRST listed row of a page owns the page (rows are ascending inside a request)
-  if (n > __ldg(rows_off + req) && __ldg(rows + n - 1) / kPage == pg) return;
+  if (n > ld_dep(rows_off + req) && ld_dep(rows + n - 1) / kPage == pg) return;
   const int priv = cow_private[e];
   int kb = k_table[e], vb = v_table[e];
   if (priv >= 0) {
@@ -190,9 +190,9 @@ scatter_kernel(uint4 *pool_k, uint4 *pool_v, int num_kv_heads, int num_reqs, int
     }
     kb = vb = priv;
   }
-  const int n_end = __ldg(rows_off + req + 1);
+  const int n_end = ld_dep(rows_off + req + 1);
   for (int m = n; m < n_end; ++m) {
-    const int q = __ldg(rows + m);
+    const int q = ld_dep(rows + m);
     if (q / kPage != pg) break;
     scatter_row(pool_k, pool_v, num_kv_heads, kb, vb, q % kPage, k_fresh + (size_t)m * row_chunks,
                 v_fresh + (size_t)m * row_chunks, lane);

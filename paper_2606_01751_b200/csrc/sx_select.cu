@@ -59,7 +59,7 @@ score_sum_kernel(int num_kv_heads, int total_tokens, const float *__restrict__ p
   const int j = blockIdx.x * 256 + threadIdx.x;
   if (j >= total_tokens) return;
   float s = 0.f;
-  for (int h = 0; h < num_kv_heads; ++h) s += partial[(size_t)h * total_tokens + j];
+  for (int h = 0; h < num_kv_heads; ++h) s += ld_dep(partial + (size_t)h * total_tokens + j);  // (colsum's output)
   scores[j] = s;
 }
 
@@ -181,7 +181,7 @@ select_kernel(int num_kv_heads, int total_tokens, const int32_t *__restrict__ se
 #pragma unroll
         for (int q = 0; q < 8; ++q) {
           const int j = j0 + q * kSelThreads + threadIdx.x;
-          u[q] = j < je ? __float_as_uint(scores[off + j]) : 0u;
+          u[q] = j < je ? __float_as_uint(ld_dep(scores + off + j)) : 0u;  // (score_sum's output)
         }
 #pragma unroll
         for (int q = 0; q < 8; ++q) {
@@ -279,7 +279,7 @@ select_kernel(int num_kv_heads, int total_tokens, const int32_t *__restrict__ se
 #pragma unroll
     for (int q = 0; q < kB; ++q) {
       const int j = j0 + q * 32 + lane;
-      u[q] = j < j_hi ? __float_as_uint(scores[off + j]) : 0u;
+      u[q] = j < j_hi ? __float_as_uint(ld_dep(scores + off + j)) : 0u;
     }
   };
   auto flags = [&](int j, uint32_t u, bool &isn, bool &gt, bool &eq, bool &frc) {
@@ -379,8 +379,8 @@ compact_rows_kernel(int num_reqs, const int32_t *__restrict__ tok_off, const int
   griddep_wait();
   int out = 0;
   for (int r = 0; r < num_reqs; ++r) {
-    const int n = cnt[r], src = tok_off[r];
-    for (int i = threadIdx.x; i < n; i += kSelThreads) rows_R[out + i] = tmp[src + i];
+    const int n = ld_dep(cnt + r), src = tok_off[r];  // (cnt, tmp: select_kernel's outputs)
+    for (int i = threadIdx.x; i < n; i += kSelThreads) rows_R[out + i] = ld_dep(tmp + src + i);
     if (threadIdx.x == 0) rows_off_out[r] = out;
     out += n;
   }

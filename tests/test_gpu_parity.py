@@ -656,3 +656,50 @@ def test_attention_output_pointer_aligned_to_16_bytes_only():
         sx.sparse_attn(g.pool, g.batch, g.q_R, ref, rows_R=g.rows_R, rows_off=g.rows_off, total_rows=n, cta_pair=pair)
         torch.cuda.synchronize()
         assert torch.equal(shifted, ref) and int(buf[:8].abs().sum()) == 0
+
+
+def test_one_workspace_reused_by_different_batches_back_to_back():
+    """Two batches of the same shape but different content (other deltas, other positions of the new tokens, other
+    block tables) take turns on ONE workspace without any synchronisation in between. Every intermediate a kernel
+    reads from the workspace (rotation table, page descriptors, work records, column tables, partial scores, row
+    lists) was written moments earlier by the preceding kernel at an address that still holds the OTHER batch's
+    values in some SM's read-only cache: under programmatic dependent launch a kernel that read them through the
+    read-only path (ld.global.nc) got the stale ones (found with the colsum work records; include/sparsex.h, ld_dep
+    in sx_ptx.cuh). Both batches must keep giving their own oracle results."""
+    GpuLayer, dev_to_bits = _gpu()
+    # four requests of 1.5-3K tokens (about 700 column-sum CTAs: every SM sees several work records per call); batch B
+    # = the requests of A in reverse order over a pool with other old positions: same sizes, other content everywhere
+    lens = [512, 768, 256, 1024, 384, 640]
+    pool_a = [wl.PoolSegment(n, 16 * (7 * i + 3)) for i, n in enumerate(lens)]
+    pool_b = [wl.PoolSegment(n, 16 * (5 * i + 40)) for i, n in enumerate(lens)]
+    reqs_a = [[("seg", 0), ("new", 128), ("seg", 3), ("new", 256), ("seg", 1), ("new", 64)],
+              [("new", 64), ("seg", 2), ("seg", 4), ("new", 512), ("seg", 5), ("new", 37)],
+              [("seg", 5), ("new", 256), ("seg", 0), ("new", 128)],
+              [("new", 192), ("seg", 1), ("new", 64), ("seg", 3), ("seg", 2), ("new", 320)]]
+    reqs_b = reqs_a[::-1]
+    ratios = [0.1, 0.25, 0.15, 0.2]
+    lays = [wl.build_layout("ws-a", 41, 8, 2, 500000.0, pool_a, reqs_a, ratios, 0.05),
+            wl.build_layout("ws-b", 42, 8, 2, 500000.0, pool_b, reqs_b, ratios[::-1], 0.05)]
+    cases = []
+    for lay in lays:
+        lt = wl.build_layer(lay, 0)
+        carve_margins(lay, lt)
+        cases.append((lay, lt, oracle_layer(lay, lt, mode="sparse")[0]))
+    gs = [GpuLayer(lay, lt) for lay, lt, _ in cases]
+    ws = gs[0].batch.workspace(gs[0].pool)
+    assert gs[1].batch.workspace(gs[1].pool).numel() == ws.numel()      # same shape, same workspace layout
+    gs[1].batch._ws = ws
+    pools0 = [(g.pool_k.clone(), g.pool_v.clone()) for g in gs]
+    for rep in range(4):
+        for g, (pk0, pv0) in zip(gs, pools0):
+            g.pool_k.copy_(pk0)
+            g.pool_v.copy_(pv0)
+            g.step_sparse()                 # no synchronisation between the two batches
+        torch.cuda.synchronize()
+        for g, (lay, lt, res) in zip(gs, cases):
+            sel, rows = g.sel_idx.cpu().numpy(), g.rows_R.cpu().numpy()
+            out = orc.bf16_to_f64(dev_to_bits(g.out))
+            for r in range(lay.num_reqs):
+                assert np.array_equal(sel[g.sel_off_h[r]:g.sel_off_h[r + 1]], res.sel[r]), (rep, lay.name, r)
+                assert np.array_equal(rows[g.rows_off_h[r]:g.rows_off_h[r + 1]], res.rows[r]), (rep, lay.name, r)
+                check_close("%s rep %d req %d O" % (lay.name, rep, r), out[g.rows_off_h[r]:g.rows_off_h[r + 1]], res.out[r])
