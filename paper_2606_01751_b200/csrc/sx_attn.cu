@@ -677,7 +677,7 @@ attn_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_constant__ CU
     // ---- epilogue
     const size_t out_row = (size_t)grow * p.num_q_heads + kvh * g + hh;
     if (p.kv_splits > 1) {
-      // key split: normalised partial O in fp32 and its log-sum-exp go to the workspace (attn_merge_kernel)
+      // key split: normalised partial O in fp32 and its log-sum-exp go to the scratch (merged below, in this launch)
       const size_t prow = (size_t)split * p.total_rows * p.num_q_heads + out_row;
       float4 *dst = reinterpret_cast<float4 *>(p.part_o + prow * kHeadDim);
       if (my_tiles > 0) {
@@ -774,9 +774,10 @@ attn_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_constant__ CU
 
 // Row sets that fill tensor-core tiles but only a few CTAs (a handful of query tiles against a long context):
 // cut the key range so that ONE wave of CTAs exists (225 KB of shared memory: one CTA per SM; a few CTAs
-// spilling into a second wave would double the time); the partial results are merged by the split that finishes
-// splits themselves once all of a row pair have arrived (split_arrive / merge_splits). The partial buffer bounds splits * total_rows * Hq (each CTA covers at most
-// 256 (row, head) pairs); one ticket word per (request, KV head, row pair) follows it.
+// spilling into a second wave would double the time); the partial results are merged by the splits themselves once
+// all splits of a row pair have arrived (split_arrive / merge_splits). The partial buffer bounds
+// splits * total_rows * Hq (each CTA covers at most 256 (row, head) pairs); one ticket word per (request, KV head,
+// row pair) follows it (or sits wherever launch_attn's `tickets` argument says: sx_attn_noalloc.cu).
 constexpr int kAttnSplitCtas = 148;
 constexpr size_t kAttnPartFloats = (size_t)2 * kAttnSplitCtas * 256 * (kHeadDim + 1);
 size_t attn_part_bytes() { return kAttnPartFloats * sizeof(float) + kAttnSplitCtas * sizeof(unsigned long long); }
