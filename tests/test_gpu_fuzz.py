@@ -300,3 +300,64 @@ def test_random_layout_extended_selection(seed):
         check_close("fuzz %d ex req %d O" % (seed, r), out[r0:r1], ref)
         check_close("fuzz %d ex zero-copy req %d O" % (seed, r), zout[r0:r1], ref)
     assert np.array_equal(dev_to_bits(g.pool_k), pk) and np.array_equal(dev_to_bits(g.pool_v), pv)
+
+
+def random_layout_medium(seed: int) -> wl.Layout:
+    """Random shapes at a few thousand tokens per request: long enough for the multi-CTA (cooperative) top-k, many key
+    tiles per CTA, several query tiles per request and segment deltas of thousands of positions."""
+    rng = np.random.default_rng(20000 + seed)
+    hkv = int(rng.choice([2, 4, 8]))
+    g = int(rng.choice([1, 4, 7]))
+    n_pool = int(rng.integers(3, 7))
+    pool = [wl.PoolSegment(16 * int(rng.integers(32, 161)), 16 * int(rng.integers(0, 600))) for _ in range(n_pool)]
+    num_reqs = int(rng.choice([1, 2, 3]))
+    reqs, ratios = [], []
+    for r in range(num_reqs):
+        spec = [("prefix", 16 * int(rng.integers(1, 9)))] if rng.random() < 0.3 else []
+        for _ in range(int(rng.integers(3, 7))):
+            spec.append(("seg", int(rng.integers(0, n_pool))) if rng.random() < 0.6 else ("new", 16 * int(rng.integers(2, 20))))
+        spec.append(("new", 16 * int(rng.integers(2, 12)) + int(rng.integers(0, 16))))
+        reqs.append(spec)
+        ratios.append(float(rng.choice([0.05, 0.1, 0.25])))
+    return wl.build_layout("fuzz-m%d" % seed, 500 + seed, g * hkv, hkv, 500000.0, pool, reqs, ratios, 0.05,
+                           cow=bool(seed & 1), rope_style=int(rng.integers(0, 2)))
+
+
+@pytest.mark.parametrize("seed", [0, 1, 2, 3, 4, 5])
+def test_random_layout_medium_sparse_layer(seed):
+    """Stage-isolated sparse layer and its zero-copy twin on medium-size random layouts (see random_layout_medium)."""
+    from paper_2606_01751_b200.layer import GpuLayer, dev_to_bits
+    lay = random_layout_medium(seed)
+    lt = wl.build_layer(lay, 0)
+    try:
+        carve_margins(lay, lt, max_iter=20)
+    except RuntimeError as e:
+        pytest.skip("margin carving: %s" % e)
+    res, pk, pv, kt, vt = oracle_layer(lay, lt, mode="sparse")
+    pk_a, pv_a = lt.pool_k.copy(), lt.pool_v.copy()
+    kt_a, vt_a = lay.k_block_table.copy(), lay.v_block_table.copy()
+    orc.realign(pk_a, pv_a, kt_a, vt_a, lay.segments, lay.src_blocks, lay.rope_theta, lay.rope_style)
+    g = GpuLayer(lay, lt)
+    g.realign()
+    torch.cuda.synchronize()
+    a64, b64 = orc.bf16_to_f64(dev_to_bits(g.pool_k)), orc.bf16_to_f64(pk_a)
+    assert np.all(np.abs(a64 - b64) <= 2.0 ** -7 * np.abs(b64) + 1e-5)
+    g.pool_k.copy_(torch.from_numpy(pk_a.view(np.int16)))
+    g.step_sparse(do_realign=False)
+    z = GpuLayer(wl.zero_copy_layout(lay), lt)
+    z.step_sparse(do_realign=False)
+    torch.cuda.synchronize()
+    sel, rows = g.sel_idx.cpu().numpy(), g.rows_R.cpu().numpy()
+    assert np.array_equal(z.sel_idx.cpu().numpy(), sel) and np.array_equal(z.rows_R.cpu().numpy(), rows)
+    out, zout = orc.bf16_to_f64(dev_to_bits(g.out)), orc.bf16_to_f64(dev_to_bits(z.out))
+    lse = g.lse.cpu().numpy().astype(np.float64)
+    for r in range(lay.num_reqs):
+        s0, s1 = g.sel_off_h[r], g.sel_off_h[r + 1]
+        r0, r1 = g.rows_off_h[r], g.rows_off_h[r + 1]
+        assert np.array_equal(sel[s0:s1], res.sel[r]), (seed, r)
+        assert np.array_equal(rows[r0:r1], res.rows[r]), (seed, r)
+        check_close("fuzz-m %d req %d O" % (seed, r), out[r0:r1], res.out[r])
+        check_close("fuzz-m %d zero-copy req %d O" % (seed, r), zout[r0:r1], res.out[r])
+        assert np.max(np.abs(lse[r0:r1] - res.lse[r])) < LSE_TOL
+    assert np.array_equal(g.batch.k_block_table.cpu().numpy(), kt) and np.array_equal(g.batch.v_block_table.cpu().numpy(), vt)
+    assert np.array_equal(dev_to_bits(g.pool_k), pk) and np.array_equal(dev_to_bits(g.pool_v), pv)
