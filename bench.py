@@ -782,13 +782,13 @@ def run_e2e(torch, sx, du, lay, layers, batch, all_rows, sel_holder, stack, args
 #   "measured"  : workloads the oracle FINISHES -- the whole C1 layer and request 0 of C2 --, every stage
 #                 timed by wall clock, nothing scaled ("estimated": false);
 #   "estimated" : the headline config. One bounded, FIXED-SIZE sample of it is timed (realign of one segment,
-#                 scatter of 256 rows, Eq. (1)-(2) scores of 32 Sparse-Q queries, attention of 384 rows) and
+#                 scatter of 1024 rows, Eq. (1)-(2) scores of 96 Sparse-Q queries, attention of 1152 rows) and
 #                 scaled to the whole step by the exact algorithmic work: sum_{i in I_nr} (i+1) for the scores,
 #                 sum_{r in R} (r+1) for the attention with R = the oracle's own recompute set
 #                 (tests/golden/rows_C3_L3.txt for the C3 stack; k evenly spread rows otherwise), T (T+1) / 2 for
 #                 full layers. value = (fraction of the step's work the sample covers) x tokens x layers / time.
 
-SAMPLE_Q, SAMPLE_ROWS, SAMPLE_SCATTER = 32, 384, 256
+SAMPLE_Q, SAMPLE_ROWS, SAMPLE_SCATTER = 96, 1152, 1024   # ~7 s of oracle time on 16 cores (10-30 s with the measured legs)
 
 
 def _oracle_layer_timed(orc, lay, lt, reqs):
