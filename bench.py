@@ -858,7 +858,6 @@ class CpuSample:
         self.nidx = nidx
         self.t_req = int(lay.seq_len[0])
         self.q_samp = nidx[np.unique(np.linspace(0, len(nidx) - 1, min(SAMPLE_Q, len(nidx))).astype(int))]
-        self.rows = np.unique(np.linspace(0, self.t_req - 1, min(SAMPLE_ROWS, self.t_req)).astype(np.int32))
         self.sc_rows = nidx[:SAMPLE_SCATTER]
         self.o = o
         # exact algorithmic work of the whole step, in (row, key) pairs
@@ -877,6 +876,9 @@ class CpuSample:
                 self.w_sparse += float(np.sum(nn + 1)) + k * (t / 2.0)
                 self.n_rows += len(nn) + k
             self.rows_src = "I_nr + k evenly spread cached rows (cost model)"
+        # (a small config is not over-sampled: never more attention rows than one request of the step computes)
+        n_samp = min(SAMPLE_ROWS, self.t_req, max(1, self.n_rows // lay.num_reqs))
+        self.rows = np.unique(np.linspace(0, self.t_req - 1, n_samp).astype(np.int32))
 
     def run(self):
         """One timed sample. Returns (whole-step seconds extrapolated, sample seconds, per-stage estimate)."""
