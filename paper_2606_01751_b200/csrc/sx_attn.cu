@@ -72,6 +72,24 @@ struct AttnParams {
   const int32_t *zc_page_seg;
 };
 
+// ---- optional per-CTA phase trace (build with -DSX_ATTN_TRACE: `SX_NVCC_FLAGS=-DSX_ATTN_TRACE python -m
+// paper_2606_01751_b200.build --force`; read with paper_2606_01751_b200/trace_attn.py). clock64() stamps of the first
+// 2048 CTAs of the LAST attention launch: [0] entry, [1] after griddepcontrol.wait, [2] lookups done, [3] after the
+// block-wide meeting, [4] warp 8: first block-table entries loaded, [5] warp 8: Q and key tile 0 issued, [6] issuer: Q
+// landed, [7] issuer: K(0) landed, [8] softmax warp 0: first S tile, [9] warp 0: key loop done, [10] warp 0: output
+// stored, [11] warp 0: exit, [12] SM id, [13] key tiles. Compiles to nothing without the flag.
+#ifdef SX_ATTN_TRACE
+__device__ long long sx_attn_trace[2048 * 16];
+extern "C" int sx_attn_trace_copy(void *host) {
+  return (int)cudaMemcpyFromSymbol(host, sx_attn_trace, sizeof(sx_attn_trace));
+}
+#define SX_TR(k) do { if (blockIdx.x < 2048 && (threadIdx.x & 31) == 0) sx_attn_trace[blockIdx.x * 16 + (k)] = clock64(); } while (0)
+#define SX_TRW(k, w) do { if (warp == (w)) SX_TR(k); } while (0)
+#else
+#define SX_TR(k) do {} while (0)
+#define SX_TRW(k, w) do {} while (0)
+#endif
+
 struct AttnCfg {
   static constexpr int kOffQ = 0;                                  // 2 query tiles
   static constexpr int kOffKV = kOffQ + 2 * kTileBytes;            // ring
@@ -128,6 +146,7 @@ attn_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_constant__ CU
 
   // ---- prologue that touches no global memory: it may overlap the tail of the previous kernel in the stream
   // (programmatic dependent launch); the next kernel's prologue may in turn overlap this kernel
+  SX_TRW(0, 0);
   griddep_launch();
   if (warp == kWarpProd0 && lane == 0) {
     tma_prefetch_desc(&tm_q);
@@ -172,6 +191,7 @@ attn_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_constant__ CU
     fence_proxy_async_smem();
   }
   griddep_wait();  // from here on: global memory (row lists, tables, pools may be outputs of the previous kernel)
+  SX_TRW(1, 0);
 
   // ---- which (request, KV head, pair of row tiles) is this CTA; heavy (late) pairs of a request first
   // consecutive blocks share a (request, KV head, row pair) and take one key split each
@@ -279,8 +299,10 @@ attn_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_constant__ CU
       const int cta_rows = pair >= 0 ? min(rpc, n_r - pair * rpc) : 0;
       if (lane == 0) issue_q(cta_rows > rpt ? 2 : 1);
       const int blk_k = lane < n_boxes ? table_entry(0, 0) : 0, blk_v = lane < n_boxes ? table_entry(1, 0) : 0;
+      SX_TR(4);
       issue_item(0, blk_k);
       issue_item(1, blk_v);
+      SX_TR(5);
       blk_ahead = lane < n_boxes ? table_entry(2, 0) : 0;  // (clamped to a valid page if there is no key tile 1)
     }
   }
@@ -324,6 +346,7 @@ attn_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_constant__ CU
     fence_mbar_init();
   }
 
+  SX_TRW(2, 0);
   tc_fence_before();
   if (kPair) {
     if (warp != kWarpProd0) {
@@ -338,6 +361,15 @@ attn_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_constant__ CU
   }
   tc_fence_after();
   const uint32_t tmem = bars->tmem_base;
+  SX_TRW(3, 0);
+#ifdef SX_ATTN_TRACE
+  if (threadIdx.x == 0 && blockIdx.x < 2048) {
+    unsigned smid;
+    asm volatile("mov.u32 %0, %%smid;" : "=r"(smid));
+    sx_attn_trace[blockIdx.x * 16 + 12] = smid;
+    sx_attn_trace[blockIdx.x * 16 + 13] = n_tiles;
+  }
+#endif
 
   if (!active) {
     // nothing to do (grid overshoot): fall through to the common exit
@@ -388,6 +420,7 @@ attn_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_constant__ CU
           if (kPair) mbar_wait_cluster(bar, parity); else mbar_wait(bar, parity);
         };
         mbar_wait(&bars->q_full, 0);
+        SX_TR(6);
         // keys [64h, 64h + 64) of the tile in `slot` -> columns [64h, 64h + 64) of S_i, no commit
         auto issue_qk_half = [&](int i, int slot, int h) {
           const uint32_t qd = q_lo + (uint32_t)i * (kTileBytes >> 4);
@@ -408,6 +441,7 @@ attn_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_constant__ CU
           if (n_tiles > 0) {  // (a key split may hold no tile of this CTA's rows)
             mbar_wait(kZc ? &bars->k_rot[0] : &bars->kv_full[0], 0);
             tc_fence_after();
+            SX_TR(7);
 #pragma unroll
             for (int i = 0; i < 2; ++i) {
               if (n_t[i] > 0) {
@@ -532,6 +566,7 @@ attn_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_constant__ CU
       }
       mbar_wait(&bars->s_full[qt], t & 1);
       tc_fence_after();
+      if (t == 0) SX_TRW(8, 0);
       // S row -> registers in two waves so that the maximum of the first 64 columns is formed while the
       // second 64 are still in flight
       uint32_t sr[4][32];
@@ -674,6 +709,7 @@ attn_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_constant__ CU
       l = l * alpha + radd;
     }
 
+    SX_TRW(9, 0);
     // ---- epilogue
     const size_t out_row = (size_t)grow * p.num_q_heads + kvh * g + hh;
     if (p.kv_splits > 1) {
@@ -760,6 +796,7 @@ attn_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_constant__ CU
       }
       if (p.lse && valid) p.lse[out_row] = m_used * p.scale + logf(l);
     }
+    SX_TRW(10, 0);
   }
 
   tc_fence_before();
@@ -770,6 +807,7 @@ attn_kernel(const __grid_constant__ CUtensorMap tm_q, const __grid_constant__ CU
     __syncthreads();
     if (warp == kWarpMma) tmem_dealloc(tmem, 512);
   }
+  SX_TRW(11, 0);
 }
 
 // Row sets that fill tensor-core tiles but only a few CTAs (a handful of query tiles against a long context):
